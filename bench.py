@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py -- one planning step of VOiLA's hot path on synthetic, seeded inputs.
+
+A "step" is one pass of the whole hot path over one batch: voila_rollout_values on P particles x
+Q action sequences x horizon H, then voila_belief_update on N particles (SURVEY.md 8(a) rows
+R1-R11).  metric = rollout steps/s = P*Q*H*n_gpus / step time, with the belief-update latency and
+per-kernel times alongside.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl voila|reference]
+
+Multi-GPU (torchrun): the path does not shard (north_star: one GPU, no collectives) -> every rank
+runs an independent replica ("replicas only"); value = units of all ranks / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+DEFAULT_CONFIG = 2
+METRIC = "rollout_steps_per_sec"
+UNIT = "particle*sequence*depth steps/s"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_burst": d["bf16_tflops"],
+                "bf16_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "src": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index = index
+        self.rows = []
+        self.stop_flag = False
+        self.proc = None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+                if self.stop_flag:
+                    break
+        except Exception:
+            pass
+
+    def finish(self):
+        self.stop_flag = True
+        if self.proc is not None:
+            try:
+                self.proc.terminate()
+            except Exception:
+                pass
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"], f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _flops_fp32_peak_tflops(sm_count, sm_mhz):
+    # 4 SMSPs x 32 FFMA lanes x 2 flop per SM per clock (B300_MICROARCH.md "Pipe rates")
+    return sm_count * 128 * 2 * sm_mhz * 1e6 / 1e12
+
+
+def _oracle_sample(cfg, model, inp, target_s=12.0):
+    """Times the oracle (as it stands) on a bounded sample of the workload: all P particles x Q'
+    sequences x H plus a belief update on N*Q'/Q particles; returns (steps/s, cores, description)."""
+    from oracle import voila_oracle as oracle
+    from paper_2606_19729_b200 import synth
+    bf16 = model.prec == synth.PREC_BF16
+    parts = synth.bf16_round_np(inp.particles) if bf16 else inp.particles
+    bu_parts = synth.bf16_round_np(inp.bu_particles) if bf16 else inp.bu_particles
+    om = oracle.OracleModel(model)
+    cores = oracle.num_threads()
+    P, (Q, H) = parts.shape[0], inp.action_seqs.shape
+    # probe: one sequence per thread on a particle subset
+    Pp = min(P, 64)
+    qp = min(Q, cores)
+    t0 = time.perf_counter()
+    om.rollout_values(parts[:Pp], inp.action_seqs[:qp], None, 1)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    rate = Pp * qp * H / dt
+    want = rate * target_s
+    Ps = P if want >= P * H * qp else max(Pp, int(want / (H * qp)))
+    Qs = int(min(Q, max(qp, (want / (Ps * H)) // qp * qp)))
+    Ns = max(1, int(round(bu_parts.shape[0] * (Ps * Qs) / (P * Q))))
+    t0 = time.perf_counter()
+    om.rollout_values(parts[:Ps], inp.action_seqs[:Qs], None, 1)
+    om.belief_update(bu_parts[:Ns], inp.bu_action, inp.observation,
+                     None if inp.bu_weights is None else inp.bu_weights[:Ns], 2)
+    dt = time.perf_counter() - t0
+    desc = (f"{Ps} of {P} particles x {Qs} of {Q} sequences x H={H} rollout + belief update on "
+            f"{Ns} of {bu_parts.shape[0]} particles, {dt:.1f} s")
+    return Ps * Qs * H / dt, cores, desc, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    from paper_2606_19729_b200 import synth
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = synth.CONFIGS[args.config]
+    model = synth.make_model(cfg)
+    inp = synth.make_inputs(cfg)
+    n = args.warmup + args.steps
+    per = max(2.0, min(20.0, 150.0 / n))
+    vals, times, desc, cores = [], [], "", 0
+    for i in range(n):
+        v, cores, desc, dt = _oracle_sample(cfg, model, inp, target_s=per)
+        if i >= args.warmup:
+            vals.append(v)
+            times.append(dt)
+    value = float(np.mean(vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "P": cfg.P, "Q": cfg.Q, "H": cfg.H, "N": cfg.N,
+                   "note": "each step is a bounded sample of the workload (see cpu_baseline.sample)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_voila(args):
+    import torch
+
+    import paper_2606_19729_b200 as vl
+    from paper_2606_19729_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    cfg = synth.CONFIGS[args.config]
+    model = synth.make_model(cfg)
+    inp = synth.make_inputs(cfg)
+    P, Q, H, N = cfg.P, cfg.Q, cfg.H, cfg.N
+    ctx = vl.Voila(model, device=local)
+    if args.kernel != "auto":
+        ctx.voila_set_kernel(vl.KERNEL_FFMA if args.kernel == "ffma" else vl.KERNEL_TCGEN05)
+    ctx.voila_reserve(P, Q, H, N)
+    chain = N == P  # the belief update's output particles are the next step's rollout particles
+    parts = ctx.to_particles(inp.particles)
+    bu_parts = parts if chain else ctx.to_particles(inp.bu_particles)
+    seqs = torch.from_numpy(inp.action_seqs).to(dev)
+    obs_all = torch.from_numpy(synth.observations_for_steps(cfg, args.warmup + args.steps + 1)).to(dev)
+    bu_w = None if inp.bu_weights is None else torch.from_numpy(inp.bu_weights).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    stream = torch.cuda.current_stream(dev)
+    seed0 = 20260619
+
+    state = {"parts": parts, "bu_parts": bu_parts}
+
+    def step(k):
+        out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * k, want_witness=True)
+        bu = ctx.voila_belief_update(state["bu_parts"], inp.bu_action, obs_all[k], bu_w,
+                                     seed0 + 2 * k + 1, want_debug=False)
+        if chain:
+            state["parts"] = state["bu_parts"] = bu["particles"]
+        return out, bu
+
+    for k in range(args.warmup):
+        step(k)
+    torch.cuda.synchronize(dev)
+    ctx.voila_set_profiling(True)
+    for w in range(4):
+        ctx.voila_profile_read(w)
+    launches0 = ctx.voila_launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.25)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True),
+           torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)  # evict L2 between timed iterations (outside the event pairs)
+        ev[k][0].record(stream)
+        out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * (k + args.warmup))
+        ev[k][1].record(stream)
+        bu = ctx.voila_belief_update(state["bu_parts"], inp.bu_action, obs_all[k + args.warmup], bu_w,
+                                     seed0 + 2 * (k + args.warmup) + 1, want_debug=False)
+        ev[k][2].record(stream)
+        if chain:
+            state["parts"] = state["bu_parts"] = bu["particles"]
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.finish() if sampler else None
+    launches = ctx.voila_launch_count() - launches0
+    roll_ms = [a.elapsed_time(b) for a, b, _ in ev]
+    bu_ms = [b.elapsed_time(c) for _, b, c in ev]
+    total_ms = float(sum(roll_ms) + sum(bu_ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    kt = [ctx.voila_profile_read(w) for w in range(4)]
+    ctx.voila_set_profiling(False)
+    assert int(bu["status"].item()) == 0 and bool(torch.isfinite(out["values"]).all())
+    ms_per_step = total_ms / args.steps
+    value = world * P * Q * H / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer C-ABI entry points (pinned host memory) ----
+    esize = 2 if ctx.prec == vl.PREC_BF16 else 4
+    h_parts = parts.cpu().pin_memory()
+    h_bu = h_parts if chain else bu_parts.cpu().pin_memory()
+    h_seqs = torch.from_numpy(inp.action_seqs).pin_memory()
+    h_obs = obs_all.cpu().pin_memory()
+    h_w = None if bu_w is None else bu_w.cpu().pin_memory()
+    h_vals = torch.empty(Q, dtype=torch.float32).pin_memory()
+    h_pout = torch.empty_like(h_bu).pin_memory()
+    h_anc = torch.empty(N, dtype=torch.int32).pin_memory()
+    h_le = torch.empty(1, dtype=torch.float32).pin_memory()
+    h_st = torch.empty(1, dtype=torch.int32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+
+    def e2e_step(k):
+        ctx.voila_rollout_values_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals)
+        ctx.voila_belief_update_host(h_bu, inp.bu_action, h_obs[k % h_obs.shape[0]], h_w,
+                                     seed0 + 2 * k + 1, h_pout, None, h_anc, h_le, h_st)
+
+    e2e_step(0)
+    torch.cuda.synchronize(dev)
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for k in range(e2e_steps):
+        e2e_step(k + 1)
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = P * cfg.S * esize + Q * H * 4 + N * cfg.S * esize + cfg.O * 4 + (N * 4 if h_w is not None else 0)
+    d2h = Q * 4 + N * cfg.S * esize + N * 4 + 8
+    e2e = {"value": world * P * Q * H * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+           "api": "voila_rollout_values_host + voila_belief_update_host"}
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel (the rollout kernel), from the library's event pairs ----
+    peaks = _peaks()
+    flop_step = synth.flops_per_rollout_step(model, algorithmic=True)
+    k_ms = float(np.mean(kt[0])) if kt[0] else float(np.mean(roll_ms))
+    achieved = P * Q * H * flop_step / (k_ms * 1e-3) / 1e12
+    if ctx.prec == vl.PREC_BF16 and "tc" in ctx.voila_last_rollout_kernel():
+        long_step = ms_per_step > 500.0
+        peak = peaks["bf16_sustained"] if long_step else peaks["bf16_burst"]
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": None,
+                "peak_kind": f"bf16 {'sustained' if long_step else 'burst'}, {peaks['src']}"}
+    else:
+        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+        mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        peak = _flops_fp32_peak_tflops(sm_count, mhz)
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "frac": achieved / peak, "traffic": None,
+                "peak_kind": "fp32 FFMA: SMs x 128 lanes x 2 flop x max SM clock (CUDA-core kernel)"}
+    roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
+                 "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
+                 "share_of_step": k_ms / ms_per_step})
+    # HBM-bound tail of the belief update (scan + resample/gather), algorithmic bytes per particle
+    row = cfg.S * esize
+    bytes_resample = N * (8 + 2 * row + 4 + 4)      # CDF read, row gather, row write, index, weight
+    bytes_scan = N * (4 + 8)                        # logit read, CDF write
+    belief = {"latency_us": 1e3 * float(np.mean(bu_ms)),
+              "propose_score_us": 1e3 * float(np.mean(kt[1])) if kt[1] else None,
+              "scan_us": 1e3 * float(np.mean(kt[2])) if kt[2] else None,
+              "resample_gather_us": 1e3 * float(np.mean(kt[3])) if kt[3] else None}
+    if kt[3]:
+        gbs = bytes_resample / (np.mean(kt[3]) * 1e-3) / 1e9
+        belief["resample_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"],
+                                       "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                                       "bytes_per_particle": bytes_resample / N}
+    if kt[2]:
+        gbs = bytes_scan / (np.mean(kt[2]) * 1e-3) / 1e9
+        belief["scan_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"],
+                                   "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                                   "bytes_per_particle": bytes_scan / N}
+
+    cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if ctx.prec == vl.PREC_BF16 else "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "P": P, "Q": Q, "H": H, "N": N, "S": cfg.S, "O": cfg.O,
+                   "A": cfg.A, "Nz": cfg.Nz, "hidden": cfg.hidden, "parallelism": "replicas only",
+                   "l2": "flushed between timed iterations (256 MiB write)",
+                   "chained_belief": chain},
+        "rollout_ms": float(np.mean(roll_ms)), "belief_update": belief,
+        "roofline": roof,
+        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="voila", choices=["voila", "reference"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "ffma", "tcgen05"])
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "voila":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_voila(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,221 @@
+/*
+ * voila.h -- C ABI of libvoila: the data-parallel hot path of VOiLA's online planner on one B200.
+ *
+ * Paper: "VOiLA: Vectorized Online Planning with Learned Diffusion Models for POMDP Agents"
+ * (arxiv/paper_2606_19729; citations are lines of /root/reference/PAPER.md).  The two hot calls:
+ *
+ *   voila_rollout_values  -- Monte-Carlo evaluation of candidate action sequences: every belief
+ *       particle x every sequence is rolled forward through the distilled generators
+ *       s' = f_T(s, a, w_T) (Eq.2) and o = f_Z(s', a, w_Z) (Eq.5, PAPER.md:124;
+ *       "given batched states and actions"), the discounted return
+ *       sum_t gamma^t R(s_t, a_t) is accumulated and averaged over the belief
+ *       (Monte-Carlo estimate of R(b,a)).
+ *   voila_belief_update   -- one step of the SIR particle filter that tracks the belief
+ *       b'(s') ~ Z(s',a,o) sum_s T(s,a,s') b(s): propose with f_T, weight with
+ *       exp(l(s',a,o)/lambda), normalise, resample.
+ *
+ * Everything the paper leaves open (two-tower l, Philox keying, exact-integer systematic
+ * resampling, reward forms, bf16 mode) is fixed in DESIGN.md "Readings of the paper".
+ *
+ * Conventions
+ *   - No torch / CUDA types in any signature: device pointers are plain pointers, the stream is a
+ *     `void*` holding a cudaStream_t (NULL = legacy default stream).
+ *   - "dev" = pointer to device memory on the ctx's GPU, "host" = pointer to host memory.
+ *   - The caller owns every buffer it passes; the library owns only the ctx (packed weights and
+ *     the workspace reserved with voila_reserve).  Hot calls never allocate.
+ *   - Device entry points are asynchronous and stream-ordered; *_host entry points copy in, run,
+ *     copy out and synchronise the stream before returning.
+ *   - Particle state buffers are fp32 when the ctx was created with VOILA_PREC_FP32 and bf16
+ *     (16-bit patterns) with VOILA_PREC_BF16; weights, values, observations are always fp32;
+ *     indices are int32.  All dev pointers must be 16-byte aligned.
+ *   - Results are a pure function of (inputs, seed): no hidden RNG state, no float atomics;
+ *     repeated calls are bit-identical.
+ *   - Errors found on the host return a status and enqueue nothing.  Conditions only the device can
+ *     see (all weights zero, non-finite scores) set *dev_status_out != 0.
+ *   - There is no CPU fallback: without a usable sm_100 device voila_create fails.
+ */
+#ifndef VOILA_H_
+#define VOILA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default) /* the library is built with -fvisibility=hidden */
+#endif
+
+typedef struct voila_ctx voila_ctx; /* opaque */
+
+typedef enum {
+    VOILA_OK = 0,
+    VOILA_ERR_INVALID_ARG = 1, /* NULL / non-positive size / action out of range / misaligned pointer */
+    VOILA_ERR_UNSUPPORTED = 2, /* no sm_100 device, or model dims over the kernels' limits */
+    VOILA_ERR_CUDA = 3,        /* a CUDA runtime call failed; see voila_last_cuda_error */
+    VOILA_ERR_WORKSPACE = 4    /* sizes exceed what voila_reserve was given */
+} voila_status;
+
+typedef enum { VOILA_ACT_NONE = 0, VOILA_ACT_RELU = 1, VOILA_ACT_SILU = 2 } voila_act;
+typedef enum { VOILA_PREC_FP32 = 0, VOILA_PREC_BF16 = 1 } voila_prec;
+
+/* A feed-forward network y = W_L act(... act(W_1 x + b_1) ...) + b_L (hidden activation `act`,
+ * output layer linear).  Used for f_T, f_Z and the likelihood towers. */
+typedef struct {
+    int n_layers;            /* 1..8 affine layers */
+    const int *dims;         /* host [n_layers+1]: dims[0] input width ... dims[n_layers] output */
+    const float *const *W;   /* host [n_layers] pointers; W[l] is [dims[l+1]][dims[l]] row-major */
+    const float *const *b;   /* host [n_layers] pointers; b[l] is [dims[l+1]] */
+    int act;                 /* voila_act */
+} voila_mlp;
+
+/* R(s,a) (bounded reward on the current state-action).  DESIGN.md reading R14. */
+typedef enum {
+    VOILA_R_NEG_L2_GOAL = 0,   /* -||s - goal||_2        param = goal[S]            */
+    VOILA_R_NEG_QUADRATIC = 1, /* -s^T M s               param = M[S][S] row-major  */
+    VOILA_R_LINEAR = 2         /* c^T s + c0             param = c[S+1] (c0 last)   */
+} voila_reward_kind;
+
+typedef struct {
+    int kind;                  /* voila_reward_kind */
+    const float *param;        /* host, see above */
+    const float *action_cost;  /* host [n_actions], added to R; or NULL */
+} voila_reward;
+
+typedef struct {
+    int state_dim;   /* S */
+    int obs_dim;     /* O */
+    int n_actions;   /* A: discrete actions, one-hot encoded */
+    int noise_dim;   /* Nz: w_T, w_Z ~ N(0, I_Nz) */
+    voila_mlp f_T;        /* [S + A + Nz] -> ... -> S ; input order [s ; onehot(a) ; w] */
+    voila_mlp f_Z;        /* [S + A + Nz] -> ... -> O ; evaluated on the successor state */
+    voila_mlp lik_obs;    /* f : O -> ... -> d   (observation tower of l = <f(o), g(s')>) */
+    voila_mlp lik_state;  /* g : S (+A if lik_action_cond) -> ... -> d */
+    int lik_action_cond;  /* 0 | 1: append onehot(a) to g's input (PAPER.md:128 writes l(s',a,o)) */
+    float lik_temperature; /* lambda > 0: weights are exp(l / lambda) */
+    float discount;        /* gamma in (0, 1] */
+    voila_reward reward;
+    int prec;              /* voila_prec */
+} voila_model_desc;
+
+/* Which kernel family runs the generator MLPs (for tests and benchmarks; default AUTO). */
+typedef enum {
+    VOILA_KERNEL_AUTO = 0,   /* tcgen05 path when prec == BF16 and the dims fit it, else FFMA */
+    VOILA_KERNEL_FFMA = 1,   /* CUDA-core path (fp32 mode; in bf16 mode rounds operands to bf16) */
+    VOILA_KERNEL_TCGEN05 = 2 /* tensor-core path only; UNSUPPORTED if the dims do not fit */
+} voila_kernel;
+
+/* Copies and packs the host weights onto `device`.  Fails with VOILA_ERR_UNSUPPORTED when the
+ * device is not compute capability 10.x or a layer is wider than the kernels handle.  *out is set
+ * only on VOILA_OK. */
+voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **out);
+void voila_destroy(voila_ctx *ctx);
+
+/* Bytes of device workspace needed for rollouts of P particles x Q sequences x H steps and belief
+ * updates of N particles (any of them may be 0). */
+size_t voila_workspace_bytes(const voila_ctx *ctx, int P, int Q, int H, int N);
+/* (Re)allocates the ctx-owned workspace (and, for the *_host entry points, staging buffers) for
+ * those maximum sizes.  Not a hot call: synchronises the device. */
+voila_status voila_reserve(voila_ctx *ctx, int P, int Q, int H, int N);
+
+voila_status voila_set_kernel(voila_ctx *ctx, int kernel /* voila_kernel */);
+/* 1 if the tcgen05 rollout / belief kernels support this ctx's dims, else 0. */
+int voila_tcgen05_supported(const voila_ctx *ctx);
+
+/*
+ * V_q = sum_p wbar_p sum_{t<H} gamma^t R(s_t, a_{q,t}),  s_0 = particles[p],
+ * s_{t+1} = f_T(s_t, a_{q,t}, w_T(p,q,t)),  o_{t+1} = f_Z(s_{t+1}, a_{q,t}, w_Z(p,q,t)),
+ * wbar_p = weights[p] / sum weights   (O4).
+ *   particles        dev [P][S]   fp32 | bf16 (see prec)
+ *   action_seqs      dev [Q][H]   int32 in [0, A)   (values are not range-checked on the device)
+ *   weights          dev [P] fp32 >= 0, unnormalised; NULL = uniform
+ *   seed             keys the Philox4x32-10 noise: counter (p, q, t, stream<<16 | block)
+ *   values_out       dev [Q] fp32
+ *   obs_witness_out  dev [Q][O] fp32 or NULL: sum_p wbar_p sum_t gamma^t o_{t+1} (R10)
+ *   returns_out      dev [Q][P] fp32 or NULL: per-(q,p) discounted return (tests)
+ *   final_states_out dev [Q][P][S] fp32 or NULL: s_H of every trajectory (tests)
+ */
+voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
+                                  const int32_t *action_seqs, int Q, int H, const float *weights,
+                                  uint64_t seed, float *values_out, float *obs_witness_out,
+                                  float *returns_out, float *final_states_out, void *cuda_stream);
+
+/*
+ * SIR step (O5):
+ *   s'_i = f_T(s_i, a, w(i)),  L_i = log w_i + <f(o), g(s'_i)> / lambda,  m = max L,
+ *   v_i = exp(L_i - m),  ancestors = systematic resample of v (exact integer definition, O7),
+ *   particles_out[k] = s'_{ancestors[k]},  weights_out[k] = 1/N.
+ *   particles         dev [N][S] fp32 | bf16
+ *   observation       dev [O] fp32
+ *   weights           dev [N] fp32 >= 0 or NULL (uniform)
+ *   particles_out     dev [N][S] same type as particles; must not alias particles
+ *   weights_out       dev [N] fp32 or NULL
+ *   ancestors_out     dev [N] int32 or NULL (non-decreasing)
+ *   post_weights_out  dev [N] fp32 or NULL: v_i (max = 1)
+ *   proposals_out     dev [N][S] same type as particles, or NULL: s'_i before resampling
+ *   log_evidence_out  dev [1] fp32 or NULL: m + log sum v - log sum w
+ *   dev_status_out    dev [1] int32 or NULL: 0 ok; 1 all weights zero or non-finite scores
+ *                     (then ancestors = identity and particles_out = proposals)
+ */
+voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                 const float *observation, const float *weights, uint64_t seed,
+                                 void *particles_out, float *weights_out, int32_t *ancestors_out,
+                                 float *post_weights_out, void *proposals_out,
+                                 float *log_evidence_out, int32_t *dev_status_out,
+                                 void *cuda_stream);
+
+/* Stage-level entry points (so that "indices bit-exact given identical weights" is testable). */
+
+/* ancestors_out[k] = min{ i : N*C_i > k*W + U }, q_i = floor(v_i 2^32), C = inclusive scan of q,
+ * W = C_{N-1}, U = (x0*W) >> 32 with x0 the Philox word of (seed, stream 4).  v dev [N] in [0,1].
+ * dev_status_out as above (1 when every q_i is 0). */
+voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, uint64_t seed,
+                                       int32_t *ancestors_out, int32_t *dev_status_out,
+                                       void *cuda_stream);
+
+/* y = MLP_which(x): which = 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower).
+ * x dev [rows][dims[0]] fp32 (the full input, one-hot block included), y dev [rows][dims[L]] fp32.
+ * Arithmetic follows the ctx precision (bf16 mode rounds weights and layer inputs to bf16). */
+voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
+                               void *cuda_stream);
+
+/* Host-buffer variants: every pointer is HOST memory (pinned for best speed); inputs are copied to
+ * ctx-owned device staging buffers, the device entry point runs, outputs are copied back and the
+ * stream is synchronised.  Optional outputs as above (NULL to skip). */
+voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, int P,
+                                       const int32_t *action_seqs, int Q, int H,
+                                       const float *weights, uint64_t seed, float *values_out,
+                                       float *obs_witness_out, void *cuda_stream);
+voila_status voila_belief_update_host(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                      const float *observation, const float *weights,
+                                      uint64_t seed, void *particles_out, float *weights_out,
+                                      int32_t *ancestors_out, float *log_evidence_out,
+                                      int32_t *status_out, void *cuda_stream);
+
+/* Introspection used by bench.py: number of kernel launches the library has enqueued on this ctx
+ * since creation, and the name / launch geometry of the last rollout kernel. */
+uint64_t voila_launch_count(const voila_ctx *ctx);
+const char *voila_last_rollout_kernel(const voila_ctx *ctx);
+
+/* Kernel timing for bench.py's roofline line.  When profiling is on, the library brackets each
+ * launch of its main kernels with CUDA events on the caller's stream (a ring of 256 pairs per
+ * kernel kind).  voila_profile_read waits for the recorded events of `which`, writes up to max_n
+ * durations in milliseconds (oldest first) to the HOST array ms_out, clears the ring for that
+ * kind and returns how many it wrote.  which: 0 rollout kernel, 1 belief propose+score kernel,
+ * 2 weight scan kernel, 3 resample+gather kernel. */
+typedef enum { VOILA_K_ROLLOUT = 0, VOILA_K_PROPOSE = 1, VOILA_K_SCAN = 2, VOILA_K_RESAMPLE = 3 } voila_kernel_kind;
+voila_status voila_set_profiling(voila_ctx *ctx, int on);
+int voila_profile_read(voila_ctx *ctx, int which, float *ms_out, int max_n);
+
+const char *voila_status_string(voila_status s);
+const char *voila_last_cuda_error(const voila_ctx *ctx);
+int voila_version(void);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOILA_H_ */

@@ -1,0 +1,413 @@
+// mlp_ffma.cu -- CUDA-core path of libvoila: the fp32 parity mode (north_star: relative 1e-4)
+// and a dims-agnostic bf16 mode (operands rounded to bf16, fp32 accumulate) used when the model
+// does not fit the tcgen05 kernels.
+//
+// One CTA = one tile of kTileRows particles of ONE action sequence, so the one-hot action block of
+// the generator input is the same for every row of the tile: it is never multiplied, the column
+// W1[:, S + a_t] is added instead (same sum, same order as the
+// definition since 0*w contributes exactly 0).  Activations live in shared memory transposed
+// ([k][row]) so a thread reads 16 rows of one k with four 128-bit loads; weights are stored
+// transposed ([k][j]) so lanes read consecutive output neurons j.  The horizon loop never touches
+// HBM except for weights (L2-resident).
+#include "voila_device.cuh"
+#include "voila_kernels.h"
+
+namespace voila {
+
+namespace {
+
+constexpr int R = kTileRows;  // 32
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+
+// y[j][r] = act(sum_k Wt[k][j] x[k][r] + b[j]) for the tile's R rows.
+// Rows k in [skip_lo, skip_hi) of the input are skipped (the one-hot block) and row a_row of Wt is
+// added in their place (a_row < 0: nothing added).
+template <bool EMU>
+__device__ __forceinline__ void mlp_layer(const float *__restrict__ Wt, const float *__restrict__ bias,
+                                          int K, int N, int act, bool last, const float *xin,
+                                          float *xout, int skip_lo, int skip_hi, int a_row) {
+    for (int item = threadIdx.x; item < 2 * N; item += kThreads) {
+        const int half = item / N, j = item - half * N;
+        float acc[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[i] = 0.0f;
+        const float *xp = xin + 16 * half;
+        auto fma_row = [&](int k) {
+            const float w = __ldg(Wt + (size_t)k * N + j);
+            const float4 *x4 = reinterpret_cast<const float4 *>(xp + k * R);
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                const float4 x = x4[v];
+                acc[4 * v + 0] = fmaf(w, x.x, acc[4 * v + 0]);
+                acc[4 * v + 1] = fmaf(w, x.y, acc[4 * v + 1]);
+                acc[4 * v + 2] = fmaf(w, x.z, acc[4 * v + 2]);
+                acc[4 * v + 3] = fmaf(w, x.w, acc[4 * v + 3]);
+            }
+        };
+        const int k_end0 = skip_lo < K ? skip_lo : K;
+#pragma unroll 4
+        for (int k = 0; k < k_end0; ++k) fma_row(k);
+        if (a_row >= 0) {
+            const float w = __ldg(Wt + (size_t)a_row * N + j);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i] += w;
+        }
+#pragma unroll 4
+        for (int k = skip_hi; k < K; ++k) fma_row(k);
+        const float bj = __ldg(bias + j);
+        float4 *o4 = reinterpret_cast<float4 *>(xout + j * R + 16 * half);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            float y[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float t = acc[4 * v + i] + bj;
+                if (!last) {
+                    t = act_apply(t, act);
+                    if (EMU) t = bf16_round(t);  // the next layer's operand is bf16
+                }
+                y[i] = t;
+            }
+            o4[v] = make_float4(y[0], y[1], y[2], y[3]);
+        }
+    }
+}
+
+// Input in bufA ([dims[0]][R]); hidden activations ping-pong bufB/bufA; the last layer writes out.
+template <bool EMU>
+__device__ __forceinline__ void mlp_chain(const MlpDev &f, float *bufA, float *bufB, float *out,
+                                          int skip_lo, int skip_hi, int a_row) {
+    float *in = bufA, *other = bufB;
+    for (int l = 0; l < f.n_layers; ++l) {
+        const bool last = (l == f.n_layers - 1);
+        float *dst = last ? out : other;
+        const int K = f.dims[l];
+        mlp_layer<EMU>(f.Wt[l], f.b[l], K, f.dims[l + 1], f.act, last, in, dst,
+                       l == 0 ? skip_lo : K, l == 0 ? skip_hi : K, l == 0 ? a_row : -1);
+        __syncthreads();
+        other = in;
+        in = dst;
+    }
+}
+
+// x[(base + j)][r] = j-th standard normal of (seed; p0 + r, q, t, stream) for j < Nz.
+template <bool EMU>
+__device__ __forceinline__ void fill_noise(float *x, int base, int Nz, uint64_t seed, uint32_t p0,
+                                           uint32_t q, uint32_t t, uint32_t stream) {
+    const int nblk = (Nz + 3) >> 2;
+    for (int idx = threadIdx.x; idx < R * nblk; idx += kThreads) {
+        const int r = idx & (R - 1), blk = idx / R;
+        float z[4];
+        normals4<false>(seed, p0 + r, q, t, stream, blk, z);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (4 * blk + i < Nz) x[(base + 4 * blk + i) * R + r] = EMU ? bf16_round(z[i]) : z[i];
+    }
+}
+
+template <bool EMU>
+__device__ __forceinline__ void copy_state(float *x, const float *s, int S) {
+    for (int idx = threadIdx.x; idx < S * R; idx += kThreads) x[idx] = EMU ? bf16_round(s[idx]) : s[idx];
+}
+
+// R(s, a) for the tile's rows, warps splitting the state index; result (before discounting) is
+// returned by warp 0's lanes (lane = row).  red = [kWarps][R] scratch.
+__device__ __forceinline__ float tile_reward(const RewardDev &rw, int S, const float *s, int a,
+                                             float *red) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float part = 0.0f;
+    if (rw.kind == VOILA_R_NEG_L2_GOAL) {
+        for (int i = warp; i < S; i += kWarps) {
+            const float d = s[i * R + lane] - __ldg(rw.param + i);
+            part = fmaf(d, d, part);
+        }
+    } else if (rw.kind == VOILA_R_NEG_QUADRATIC) {
+        for (int i = warp; i < S; i += kWarps) {
+            float row = 0.0f;
+            for (int j = 0; j < S; ++j) row = fmaf(__ldg(rw.param + i * S + j), s[j * R + lane], row);
+            part = fmaf(s[i * R + lane], row, part);
+        }
+    } else {
+        for (int i = warp; i < S; i += kWarps) part = fmaf(__ldg(rw.param + i), s[i * R + lane], part);
+    }
+    red[warp * R + lane] = part;
+    __syncthreads();
+    float r = 0.0f;
+    if (warp == 0) {
+        float tot = 0.0f;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) tot += red[w * R + lane];
+        if (rw.kind == VOILA_R_NEG_L2_GOAL) r = -sqrtf(tot);
+        else if (rw.kind == VOILA_R_NEG_QUADRATIC) r = -tot;
+        else r = tot + __ldg(rw.param + S);
+        if (rw.action_cost) r += __ldg(rw.action_cost + a);
+    }
+    return r;
+}
+
+template <bool EMU>
+__device__ __forceinline__ void load_particles(const void *particles, int S, int n_rows_total,
+                                               int row0, float *s) {
+    for (int idx = threadIdx.x; idx < S * R; idx += kThreads) {
+        const int r = idx / S, i = idx - r * S;
+        float v = 0.0f;
+        if (row0 + r < n_rows_total) {
+            const size_t g = (size_t)(row0 + r) * S + i;
+            v = EMU ? bf16_to_float(reinterpret_cast<const uint16_t *>(particles)[g])
+                    : reinterpret_cast<const float *>(particles)[g];
+        }
+        s[i * R + r] = v;
+    }
+}
+
+__device__ __forceinline__ double warp_sum_double(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m, const RolloutArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    const int S = m.S, O = m.O, A = m.A, Nz = m.Nz, KW = m.max_width;
+    float *xa = smem, *xb = xa + KW * R, *s = xb + KW * R, *sn = s + S * R, *wit = sn + S * R;
+    float *obs = wit + O * R, *red = obs + O * R, *G = red + kWarps * R;
+    const int tile = blockIdx.x, q = blockIdx.y, p0 = tile * R;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    load_particles<EMU>(a.particles, S, a.P, p0, s);
+    for (int idx = threadIdx.x; idx < O * R; idx += kThreads) wit[idx] = 0.0f;
+    if (threadIdx.x < R) G[threadIdx.x] = 0.0f;
+    __syncthreads();
+
+    float disc = 1.0f;
+    for (int t = 0; t < a.H; ++t) {
+        const int act_t = __ldg(a.action_seqs + (size_t)q * a.H + t);
+        // reward on the CURRENT state (reading R7)
+        const float rew = tile_reward(m.reward, S, s, act_t, red);
+        if (warp == 0) G[lane] = fmaf(disc, rew, G[lane]);
+        // s' = f_T([s ; onehot(a) ; w_T])
+        copy_state<EMU>(xa, s, S);
+        fill_noise<EMU>(xa, S + A, Nz, a.seed, p0, q, t, kStreamRolloutT);
+        __syncthreads();
+        mlp_chain<EMU>(m.mlp[0], xa, xb, sn, S, S + A, S + act_t);
+        // o = f_Z([s' ; onehot(a) ; w_Z])
+        copy_state<EMU>(xa, sn, S);
+        fill_noise<EMU>(xa, S + A, Nz, a.seed, p0, q, t, kStreamRolloutZ);
+        __syncthreads();
+        mlp_chain<EMU>(m.mlp[1], xa, xb, obs, S, S + A, S + act_t);
+        for (int idx = threadIdx.x; idx < O * R; idx += kThreads) wit[idx] = fmaf(disc, obs[idx], wit[idx]);
+        for (int idx = threadIdx.x; idx < S * R; idx += kThreads) s[idx] = sn[idx];
+        disc *= m.gamma;
+        __syncthreads();
+    }
+
+    // weighted partial sums for this (q, tile); fixed order => bit-reproducible
+    const bool valid = (p0 + lane) < a.P;
+    const float wl = valid ? (a.weights ? __ldg(a.weights + p0 + lane) : 1.0f) : 0.0f;
+    if (warp == 0) {
+        const double v = warp_sum_double((double)wl * (double)G[lane]);
+        if (lane == 0) a.part_value[(size_t)q * a.tiles + tile] = v;
+        if (a.returns_out && valid) a.returns_out[(size_t)q * a.P + p0 + lane] = G[lane];
+        red[lane] = wl;
+    }
+    __syncthreads();
+    if (a.part_witness) {
+        for (int i = threadIdx.x; i < O; i += kThreads) {
+            double acc = 0.0;
+            for (int r = 0; r < R; ++r) acc += (double)red[r] * (double)wit[i * R + r];
+            a.part_witness[((size_t)q * a.tiles + tile) * O + i] = acc;
+        }
+    }
+    if (a.final_states_out) {
+        for (int idx = threadIdx.x; idx < S * R; idx += kThreads) {
+            const int r = idx / S, i = idx - r * S;
+            if (p0 + r < a.P) a.final_states_out[((size_t)q * a.P + p0 + r) * S + i] = s[i * R + r];
+        }
+    }
+}
+
+__global__ void weight_sum_kernel(const float *__restrict__ w, int n, double *out) {
+    __shared__ double sh[256];
+    double acc = 0.0;
+    if (w) {
+        for (int i = threadIdx.x; i < n; i += 256) acc += (double)w[i];
+    } else if (threadIdx.x == 0) {
+        acc = (double)n;
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0];
+}
+
+__global__ void rollout_reduce_kernel(const double *__restrict__ part_value,
+                                      const double *__restrict__ part_witness, int tiles, int O,
+                                      const double *__restrict__ wsum, float *values, float *witness) {
+    const int q = blockIdx.x;
+    const double inv = 1.0 / *wsum;
+    for (int i = threadIdx.x; i < O + 1; i += blockDim.x) {
+        double acc = 0.0;
+        if (i == O) {
+            for (int t = 0; t < tiles; ++t) acc += part_value[(size_t)q * tiles + t];
+            values[q] = (float)(acc * inv);
+        } else if (witness) {
+            for (int t = 0; t < tiles; ++t) acc += part_witness[((size_t)q * tiles + t) * O + i];
+            witness[(size_t)q * O + i] = (float)(acc * inv);
+        }
+    }
+}
+
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) mlp_forward_ffma_kernel(const ModelDev m, int which,
+                                                                    const float *__restrict__ x,
+                                                                    int rows, float *y) {
+    extern __shared__ __align__(16) float smem[];
+    const MlpDev &f = m.mlp[which];
+    const int KW = m.max_width, K0 = f.dims[0], NL = f.dims[f.n_layers];
+    float *xa = smem, *xb = xa + KW * R, *out = xb + KW * R;
+    const int row0 = blockIdx.x * R;
+    for (int idx = threadIdx.x; idx < K0 * R; idx += kThreads) {
+        const int r = idx / K0, k = idx - r * K0;
+        float v = (row0 + r < rows) ? x[(size_t)(row0 + r) * K0 + k] : 0.0f;
+        xa[k * R + r] = EMU ? bf16_round(v) : v;
+    }
+    __syncthreads();
+    mlp_chain<EMU>(f, xa, xb, out, K0, K0, -1);
+    for (int idx = threadIdx.x; idx < NL * R; idx += kThreads) {
+        const int r = idx / NL, j = idx - r * NL;
+        if (row0 + r < rows) y[(size_t)(row0 + r) * NL + j] = out[j * R + r];
+    }
+}
+
+// Belief update, stage 1 (O5): proposal s' = f_T(s, a, w), score L = log w + <e, g(s')>/lambda.
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) bu_propose_score_ffma_kernel(const ModelDev m,
+                                                                         const BeliefArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    const int S = m.S, A = m.A, Nz = m.Nz, KW = m.max_width;
+    const MlpDev &g = m.mlp[3];
+    const int d = g.dims[g.n_layers];
+    float *xa = smem, *xb = xa + KW * R, *s = xb + KW * R, *sn = s + S * R, *gout = sn + S * R;
+    const int i0 = blockIdx.x * R;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    load_particles<EMU>(a.particles, S, a.N, i0, s);
+    __syncthreads();
+    copy_state<EMU>(xa, s, S);
+    fill_noise<EMU>(xa, S + A, Nz, a.seed, i0, 0u, 0u, kStreamBeliefT);
+    __syncthreads();
+    mlp_chain<EMU>(m.mlp[0], xa, xb, sn, S, S + A, S + a.action);
+    // the stored particle is what the filter carries forward: in bf16 mode it is bf16(s')
+    for (int idx = threadIdx.x; idx < S * R; idx += kThreads) {
+        const int r = idx / S, i = idx - r * S;
+        if (i0 + r < a.N) {
+            const float v = sn[i * R + r];
+            const size_t gidx = (size_t)(i0 + r) * S + i;
+            if (EMU) reinterpret_cast<uint16_t *>(a.proposals)[gidx] = bf16_bits(v);
+            else reinterpret_cast<float *>(a.proposals)[gidx] = v;
+        }
+    }
+    copy_state<EMU>(xa, sn, S);
+    __syncthreads();
+    if (m.lik_action_cond) mlp_chain<EMU>(g, xa, xb, gout, S, S + A, S + a.action);
+    else mlp_chain<EMU>(g, xa, xb, gout, S, S, -1);
+    if (warp == 0) {
+        float ell = 0.0f;
+        for (int k = 0; k < d; ++k) ell += __ldg(a.e + k) * gout[k * R + lane];
+        const bool valid = (i0 + lane) < a.N;
+        float w = 1.0f, lw = 0.0f;
+        if (a.weights) {
+            w = valid ? __ldg(a.weights + i0 + lane) : 0.0f;
+            lw = w > 0.0f ? logf(w) : -INFINITY;
+        }
+        const float L = lw + ell / m.lambda;
+        int ord = float_to_ordered(valid ? L : -INFINITY);
+        if (valid) a.logits[i0 + lane] = L;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ord = max(ord, __shfl_xor_sync(0xffffffffu, ord, o));
+        const double ws = warp_sum_double(valid ? (double)w : 0.0);
+        if (lane == 0) {
+            atomicMax(a.max_ordered, ord);
+            a.part_wsum[blockIdx.x] = ws;
+        }
+    }
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t bytes) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+}  // namespace
+
+size_t ffma_smem_bytes(const ModelDev &m) {
+    const int d = m.mlp[3].dims[m.mlp[3].n_layers];
+    const size_t rollout = (size_t)(2 * m.max_width + 2 * m.S + 2 * m.O + kWarps + 1) * R * sizeof(float);
+    const size_t belief = (size_t)(2 * m.max_width + 2 * m.S + d) * R * sizeof(float);
+    const size_t fwd = (size_t)(3 * m.max_width) * R * sizeof(float);
+    size_t b = rollout > belief ? rollout : belief;
+    return b > fwd ? b : fwd;
+}
+
+cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cudaStream_t st) {
+    weight_sum_kernel<<<1, 256, 0, st>>>(weights, n, wsum_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rollout_ffma(const ModelDev &m, const RolloutArgs &a, bool bf16, cudaStream_t st) {
+    const size_t smem = ffma_smem_bytes(m);
+    dim3 grid(a.tiles, a.Q);
+    cudaError_t e;
+    if (bf16) {
+        if ((e = set_smem(rollout_ffma_kernel<true>, smem)) != cudaSuccess) return e;
+        rollout_ffma_kernel<true><<<grid, kThreads, smem, st>>>(m, a);
+    } else {
+        if ((e = set_smem(rollout_ffma_kernel<false>, smem)) != cudaSuccess) return e;
+        rollout_ffma_kernel<false><<<grid, kThreads, smem, st>>>(m, a);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rollout_reduce(const RolloutArgs &a, int O, const double *wsum, float *values,
+                                  float *witness, cudaStream_t st) {
+    rollout_reduce_kernel<<<a.Q, 128, 0, st>>>(a.part_value, witness ? a.part_witness : nullptr,
+                                               a.tiles, O, wsum, values, witness);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mlp_forward_ffma(const ModelDev &m, int which, const float *x, int rows, float *y,
+                                    bool bf16, cudaStream_t st) {
+    const size_t smem = ffma_smem_bytes(m);
+    const int grid = (rows + R - 1) / R;
+    cudaError_t e;
+    if (bf16) {
+        if ((e = set_smem(mlp_forward_ffma_kernel<true>, smem)) != cudaSuccess) return e;
+        mlp_forward_ffma_kernel<true><<<grid, kThreads, smem, st>>>(m, which, x, rows, y);
+    } else {
+        if ((e = set_smem(mlp_forward_ffma_kernel<false>, smem)) != cudaSuccess) return e;
+        mlp_forward_ffma_kernel<false><<<grid, kThreads, smem, st>>>(m, which, x, rows, y);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_bu_propose_score_ffma(const ModelDev &m, const BeliefArgs &a, bool bf16,
+                                         cudaStream_t st) {
+    const size_t smem = ffma_smem_bytes(m);
+    const int grid = (a.N + R - 1) / R;
+    cudaError_t e;
+    if (bf16) {
+        if ((e = set_smem(bu_propose_score_ffma_kernel<true>, smem)) != cudaSuccess) return e;
+        bu_propose_score_ffma_kernel<true><<<grid, kThreads, smem, st>>>(m, a);
+    } else {
+        if ((e = set_smem(bu_propose_score_ffma_kernel<false>, smem)) != cudaSuccess) return e;
+        bu_propose_score_ffma_kernel<false><<<grid, kThreads, smem, st>>>(m, a);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace voila

@@ -1,0 +1,602 @@
+// voila_api.cu -- the C ABI of libvoila (include/voila.h): context, weight packing, argument
+// validation, workspace carving and the launch sequences of the two hot calls.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "voila_kernels.h"
+
+using namespace voila;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+float host_bf16_round(float x) {
+    uint32_t u;
+    std::memcpy(&u, &x, 4);
+    if ((u & 0x7f800000u) != 0x7f800000u) {
+        u += 0x7fffu + ((u >> 16) & 1u);
+        u &= 0xffff0000u;
+    }
+    std::memcpy(&x, &u, 4);
+    return x;
+}
+
+voila_status cuda_fail(voila_ctx *ctx, cudaError_t e) {
+    if (ctx) ctx->last_cuda_error = cudaGetErrorString(e);
+    return VOILA_ERR_CUDA;
+}
+
+bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+bool valid_mlp(const voila_mlp &f, int in_dim, int out_dim) {
+    if (f.n_layers < 1 || f.n_layers > kMaxLayers || !f.dims || !f.W || !f.b) return false;
+    if (f.act < VOILA_ACT_NONE || f.act > VOILA_ACT_SILU) return false;
+    for (int l = 0; l <= f.n_layers; ++l)
+        if (f.dims[l] < 1) return false;
+    for (int l = 0; l < f.n_layers; ++l)
+        if (!f.W[l] || !f.b[l]) return false;
+    if (f.dims[0] != in_dim) return false;
+    if (out_dim > 0 && f.dims[f.n_layers] != out_dim) return false;
+    return true;
+}
+
+// Workspace layout for reserved maxima (P, Q, N); all offsets kAlign-aligned.
+struct Layout {
+    size_t wsum, part_value, part_witness, e, proposals, logits, max_ordered, state, tile_flag,
+        tile_agg, tile_incl, tile_sumv, cdf, part_wsum, total;
+};
+
+Layout make_layout(const voila_ctx *ctx, int P, int Q, int N) {
+    Layout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t o = off;
+        off += align_up(bytes > 0 ? bytes : 1);
+        return o;
+    };
+    const size_t tiles = (size_t)(P + kTileRows - 1) / kTileRows;
+    const size_t esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    const size_t stiles = (size_t)scan_tiles(N > 0 ? N : 1);
+    L.wsum = take(sizeof(double));
+    L.part_value = take((size_t)Q * tiles * sizeof(double));
+    L.part_witness = take((size_t)Q * tiles * ctx->O * sizeof(double));
+    L.e = take((size_t)ctx->d * sizeof(float));
+    L.proposals = take((size_t)N * ctx->S * esize);
+    L.logits = take((size_t)N * sizeof(float));
+    L.max_ordered = take(sizeof(int));
+    L.state = take(sizeof(ScanState));
+    L.tile_flag = take(stiles * sizeof(unsigned));
+    L.tile_agg = take(stiles * sizeof(unsigned long long));
+    L.tile_incl = take(stiles * sizeof(unsigned long long));
+    L.tile_sumv = take(stiles * sizeof(double));
+    L.cdf = take((size_t)N * sizeof(unsigned long long));
+    L.part_wsum = take(((size_t)(N + kTileRows - 1) / kTileRows) * sizeof(double));
+    L.total = off;
+    return L;
+}
+
+ScanBuffers scan_buffers(const voila_ctx *ctx, const Layout &L) {
+    uint8_t *w = reinterpret_cast<uint8_t *>(ctx->ws);
+    ScanBuffers sb;
+    sb.state = reinterpret_cast<ScanState *>(w + L.state);
+    sb.tile_flag = reinterpret_cast<unsigned *>(w + L.tile_flag);
+    sb.tile_agg = reinterpret_cast<unsigned long long *>(w + L.tile_agg);
+    sb.tile_incl = reinterpret_cast<unsigned long long *>(w + L.tile_incl);
+    sb.tile_sumv = reinterpret_cast<double *>(w + L.tile_sumv);
+    sb.cdf = reinterpret_cast<unsigned long long *>(w + L.cdf);
+    sb.max_ordered = reinterpret_cast<int *>(w + L.max_ordered);
+    sb.part_wsum = reinterpret_cast<double *>(w + L.part_wsum);
+    return sb;
+}
+
+// Staging layout of the *_host entry points.
+struct Stage {
+    size_t particles, actions, weights, values, witness, obs, particles_out, weights_out, ancestors,
+        scalars, total;
+};
+
+Stage make_stage(const voila_ctx *ctx, int P, int Q, int H, int N) {
+    Stage s{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t o = off;
+        off += align_up(bytes > 0 ? bytes : 1);
+        return o;
+    };
+    const size_t esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    const size_t rows = (size_t)(P > N ? P : N);
+    s.particles = take(rows * ctx->S * esize);
+    s.actions = take((size_t)Q * H * sizeof(int32_t));
+    s.weights = take(rows * sizeof(float));
+    s.values = take((size_t)Q * sizeof(float));
+    s.witness = take((size_t)Q * ctx->O * sizeof(float));
+    s.obs = take((size_t)ctx->O * sizeof(float));
+    s.particles_out = take((size_t)N * ctx->S * esize);
+    s.weights_out = take((size_t)N * sizeof(float));
+    s.ancestors = take((size_t)N * sizeof(int32_t));
+    s.scalars = take(64);
+    s.total = off;
+    return s;
+}
+
+// Brackets one kernel launch with a CUDA event pair when profiling is on.
+struct ProfScope {
+    voila_ctx *ctx;
+    int kind, slot;
+    cudaStream_t st;
+    ProfScope(voila_ctx *c, int k, cudaStream_t s) : ctx(c), kind(k), slot(-1), st(s) {
+        if (!ctx->profiling || ctx->prof_n[kind] >= voila_ctx::kProfRing) return;
+        slot = ctx->prof_n[kind];
+        if (!ctx->prof_ev[kind][slot][0]) {
+            cudaEventCreate(&ctx->prof_ev[kind][slot][0]);
+            cudaEventCreate(&ctx->prof_ev[kind][slot][1]);
+        }
+        cudaEventRecord(ctx->prof_ev[kind][slot][0], st);
+    }
+    ~ProfScope() {
+        if (slot < 0) return;
+        cudaEventRecord(ctx->prof_ev[kind][slot][1], st);
+        ctx->prof_n[kind] = slot + 1;
+    }
+};
+
+bool use_tc(const voila_ctx *ctx) {
+    return ctx->prec == VOILA_PREC_BF16 && ctx->tc != nullptr && ctx->kernel != VOILA_KERNEL_FFMA;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *voila_status_string(voila_status s) {
+    switch (s) {
+        case VOILA_OK: return "ok";
+        case VOILA_ERR_INVALID_ARG: return "invalid argument";
+        case VOILA_ERR_UNSUPPORTED: return "unsupported device or model dimensions";
+        case VOILA_ERR_CUDA: return "CUDA error";
+        case VOILA_ERR_WORKSPACE: return "sizes exceed the reserved workspace (call voila_reserve)";
+    }
+    return "unknown status";
+}
+
+int voila_version(void) { return 100; }
+
+voila_status voila_set_profiling(voila_ctx *ctx, int on) {
+    if (!ctx) return VOILA_ERR_INVALID_ARG;
+    ctx->profiling = on != 0;
+    return VOILA_OK;
+}
+
+int voila_profile_read(voila_ctx *ctx, int which, float *ms_out, int max_n) {
+    if (!ctx || which < 0 || which > 3 || !ms_out || max_n < 0) return 0;
+    DeviceGuard guard(ctx->device);
+    int n = 0;
+    for (int i = 0; i < ctx->prof_n[which] && n < max_n; ++i) {
+        float ms = 0.0f;
+        if (cudaEventSynchronize(ctx->prof_ev[which][i][1]) != cudaSuccess) break;
+        if (cudaEventElapsedTime(&ms, ctx->prof_ev[which][i][0], ctx->prof_ev[which][i][1]) != cudaSuccess) break;
+        ms_out[n++] = ms;
+    }
+    ctx->prof_n[which] = 0;
+    return n;
+}
+
+const char *voila_last_cuda_error(const voila_ctx *ctx) { return ctx ? ctx->last_cuda_error.c_str() : ""; }
+uint64_t voila_launch_count(const voila_ctx *ctx) { return ctx ? ctx->launches : 0; }
+const char *voila_last_rollout_kernel(const voila_ctx *ctx) {
+    return ctx ? ctx->last_rollout_kernel.c_str() : "";
+}
+
+voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **out) {
+    if (!desc || !out) return VOILA_ERR_INVALID_ARG;
+    const int S = desc->state_dim, O = desc->obs_dim, A = desc->n_actions, Nz = desc->noise_dim;
+    if (S < 1 || O < 1 || A < 1 || Nz < 0) return VOILA_ERR_INVALID_ARG;
+    if (desc->prec != VOILA_PREC_FP32 && desc->prec != VOILA_PREC_BF16) return VOILA_ERR_INVALID_ARG;
+    if (!(desc->lik_temperature > 0.0f) || !(desc->discount > 0.0f) || !(desc->discount <= 1.0f))
+        return VOILA_ERR_INVALID_ARG;
+    if (desc->lik_action_cond != 0 && desc->lik_action_cond != 1) return VOILA_ERR_INVALID_ARG;
+    if (!valid_mlp(desc->f_T, S + A + Nz, S) || !valid_mlp(desc->f_Z, S + A + Nz, O) ||
+        !valid_mlp(desc->lik_obs, O, -1) ||
+        !valid_mlp(desc->lik_state, S + (desc->lik_action_cond ? A : 0), -1))
+        return VOILA_ERR_INVALID_ARG;
+    const int d = desc->lik_obs.dims[desc->lik_obs.n_layers];
+    if (d != desc->lik_state.dims[desc->lik_state.n_layers]) return VOILA_ERR_INVALID_ARG;
+    if (desc->reward.kind < VOILA_R_NEG_L2_GOAL || desc->reward.kind > VOILA_R_LINEAR || !desc->reward.param)
+        return VOILA_ERR_INVALID_ARG;
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
+        cudaGetLastError();
+        return VOILA_ERR_UNSUPPORTED;  // no CPU fallback
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return VOILA_ERR_CUDA;
+    if (prop.major != 10) return VOILA_ERR_UNSUPPORTED;  // built for sm_100a only
+
+    voila_ctx *ctx = new (std::nothrow) voila_ctx();
+    if (!ctx) return VOILA_ERR_INVALID_ARG;
+    ctx->device = device;
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->prec = desc->prec;
+    ctx->S = S; ctx->O = O; ctx->A = A; ctx->Nz = Nz; ctx->d = d;
+    DeviceGuard guard(device);
+
+    ModelDev &m = ctx->model;
+    m.S = S; m.O = O; m.A = A; m.Nz = Nz;
+    m.lik_action_cond = desc->lik_action_cond;
+    m.lambda = desc->lik_temperature;
+    m.gamma = desc->discount;
+    m.max_width = 1;
+    const voila_mlp *src[4] = {&desc->f_T, &desc->f_Z, &desc->lik_obs, &desc->lik_state};
+    const bool bf16 = desc->prec == VOILA_PREC_BF16;
+
+    auto upload = [&](const std::vector<float> &h, const float **dst) -> cudaError_t {
+        void *p = nullptr;
+        cudaError_t e = cudaMalloc(&p, h.size() * sizeof(float));
+        if (e != cudaSuccess) return e;
+        ctx->dev_allocs.push_back(p);
+        *dst = reinterpret_cast<const float *>(p);
+        return cudaMemcpy(p, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice);
+    };
+    cudaError_t e = cudaSuccess;
+    for (int w = 0; w < 4 && e == cudaSuccess; ++w) {
+        const voila_mlp &f = *src[w];
+        MlpDev &g = m.mlp[w];
+        g.n_layers = f.n_layers;
+        g.act = f.act;
+        for (int l = 0; l <= f.n_layers; ++l) {
+            g.dims[l] = f.dims[l];
+            if (f.dims[l] > m.max_width) m.max_width = f.dims[l];
+        }
+        for (int l = 0; l < f.n_layers && e == cudaSuccess; ++l) {
+            const int K = f.dims[l], N = f.dims[l + 1];
+            std::vector<float> wt((size_t)K * N), bb(f.b[l], f.b[l] + N);
+            for (int j = 0; j < N; ++j)
+                for (int k = 0; k < K; ++k) {
+                    const float v = f.W[l][(size_t)j * K + k];
+                    wt[(size_t)k * N + j] = bf16 ? host_bf16_round(v) : v;  // k-major: lanes read j
+                }
+            e = upload(wt, &g.Wt[l]);
+            if (e == cudaSuccess) e = upload(bb, &g.b[l]);
+        }
+    }
+    if (e == cudaSuccess) {
+        const int n = desc->reward.kind == VOILA_R_NEG_L2_GOAL ? S
+                      : desc->reward.kind == VOILA_R_NEG_QUADRATIC ? S * S : S + 1;
+        m.reward.kind = desc->reward.kind;
+        e = upload(std::vector<float>(desc->reward.param, desc->reward.param + n), &m.reward.param);
+        m.reward.action_cost = nullptr;
+        if (e == cudaSuccess && desc->reward.action_cost)
+            e = upload(std::vector<float>(desc->reward.action_cost, desc->reward.action_cost + A),
+                       &m.reward.action_cost);
+    }
+    if (e != cudaSuccess) {
+        voila_destroy(ctx);
+        return VOILA_ERR_CUDA;
+    }
+    if (ffma_smem_bytes(m) > (size_t)prop.sharedMemPerBlockOptin) {
+        voila_destroy(ctx);
+        return VOILA_ERR_UNSUPPORTED;
+    }
+    if (bf16) {
+        std::string why;
+        if (tc_supported(desc, &why)) {
+            std::string err;
+            ctx->tc = tc_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
+            if (!ctx->tc) {
+                ctx->last_cuda_error = err;
+                voila_destroy(ctx);
+                return VOILA_ERR_CUDA;
+            }
+        }
+    }
+    *out = ctx;
+    return VOILA_OK;
+}
+
+void voila_destroy(voila_ctx *ctx) {
+    if (!ctx) return;
+    {
+        DeviceGuard guard(ctx->device);
+        cudaDeviceSynchronize();
+        if (ctx->tc) tc_destroy(ctx->tc);
+        for (auto &kind : ctx->prof_ev)
+            for (auto &pair : kind)
+                for (auto &ev : pair)
+                    if (ev) cudaEventDestroy(ev);
+        for (void *p : ctx->dev_allocs) cudaFree(p);
+        if (ctx->ws) cudaFree(ctx->ws);
+        if (ctx->stage) cudaFree(ctx->stage);
+    }
+    delete ctx;
+}
+
+size_t voila_workspace_bytes(const voila_ctx *ctx, int P, int Q, int H, int N) {
+    (void)H;
+    if (!ctx || P < 0 || Q < 0 || N < 0) return 0;
+    return make_layout(ctx, P, Q, N).total;
+}
+
+voila_status voila_reserve(voila_ctx *ctx, int P, int Q, int H, int N) {
+    if (!ctx || P < 0 || Q < 0 || H < 0 || N < 0) return VOILA_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    cudaDeviceSynchronize();
+    const Layout L = make_layout(ctx, P, Q, N);
+    const Stage s = make_stage(ctx, P, Q, H, N);
+    if (ctx->ws) cudaFree(ctx->ws);
+    if (ctx->stage) cudaFree(ctx->stage);
+    ctx->ws = ctx->stage = nullptr;
+    ctx->res_P = ctx->res_Q = ctx->res_H = ctx->res_N = 0;
+    cudaError_t e = cudaMalloc(&ctx->ws, L.total);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->stage, s.total);
+    if (e != cudaSuccess) {
+        if (ctx->ws) cudaFree(ctx->ws);
+        ctx->ws = nullptr;
+        return cuda_fail(ctx, e);
+    }
+    ctx->ws_bytes = L.total;
+    ctx->stage_bytes = s.total;
+    ctx->res_P = P; ctx->res_Q = Q; ctx->res_H = H; ctx->res_N = N;
+    return VOILA_OK;
+}
+
+voila_status voila_set_kernel(voila_ctx *ctx, int kernel) {
+    if (!ctx || kernel < VOILA_KERNEL_AUTO || kernel > VOILA_KERNEL_TCGEN05) return VOILA_ERR_INVALID_ARG;
+    if (kernel == VOILA_KERNEL_TCGEN05 && !ctx->tc) return VOILA_ERR_UNSUPPORTED;
+    ctx->kernel = kernel;
+    return VOILA_OK;
+}
+
+int voila_tcgen05_supported(const voila_ctx *ctx) { return ctx && ctx->tc ? 1 : 0; }
+
+voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
+                                  const int32_t *action_seqs, int Q, int H, const float *weights,
+                                  uint64_t seed, float *values_out, float *obs_witness_out,
+                                  float *returns_out, float *final_states_out, void *cuda_stream) {
+    if (!ctx || !particles || !action_seqs || !values_out || P < 1 || Q < 1 || H < 1)
+        return VOILA_ERR_INVALID_ARG;
+    if (misaligned(particles) || misaligned(action_seqs) || misaligned(weights) ||
+        misaligned(values_out) || misaligned(obs_witness_out) || misaligned(returns_out) ||
+        misaligned(final_states_out))
+        return VOILA_ERR_INVALID_ARG;
+    if (!ctx->ws || P > ctx->res_P || Q > ctx->res_Q) return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const Layout L = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
+    uint8_t *w = reinterpret_cast<uint8_t *>(ctx->ws);
+
+    RolloutArgs a{};
+    a.particles = particles;
+    a.action_seqs = action_seqs;
+    a.weights = weights;
+    a.P = P; a.Q = Q; a.H = H;
+    a.seed = seed;
+    a.part_value = reinterpret_cast<double *>(w + L.part_value);
+    a.part_witness = obs_witness_out ? reinterpret_cast<double *>(w + L.part_witness) : nullptr;
+    a.returns_out = returns_out;
+    a.final_states_out = final_states_out;
+    const int tile_rows = use_tc(ctx) ? 128 : kTileRows;
+    a.tiles = (P + tile_rows - 1) / tile_rows;
+    double *wsum = reinterpret_cast<double *>(w + L.wsum);
+
+    cudaError_t e = launch_weight_sum(weights, P, wsum, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    if (use_tc(ctx)) {
+        int n = 0;
+        ProfScope prof(ctx, VOILA_K_ROLLOUT, st);
+        e = launch_rollout_tc(ctx->tc, ctx->model, a, st, &ctx->last_rollout_kernel, &n);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += n;
+    } else {
+        ProfScope prof(ctx, VOILA_K_ROLLOUT, st);
+        e = launch_rollout_ffma(ctx->model, a, ctx->prec == VOILA_PREC_BF16, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 1;
+        ctx->last_rollout_kernel = ctx->prec == VOILA_PREC_BF16 ? "rollout_ffma_kernel<bf16>"
+                                                                 : "rollout_ffma_kernel<fp32>";
+    }
+    e = launch_rollout_reduce(a, ctx->O, wsum, values_out, obs_witness_out, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    return VOILA_OK;
+}
+
+static voila_status run_resample(voila_ctx *ctx, const ScanBuffers &sb, int N, const void *proposals,
+                                 void *particles_out, float *weights_out, int32_t *ancestors_out,
+                                 cudaStream_t st) {
+    const int esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    ProfScope prof(ctx, VOILA_K_RESAMPLE, st);
+    cudaError_t e = launch_resample_gather(sb, N, proposals, ctx->S * esize, particles_out,
+                                           weights_out, ancestors_out, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    return VOILA_OK;
+}
+
+voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                 const float *observation, const float *weights, uint64_t seed,
+                                 void *particles_out, float *weights_out, int32_t *ancestors_out,
+                                 float *post_weights_out, void *proposals_out,
+                                 float *log_evidence_out, int32_t *dev_status_out, void *cuda_stream) {
+    if (!ctx || !particles || !observation || !particles_out || N < 1) return VOILA_ERR_INVALID_ARG;
+    if (action < 0 || action >= ctx->A) return VOILA_ERR_INVALID_ARG;
+    if (particles_out == particles || proposals_out == particles) return VOILA_ERR_INVALID_ARG;
+    if (misaligned(particles) || misaligned(observation) || misaligned(weights) ||
+        misaligned(particles_out) || misaligned(weights_out) || misaligned(ancestors_out) ||
+        misaligned(post_weights_out) || misaligned(proposals_out))
+        return VOILA_ERR_INVALID_ARG;
+    if (!ctx->ws || N > ctx->res_N) return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const Layout L = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
+    uint8_t *w = reinterpret_cast<uint8_t *>(ctx->ws);
+    const ScanBuffers sb = scan_buffers(ctx, L);
+    const bool bf16 = ctx->prec == VOILA_PREC_BF16;
+    float *e_dev = reinterpret_cast<float *>(w + L.e);
+
+    cudaError_t e = launch_bu_init(sb, N, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    // e = f(o): the observation tower, once (one row through the generic MLP kernel)
+    e = launch_mlp_forward_ffma(ctx->model, 2, observation, 1, e_dev, bf16, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 2;
+
+    BeliefArgs a{};
+    a.particles = particles;
+    a.weights = weights;
+    a.N = N;
+    a.action = action;
+    a.seed = seed;
+    a.e = e_dev;
+    a.proposals = proposals_out ? proposals_out : (void *)(w + L.proposals);
+    a.logits = reinterpret_cast<float *>(w + L.logits);
+    a.max_ordered = sb.max_ordered;
+    a.part_wsum = sb.part_wsum;
+    int n_parts = (N + kTileRows - 1) / kTileRows;
+    if (use_tc(ctx)) {
+        int n = 0;
+        ProfScope prof(ctx, VOILA_K_PROPOSE, st);
+        e = launch_bu_propose_score_tc(ctx->tc, ctx->model, a, st, &n);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += n;
+        n_parts = (N + 127) / 128;
+    } else {
+        ProfScope prof(ctx, VOILA_K_PROPOSE, st);
+        e = launch_bu_propose_score_ffma(ctx->model, a, bf16, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 1;
+    }
+    {
+        ProfScope prof(ctx, VOILA_K_SCAN, st);
+        e = launch_weight_scan(sb, a.logits, N, true, post_weights_out, st);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    e = launch_bu_finalize(sb, N, n_parts, weights != nullptr, seed, log_evidence_out, dev_status_out, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 2;
+    return run_resample(ctx, sb, N, a.proposals, particles_out, weights_out, ancestors_out, st);
+}
+
+voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, uint64_t seed,
+                                       int32_t *ancestors_out, int32_t *dev_status_out,
+                                       void *cuda_stream) {
+    if (!ctx || !v || !ancestors_out || N < 1) return VOILA_ERR_INVALID_ARG;
+    if (misaligned(v) || misaligned(ancestors_out)) return VOILA_ERR_INVALID_ARG;
+    if (!ctx->ws || N > ctx->res_N) return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const Layout L = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
+    const ScanBuffers sb = scan_buffers(ctx, L);
+    cudaError_t e = launch_bu_init(sb, N, st);
+    if (e == cudaSuccess) e = launch_weight_scan(sb, v, N, false, nullptr, st);
+    if (e == cudaSuccess) e = launch_bu_finalize(sb, N, -1, false, seed, nullptr, dev_status_out, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 3;
+    return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st);
+}
+
+voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
+                               void *cuda_stream) {
+    if (!ctx || which < 0 || which > 3 || !x || !y || rows < 1) return VOILA_ERR_INVALID_ARG;
+    if (misaligned(x) || misaligned(y)) return VOILA_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = launch_mlp_forward_ffma(ctx->model, which, x, rows, y, ctx->prec == VOILA_PREC_BF16,
+                                            reinterpret_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    return VOILA_OK;
+}
+
+voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, int P,
+                                       const int32_t *action_seqs, int Q, int H, const float *weights,
+                                       uint64_t seed, float *values_out, float *obs_witness_out,
+                                       void *cuda_stream) {
+    if (!ctx || !particles || !action_seqs || !values_out || P < 1 || Q < 1 || H < 1)
+        return VOILA_ERR_INVALID_ARG;
+    if (!ctx->stage || P > ctx->res_P || Q > ctx->res_Q || H > ctx->res_H) return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const Stage s = make_stage(ctx, ctx->res_P, ctx->res_Q, ctx->res_H, ctx->res_N);
+    uint8_t *g = reinterpret_cast<uint8_t *>(ctx->stage);
+    const size_t esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    cudaError_t e = cudaMemcpyAsync(g + s.particles, particles, (size_t)P * ctx->S * esize,
+                                    cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(g + s.actions, action_seqs, (size_t)Q * H * sizeof(int32_t),
+                            cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && weights)
+        e = cudaMemcpyAsync(g + s.weights, weights, (size_t)P * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    voila_status vs = voila_rollout_values(
+        ctx, g + s.particles, P, reinterpret_cast<const int32_t *>(g + s.actions), Q, H,
+        weights ? reinterpret_cast<const float *>(g + s.weights) : nullptr, seed,
+        reinterpret_cast<float *>(g + s.values),
+        obs_witness_out ? reinterpret_cast<float *>(g + s.witness) : nullptr, nullptr, nullptr, cuda_stream);
+    if (vs != VOILA_OK) return vs;
+    e = cudaMemcpyAsync(values_out, g + s.values, (size_t)Q * sizeof(float), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && obs_witness_out)
+        e = cudaMemcpyAsync(obs_witness_out, g + s.witness, (size_t)Q * ctx->O * sizeof(float),
+                            cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return VOILA_OK;
+}
+
+voila_status voila_belief_update_host(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                      const float *observation, const float *weights, uint64_t seed,
+                                      void *particles_out, float *weights_out, int32_t *ancestors_out,
+                                      float *log_evidence_out, int32_t *status_out, void *cuda_stream) {
+    if (!ctx || !particles || !observation || !particles_out || N < 1) return VOILA_ERR_INVALID_ARG;
+    if (!ctx->stage || N > ctx->res_N) return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const Stage s = make_stage(ctx, ctx->res_P, ctx->res_Q, ctx->res_H, ctx->res_N);
+    uint8_t *g = reinterpret_cast<uint8_t *>(ctx->stage);
+    const size_t esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    const size_t pbytes = (size_t)N * ctx->S * esize;
+    cudaError_t e = cudaMemcpyAsync(g + s.particles, particles, pbytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(g + s.obs, observation, (size_t)ctx->O * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && weights)
+        e = cudaMemcpyAsync(g + s.weights, weights, (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    float *le = reinterpret_cast<float *>(g + s.scalars);
+    int32_t *stat = reinterpret_cast<int32_t *>(g + s.scalars + 16);
+    voila_status vs = voila_belief_update(
+        ctx, g + s.particles, N, action, reinterpret_cast<const float *>(g + s.obs),
+        weights ? reinterpret_cast<const float *>(g + s.weights) : nullptr, seed, g + s.particles_out,
+        weights_out ? reinterpret_cast<float *>(g + s.weights_out) : nullptr,
+        ancestors_out ? reinterpret_cast<int32_t *>(g + s.ancestors) : nullptr, nullptr, nullptr, le, stat,
+        cuda_stream);
+    if (vs != VOILA_OK) return vs;
+    e = cudaMemcpyAsync(particles_out, g + s.particles_out, pbytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && weights_out)
+        e = cudaMemcpyAsync(weights_out, g + s.weights_out, (size_t)N * sizeof(float), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && ancestors_out)
+        e = cudaMemcpyAsync(ancestors_out, g + s.ancestors, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && log_evidence_out)
+        e = cudaMemcpyAsync(log_evidence_out, le, sizeof(float), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && status_out)
+        e = cudaMemcpyAsync(status_out, stat, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return VOILA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,107 @@
+// voila_internal.h -- host-side context and kernel parameter blocks of libvoila.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/voila.h"
+
+namespace voila {
+
+constexpr int kMaxLayers = 8;
+constexpr int kTileRows = 32;  // rows (particles) per CTA in the CUDA-core kernels
+
+// One MLP as the CUDA-core kernels see it: per layer a TRANSPOSED fp32 weight matrix
+// Wt[l] = [dims[l]][dims[l+1]] (k-major so that lanes read consecutive output neurons) and bias.
+struct MlpDev {
+    int n_layers;
+    int act;
+    int dims[kMaxLayers + 1];
+    const float *Wt[kMaxLayers];
+    const float *b[kMaxLayers];
+};
+
+struct RewardDev {
+    int kind;
+    const float *param;        // goal[S] | M[S][S] | c[S+1]
+    const float *action_cost;  // [A] or nullptr
+};
+
+struct ModelDev {
+    int S, O, A, Nz;
+    int lik_action_cond;
+    float lambda, gamma;
+    MlpDev mlp[4];  // 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower)
+    RewardDev reward;
+    int max_width;  // widest activation vector over all four networks (incl. inputs)
+};
+
+struct RolloutArgs {
+    const void *particles;  // [P][S] fp32 | bf16
+    const int32_t *action_seqs;
+    const float *weights;  // or nullptr
+    int P, Q, H;
+    uint64_t seed;
+    double *part_value;    // [Q][tiles]
+    double *part_witness;  // [Q][tiles][O] or nullptr
+    float *returns_out;
+    float *final_states_out;
+    int tiles;
+};
+
+struct BeliefArgs {
+    const void *particles;
+    const float *weights;
+    int N;
+    int action;
+    uint64_t seed;
+    const float *e;        // f(o), [d]
+    void *proposals;       // [N][S] fp32 | bf16
+    float *logits;         // [N]
+    int *max_ordered;      // [1]
+    double *part_wsum;     // [tiles]
+};
+
+// Bookkeeping block of the scan / resample kernels (device memory, zeroed per call by a kernel).
+struct ScanState {
+    unsigned long long total_q;  // W
+    unsigned long long offset_u; // U
+    double sum_v;
+    double sum_w;
+    float max_logit;
+    int status;
+    unsigned int tile_counter;
+    unsigned int pad;
+};
+
+}  // namespace voila
+
+struct voila_ctx {
+    int device = 0;
+    int sm_count = 0;
+    int prec = 0;
+    int kernel = 0;
+    voila::ModelDev model{};      // pointers into dev_blob
+    std::vector<void *> dev_allocs;
+    // workspace
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    int res_P = 0, res_Q = 0, res_H = 0, res_N = 0;
+    // staging for *_host entry points
+    void *stage = nullptr;
+    size_t stage_bytes = 0;
+    // tcgen05 path (opaque here; owned by rollout_tc.cu)
+    void *tc = nullptr;
+    // profiling rings (voila_set_profiling): event pairs per kernel kind
+    bool profiling = false;
+    static constexpr int kProfRing = 256;
+    cudaEvent_t prof_ev[4][kProfRing][2] = {};
+    int prof_n[4] = {0, 0, 0, 0};
+    uint64_t launches = 0;
+    std::string last_rollout_kernel;
+    std::string last_cuda_error;
+    // host copies needed for validation
+    int S = 0, O = 0, A = 0, Nz = 0, d = 0;
+};

@@ -1,0 +1,52 @@
+// voila_kernels.h -- launchers implemented by the .cu files of libvoila (host-callable).
+#pragma once
+#include "voila_internal.h"
+
+namespace voila {
+
+// ---- mlp_ffma.cu : CUDA-core (FFMA) path, any dims; bf16 mode rounds operands to bf16 ----
+size_t ffma_smem_bytes(const ModelDev &m);
+cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cudaStream_t st);
+cudaError_t launch_rollout_ffma(const ModelDev &m, const RolloutArgs &a, bool bf16, cudaStream_t st);
+cudaError_t launch_rollout_reduce(const RolloutArgs &a, int O, const double *wsum, float *values,
+                                  float *witness, cudaStream_t st);
+cudaError_t launch_mlp_forward_ffma(const ModelDev &m, int which, const float *x, int rows, float *y,
+                                    bool bf16, cudaStream_t st);
+cudaError_t launch_bu_propose_score_ffma(const ModelDev &m, const BeliefArgs &a, bool bf16,
+                                         cudaStream_t st);
+
+// ---- belief.cu : normalise, uint64 decoupled-lookback scan, systematic resample + gather ----
+constexpr int kScanTile = 2048;
+struct ScanBuffers {
+    ScanState *state;
+    unsigned int *tile_flag;           // [tiles]
+    unsigned long long *tile_agg;      // [tiles]
+    unsigned long long *tile_incl;     // [tiles]
+    double *tile_sumv;                 // [tiles]
+    unsigned long long *cdf;           // [N]
+    int *max_ordered;                  // [1]
+    double *part_wsum;                 // [bu tiles]
+};
+inline int scan_tiles(int N) { return (N + kScanTile - 1) / kScanTile; }
+cudaError_t launch_bu_init(const ScanBuffers &sb, int N, cudaStream_t st);
+// from_logits: v_i = exp(L_i - max) (belief update) ; else v_i = in[i] (stage-level resampler)
+cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bool from_logits,
+                               float *post_weights_out, cudaStream_t st);
+cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, bool has_prior,
+                               uint64_t seed, float *log_evidence_out, int32_t *dev_status_out,
+                               cudaStream_t st);
+cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *proposals,
+                                   int row_bytes, void *particles_out, float *weights_out,
+                                   int32_t *ancestors_out, cudaStream_t st);
+
+// ---- rollout_tc.cu : tcgen05 / TMEM / bulk-copy path (bf16 mode) ----
+bool tc_supported(const voila_model_desc *desc, std::string *why);
+void *tc_create(const voila_model_desc *desc, int sm_count, std::vector<void *> *allocs,
+                std::string *err);
+void tc_destroy(void *tc);
+cudaError_t launch_rollout_tc(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
+                              std::string *kernel_name, int *n_launches);
+cudaError_t launch_bu_propose_score_tc(void *tc, const ModelDev &m, const BeliefArgs &a,
+                                       cudaStream_t st, int *n_launches);
+
+}  // namespace voila

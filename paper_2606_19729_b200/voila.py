@@ -1,0 +1,325 @@
+"""Thin ctypes binding of libvoila (include/voila.h).  Argument marshalling only: every step of the
+hot path runs in the CUDA kernels behind the C ABI.  torch is used for device memory and streams.
+
+There is NO CPU fallback: if libvoila.so is missing it is built with nvcc; if that fails, or no
+sm_100 device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+KERNEL_AUTO, KERNEL_FFMA, KERNEL_TCGEN05 = 0, 1, 2
+PREC_FP32, PREC_BF16 = 0, 1
+
+# every symbol include/voila.h declares (tests check that the library exports all of them)
+EXPORTS = [
+    "voila_create", "voila_destroy", "voila_workspace_bytes", "voila_reserve", "voila_set_kernel",
+    "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update",
+    "voila_resample_systematic", "voila_mlp_forward", "voila_rollout_values_host",
+    "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel",
+    "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
+    "voila_profile_read",
+]
+
+
+class VoilaError(RuntimeError):
+    pass
+
+
+class _Mlp(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("dims", C.POINTER(C.c_int)),
+                ("W", C.POINTER(C.POINTER(C.c_float))), ("b", C.POINTER(C.POINTER(C.c_float))),
+                ("act", C.c_int)]
+
+
+class _Reward(C.Structure):
+    _fields_ = [("kind", C.c_int), ("param", C.POINTER(C.c_float)),
+                ("action_cost", C.POINTER(C.c_float))]
+
+
+class _ModelDesc(C.Structure):
+    _fields_ = [("state_dim", C.c_int), ("obs_dim", C.c_int), ("n_actions", C.c_int),
+                ("noise_dim", C.c_int), ("f_T", _Mlp), ("f_Z", _Mlp), ("lik_obs", _Mlp),
+                ("lik_state", _Mlp), ("lik_action_cond", C.c_int), ("lik_temperature", C.c_float),
+                ("discount", C.c_float), ("reward", _Reward), ("prec", C.c_int)]
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libvoila.so")
+
+
+def load_library():
+    """dlopen libvoila.so (building it in-tree first if it is missing or stale)."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    from . import build as _build
+    path = _build.build()
+    lib = C.CDLL(path)
+    vp, i32, u64, sz = C.c_void_p, C.c_int, C.c_uint64, C.c_size_t
+    lib.voila_create.argtypes = [C.POINTER(_ModelDesc), i32, C.POINTER(vp)]
+    lib.voila_create.restype = i32
+    lib.voila_destroy.argtypes = [vp]
+    lib.voila_destroy.restype = None
+    lib.voila_workspace_bytes.argtypes = [vp, i32, i32, i32, i32]
+    lib.voila_workspace_bytes.restype = sz
+    lib.voila_reserve.argtypes = [vp, i32, i32, i32, i32]
+    lib.voila_reserve.restype = i32
+    lib.voila_set_kernel.argtypes = [vp, i32]
+    lib.voila_set_kernel.restype = i32
+    lib.voila_tcgen05_supported.argtypes = [vp]
+    lib.voila_tcgen05_supported.restype = i32
+    lib.voila_rollout_values.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp, vp, vp]
+    lib.voila_rollout_values.restype = i32
+    lib.voila_belief_update.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp, vp,
+                                        vp, vp]
+    lib.voila_belief_update.restype = i32
+    lib.voila_resample_systematic.argtypes = [vp, vp, i32, u64, vp, vp, vp]
+    lib.voila_resample_systematic.restype = i32
+    lib.voila_mlp_forward.argtypes = [vp, i32, vp, i32, vp, vp]
+    lib.voila_mlp_forward.restype = i32
+    lib.voila_rollout_values_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp]
+    lib.voila_rollout_values_host.restype = i32
+    lib.voila_belief_update_host.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp,
+                                             vp]
+    lib.voila_belief_update_host.restype = i32
+    lib.voila_launch_count.argtypes = [vp]
+    lib.voila_launch_count.restype = u64
+    lib.voila_last_rollout_kernel.argtypes = [vp]
+    lib.voila_last_rollout_kernel.restype = C.c_char_p
+    lib.voila_status_string.argtypes = [i32]
+    lib.voila_status_string.restype = C.c_char_p
+    lib.voila_last_cuda_error.argtypes = [vp]
+    lib.voila_last_cuda_error.restype = C.c_char_p
+    lib.voila_set_profiling.argtypes = [vp, i32]
+    lib.voila_set_profiling.restype = i32
+    lib.voila_profile_read.argtypes = [vp, i32, C.POINTER(C.c_float), i32]
+    lib.voila_profile_read.restype = i32
+    lib.voila_version.argtypes = []
+    lib.voila_version.restype = i32
+    _LIB = lib
+    return lib
+
+
+def _fptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _pack_mlp(f, keep: list) -> _Mlp:
+    n = len(f.W)
+    dims = (C.c_int * (n + 1))(*[int(d) for d in f.dims])
+    Ws = [np.ascontiguousarray(w, dtype=np.float32) for w in f.W]
+    bs = [np.ascontiguousarray(b, dtype=np.float32) for b in f.b]
+    Wp = (C.POINTER(C.c_float) * n)(*[_fptr(w) for w in Ws])
+    bp = (C.POINTER(C.c_float) * n)(*[_fptr(b) for b in bs])
+    keep.extend([dims, Ws, bs, Wp, bp])
+    return _Mlp(n, C.cast(dims, C.POINTER(C.c_int)), C.cast(Wp, C.POINTER(C.POINTER(C.c_float))),
+                C.cast(bp, C.POINTER(C.POINTER(C.c_float))), int(f.act))
+
+
+def _dptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _hptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+
+
+class Voila:
+    """One libvoila context: packed generator / tower weights on one GPU plus a reserved workspace.
+
+    `model` is duck-typed like synth.ModelSpec (S, O, A, Nz, f_T, f_Z, lik_obs, lik_state each
+    with dims/act/W/b, lik_action_cond, lam, gamma, reward_kind, reward_param, action_cost, prec).
+    All tensors passed to the device entry points are torch CUDA tensors on `device`.
+    """
+
+    def __init__(self, model, device: int = 0, prec: Optional[int] = None):
+        import torch
+        self._torch = torch
+        self.lib = load_library()
+        self.S, self.O, self.A, self.Nz = model.S, model.O, model.A, model.Nz
+        self.prec = int(model.prec if prec is None else prec)
+        self.device = int(device)
+        self.d = int(model.lik_obs.dims[-1])
+        keep: list = []
+        desc = _ModelDesc()
+        desc.state_dim, desc.obs_dim, desc.n_actions, desc.noise_dim = self.S, self.O, self.A, self.Nz
+        desc.f_T = _pack_mlp(model.f_T, keep)
+        desc.f_Z = _pack_mlp(model.f_Z, keep)
+        desc.lik_obs = _pack_mlp(model.lik_obs, keep)
+        desc.lik_state = _pack_mlp(model.lik_state, keep)
+        desc.lik_action_cond = int(model.lik_action_cond)
+        desc.lik_temperature = float(model.lam)
+        desc.discount = float(model.gamma)
+        param = np.ascontiguousarray(model.reward_param, dtype=np.float32).ravel()
+        cost = None if model.action_cost is None else np.ascontiguousarray(model.action_cost, np.float32)
+        keep.extend([param, cost])
+        desc.reward = _Reward(int(model.reward_kind), _fptr(param), _fptr(cost))
+        desc.prec = self.prec
+        h = C.c_void_p()
+        self._h = None
+        self._check(self.lib.voila_create(C.byref(desc), self.device, C.byref(h)), "voila_create")
+        self._h = h
+        self._res = (0, 0, 0, 0)
+
+    # -- plumbing ------------------------------------------------------------------------------
+    def _check(self, status: int, what: str):
+        if status != 0:
+            msg = self.lib.voila_status_string(status).decode()
+            cuda = self.lib.voila_last_cuda_error(self._h).decode() if self._h else ""
+            raise VoilaError(f"{what}: {msg}" + (f" ({cuda})" if cuda else ""))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.voila_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def particle_dtype(self):
+        return self._torch.bfloat16 if self.prec == PREC_BF16 else self._torch.float32
+
+    def _stream(self):
+        return C.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
+
+    def voila_workspace_bytes(self, P, Q, H, N) -> int:
+        return int(self.lib.voila_workspace_bytes(self._h, P, Q, H, N))
+
+    def voila_reserve(self, P=0, Q=0, H=0, N=0):
+        self._check(self.lib.voila_reserve(self._h, P, Q, H, N), "voila_reserve")
+        self._res = (P, Q, H, N)
+
+    def _ensure(self, P=0, Q=0, H=0, N=0):
+        r = self._res
+        if P > r[0] or Q > r[1] or H > r[2] or N > r[3]:
+            self.voila_reserve(max(P, r[0]), max(Q, r[1]), max(H, r[2]), max(N, r[3]))
+
+    def voila_set_kernel(self, kernel: int):
+        self._check(self.lib.voila_set_kernel(self._h, kernel), "voila_set_kernel")
+
+    def voila_tcgen05_supported(self) -> bool:
+        return bool(self.lib.voila_tcgen05_supported(self._h))
+
+    def voila_launch_count(self) -> int:
+        return int(self.lib.voila_launch_count(self._h))
+
+    def voila_last_rollout_kernel(self) -> str:
+        return self.lib.voila_last_rollout_kernel(self._h).decode()
+
+    def voila_set_profiling(self, on: bool):
+        self._check(self.lib.voila_set_profiling(self._h, int(bool(on))), "voila_set_profiling")
+
+    def voila_profile_read(self, which: int):
+        buf = (C.c_float * 256)()
+        n = self.lib.voila_profile_read(self._h, int(which), buf, 256)
+        return [float(buf[i]) for i in range(n)]
+
+    def to_particles(self, x: np.ndarray):
+        """numpy fp32 [n][S] -> device tensor of the ctx's particle dtype (plain dtype conversion)."""
+        t = self._torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(f"cuda:{self.device}")
+        return t.to(self.particle_dtype).contiguous()
+
+    # -- hot calls (device buffers) -------------------------------------------------------------
+    def voila_rollout_values(self, particles, action_seqs, weights, seed, want_witness=True,
+                             want_returns=False, want_final_states=False):
+        torch = self._torch
+        P, S = particles.shape
+        Q, H = action_seqs.shape
+        assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
+        assert action_seqs.dtype == torch.int32 and action_seqs.is_contiguous()
+        self._ensure(P=P, Q=Q, H=H)
+        dev = particles.device
+        values = torch.empty(Q, dtype=torch.float32, device=dev)
+        witness = torch.empty((Q, self.O), dtype=torch.float32, device=dev) if want_witness else None
+        returns = torch.empty((Q, P), dtype=torch.float32, device=dev) if want_returns else None
+        finals = torch.empty((Q, P, S), dtype=torch.float32, device=dev) if want_final_states else None
+        self._check(self.lib.voila_rollout_values(
+            self._h, _dptr(particles), P, _dptr(action_seqs), Q, H, _dptr(weights),
+            C.c_uint64(int(seed)), _dptr(values), _dptr(witness), _dptr(returns), _dptr(finals),
+            self._stream()), "voila_rollout_values")
+        out = {"values": values, "witness": witness}
+        if want_returns:
+            out["returns"] = returns
+        if want_final_states:
+            out["final_states"] = finals
+        return out
+
+    def voila_belief_update(self, particles, action, observation, weights, seed, want_debug=True):
+        torch = self._torch
+        N, S = particles.shape
+        assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
+        assert observation.dtype == torch.float32 and observation.numel() == self.O
+        self._ensure(N=N)
+        dev = particles.device
+        out = {
+            "particles": torch.empty_like(particles),
+            "weights": torch.empty(N, dtype=torch.float32, device=dev),
+            "ancestors": torch.empty(N, dtype=torch.int32, device=dev),
+            "log_evidence": torch.empty(1, dtype=torch.float32, device=dev),
+            "status": torch.empty(1, dtype=torch.int32, device=dev),
+        }
+        if want_debug:
+            out["post_weights"] = torch.empty(N, dtype=torch.float32, device=dev)
+            out["proposals"] = torch.empty_like(particles)
+        self._check(self.lib.voila_belief_update(
+            self._h, _dptr(particles), N, int(action), _dptr(observation), _dptr(weights),
+            C.c_uint64(int(seed)), _dptr(out["particles"]), _dptr(out["weights"]),
+            _dptr(out["ancestors"]), _dptr(out.get("post_weights")), _dptr(out.get("proposals")),
+            _dptr(out["log_evidence"]), _dptr(out["status"]), self._stream()), "voila_belief_update")
+        return out
+
+    def voila_resample_systematic(self, v, seed):
+        torch = self._torch
+        N = v.numel()
+        assert v.dtype == torch.float32 and v.is_contiguous()
+        self._ensure(N=N)
+        anc = torch.empty(N, dtype=torch.int32, device=v.device)
+        status = torch.empty(1, dtype=torch.int32, device=v.device)
+        self._check(self.lib.voila_resample_systematic(
+            self._h, _dptr(v), N, C.c_uint64(int(seed)), _dptr(anc), _dptr(status), self._stream()),
+            "voila_resample_systematic")
+        return anc, status
+
+    def voila_mlp_forward(self, which, x):
+        torch = self._torch
+        rows = x.shape[0]
+        assert x.dtype == torch.float32 and x.is_contiguous()
+        out_dim = [self.S, self.O, self.d, self.d][which]
+        y = torch.empty((rows, out_dim), dtype=torch.float32, device=x.device)
+        self._check(self.lib.voila_mlp_forward(self._h, which, _dptr(x), rows, _dptr(y), self._stream()),
+                    "voila_mlp_forward")
+        return y
+
+    # -- host-buffer variants (pinned torch CPU tensors or numpy arrays) --------------------------
+    def voila_rollout_values_host(self, particles, action_seqs, weights, seed, values_out,
+                                  witness_out=None):
+        P, Q, H = particles.shape[0], action_seqs.shape[0], action_seqs.shape[1]
+        self._ensure(P=P, Q=Q, H=H)
+        self._check(self.lib.voila_rollout_values_host(
+            self._h, _hptr(particles), P, _hptr(action_seqs), Q, H, _hptr(weights),
+            C.c_uint64(int(seed)), _hptr(values_out), _hptr(witness_out), self._stream()),
+            "voila_rollout_values_host")
+        return values_out
+
+    def voila_belief_update_host(self, particles, action, observation, weights, seed, particles_out,
+                                 weights_out=None, ancestors_out=None, log_evidence_out=None,
+                                 status_out=None):
+        N = particles.shape[0]
+        self._ensure(N=N)
+        self._check(self.lib.voila_belief_update_host(
+            self._h, _hptr(particles), N, int(action), _hptr(observation), _hptr(weights),
+            C.c_uint64(int(seed)), _hptr(particles_out), _hptr(weights_out), _hptr(ancestors_out),
+            _hptr(log_evidence_out), _hptr(status_out), self._stream()), "voila_belief_update_host")
+        return particles_out
