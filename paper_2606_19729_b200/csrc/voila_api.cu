@@ -469,7 +469,7 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
     a.max_ordered = sb.max_ordered;
     a.part_wsum = sb.part_wsum;
     int n_parts = (N + kTileRows - 1) / kTileRows;
-    if (use_tc(ctx)) {
+    if (use_tc(ctx) && tc_has_belief(ctx->tc)) {
         int n = 0;
         ProfScope prof(ctx, VOILA_K_PROPOSE, st);
         e = launch_bu_propose_score_tc(ctx->tc, ctx->model, a, st, &n);

@@ -44,6 +44,7 @@ bool tc_supported(const voila_model_desc *desc, std::string *why);
 void *tc_create(const voila_model_desc *desc, int sm_count, std::vector<void *> *allocs,
                 std::string *err);
 void tc_destroy(void *tc);
+bool tc_has_belief(const void *tc);  // the belief-update propose+score program was built too
 cudaError_t launch_rollout_tc(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
                               std::string *kernel_name, int *n_launches);
 cudaError_t launch_bu_propose_score_tc(void *tc, const ModelDev &m, const BeliefArgs &a,

@@ -150,7 +150,8 @@ def test_resample_indices_bit_exact(torch_cuda, oracle, resample_ctx, N, kind):
     for seed in (0, 0xDEADBEEFCAFE):
         anc, status = ctx.voila_resample_systematic(torch.from_numpy(v).cuda(), seed)
         ref, st = oracle.resample_systematic(v, seed)
-        assert int(status.item()) == 0 and st == 0
+        # every weight below 2^-32 quantises to zero: both sides flag it and return the identity
+        assert int(status.item()) == (0 if st == 0 else 1)
         assert np.array_equal(anc.cpu().numpy(), ref)
         if kind == "uniform":
             assert np.array_equal(ref, np.arange(N))
