@@ -180,6 +180,15 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
 voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
                                void *cuda_stream);
 
+/* Root action selection for an open-loop sequence sweep: q* = argmax_q values[q] (ties -> lowest q,
+ * NaN never wins), best_action_out[0] = action_seqs[q*][0], best_q_out[0] = q* (the
+ * planner returns an action for the current belief; DESIGN.md input recipe, config 5).
+ *   values dev [Q] fp32, action_seqs dev [Q][H] int32, best_q_out / best_action_out dev [1] int32
+ *   (best_q_out may be NULL). */
+voila_status voila_best_action(voila_ctx *ctx, const float *values, const int32_t *action_seqs, int Q,
+                               int H, int32_t *best_q_out, int32_t *best_action_out,
+                               void *cuda_stream);
+
 /* Host-buffer variants: every pointer is HOST memory (pinned for best speed); inputs are copied to
  * ctx-owned device staging buffers, the device entry point runs, outputs are copied back and the
  * stream is synchronised.  Optional outputs as above (NULL to skip). */

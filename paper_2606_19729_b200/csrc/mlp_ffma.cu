@@ -262,6 +262,43 @@ __global__ void rollout_reduce_kernel(const double *__restrict__ part_value,
     }
 }
 
+// q* = argmax_q values[q], ties -> lowest q, NaN never wins; one block.
+__global__ void __launch_bounds__(256) best_action_kernel(const float *__restrict__ values,
+                                                          const int32_t *__restrict__ seqs, int Q, int H,
+                                                          int32_t *best_q, int32_t *best_action) {
+    __shared__ float sv[256];
+    __shared__ int si[256];
+    float bv = -INFINITY;
+    int bi = 0x7fffffff;
+    for (int q = threadIdx.x; q < Q; q += 256) {
+        const float v = values[q];
+        if (v == v && (bi == 0x7fffffff || v > bv)) {  // q ascends per thread: strict > keeps the lowest
+            bv = v;
+            bi = q;
+        }
+    }
+    sv[threadIdx.x] = bv;
+    si[threadIdx.x] = bi;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            const float v = sv[threadIdx.x + o];
+            const int i = si[threadIdx.x + o];
+            if (i != 0x7fffffff && (si[threadIdx.x] == 0x7fffffff || v > sv[threadIdx.x] ||
+                                    (v == sv[threadIdx.x] && i < si[threadIdx.x]))) {
+                sv[threadIdx.x] = v;
+                si[threadIdx.x] = i;
+            }
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const int q = si[0] == 0x7fffffff ? 0 : si[0];  // every value NaN: sequence 0
+        if (best_q) *best_q = q;
+        *best_action = seqs[(size_t)q * H];
+    }
+}
+
 template <bool EMU>
 __global__ void __launch_bounds__(kThreads) mlp_forward_ffma_kernel(const ModelDev m, int which,
                                                                     const float *__restrict__ x,
@@ -377,6 +414,12 @@ cudaError_t launch_rollout_reduce(const RolloutArgs &a, int O, const double *wsu
                                   float *witness, cudaStream_t st) {
     rollout_reduce_kernel<<<a.Q, 128, 0, st>>>(a.part_value, witness ? a.part_witness : nullptr,
                                                a.tiles, O, wsum, values, witness);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_best_action(const float *values, const int32_t *seqs, int Q, int H, int32_t *best_q,
+                               int32_t *best_action, cudaStream_t st) {
+    best_action_kernel<<<1, 256, 0, st>>>(values, seqs, Q, H, best_q, best_action);
     return cudaGetLastError();
 }
 

@@ -523,6 +523,17 @@ voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int ro
     return VOILA_OK;
 }
 
+voila_status voila_best_action(voila_ctx *ctx, const float *values, const int32_t *action_seqs, int Q,
+                               int H, int32_t *best_q_out, int32_t *best_action_out, void *cuda_stream) {
+    if (!ctx || !values || !action_seqs || !best_action_out || Q < 1 || H < 1) return VOILA_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    cudaError_t e = launch_best_action(values, action_seqs, Q, H, best_q_out, best_action_out,
+                                       reinterpret_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    return VOILA_OK;
+}
+
 voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, int P,
                                        const int32_t *action_seqs, int Q, int H, const float *weights,
                                        uint64_t seed, float *values_out, float *obs_witness_out,

@@ -10,6 +10,8 @@ cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cud
 cudaError_t launch_rollout_ffma(const ModelDev &m, const RolloutArgs &a, bool bf16, cudaStream_t st);
 cudaError_t launch_rollout_reduce(const RolloutArgs &a, int O, const double *wsum, float *values,
                                   float *witness, cudaStream_t st);
+cudaError_t launch_best_action(const float *values, const int32_t *seqs, int Q, int H, int32_t *best_q,
+                               int32_t *best_action, cudaStream_t st);
 cudaError_t launch_mlp_forward_ffma(const ModelDev &m, int which, const float *x, int rows, float *y,
                                     bool bf16, cudaStream_t st);
 cudaError_t launch_bu_propose_score_ffma(const ModelDev &m, const BeliefArgs &a, bool bf16,

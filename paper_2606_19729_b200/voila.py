@@ -22,7 +22,8 @@ PREC_FP32, PREC_BF16 = 0, 1
 EXPORTS = [
     "voila_create", "voila_destroy", "voila_workspace_bytes", "voila_reserve", "voila_set_kernel",
     "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update",
-    "voila_resample_systematic", "voila_mlp_forward", "voila_rollout_values_host",
+    "voila_resample_systematic", "voila_mlp_forward", "voila_best_action",
+    "voila_rollout_values_host",
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read",
@@ -85,6 +86,8 @@ def load_library():
     lib.voila_resample_systematic.restype = i32
     lib.voila_mlp_forward.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.voila_mlp_forward.restype = i32
+    lib.voila_best_action.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
+    lib.voila_best_action.restype = i32
     lib.voila_rollout_values_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp]
     lib.voila_rollout_values_host.restype = i32
     lib.voila_belief_update_host.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp,
@@ -301,6 +304,17 @@ class Voila:
         self._check(self.lib.voila_mlp_forward(self._h, which, _dptr(x), rows, _dptr(y), self._stream()),
                     "voila_mlp_forward")
         return y
+
+    def voila_best_action(self, values, action_seqs):
+        """-> (best_q, best_action) device int32 tensors of one element each."""
+        torch = self._torch
+        Q, H = action_seqs.shape
+        assert values.dtype == torch.float32 and values.numel() == Q
+        bq = torch.empty(1, dtype=torch.int32, device=values.device)
+        ba = torch.empty(1, dtype=torch.int32, device=values.device)
+        self._check(self.lib.voila_best_action(self._h, _dptr(values), _dptr(action_seqs), Q, H,
+                                               _dptr(bq), _dptr(ba), self._stream()), "voila_best_action")
+        return bq, ba
 
     # -- host-buffer variants (pinned torch CPU tensors or numpy arrays) --------------------------
     def voila_rollout_values_host(self, particles, action_seqs, weights, seed, values_out,
