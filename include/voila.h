@@ -103,7 +103,8 @@ typedef struct {
 typedef enum {
     VOILA_KERNEL_AUTO = 0,   /* tcgen05 path when prec == BF16 and the dims fit it, else FFMA */
     VOILA_KERNEL_FFMA = 1,   /* CUDA-core path (fp32 mode; in bf16 mode rounds operands to bf16) */
-    VOILA_KERNEL_TCGEN05 = 2 /* tensor-core path only; UNSUPPORTED if the dims do not fit */
+    VOILA_KERNEL_TCGEN05 = 2, /* single-CTA tensor-core path (M = 128 per SM); UNSUPPORTED if the dims do not fit */
+    VOILA_KERNEL_TCGEN05_PAIR = 3 /* CTA-pair tensor-core path (cta_group::2, M = 256 per SM pair): what AUTO picks */
 } voila_kernel;
 
 /* Copies and packs the host weights onto `device`.  Fails with VOILA_ERR_UNSUPPORTED when the

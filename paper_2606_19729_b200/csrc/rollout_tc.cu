@@ -14,9 +14,7 @@
 #include <string>
 #include <vector>
 
-#include "sm100_ptx.cuh"
-#include "tc_program.h"
-#include "voila_device.cuh"
+#include "tc_common.cuh"
 #include "voila_kernels.h"
 
 namespace voila {
@@ -24,6 +22,15 @@ namespace voila {
 namespace {
 
 using namespace ptx;
+
+#ifdef VOILA_TC_TRACE
+__device__ unsigned long long g_tc_trace[32];
+#define TRACE_T0() const long long _t0 = clock64()
+#define TRACE_ADD(var) var += clock64() - _t0
+#else
+#define TRACE_T0()
+#define TRACE_ADD(var)
+#endif
 
 struct TcRolloutParams {
     const uint8_t *wstream;
@@ -64,92 +71,7 @@ __host__ __device__ inline SmemMap smem_map(const TcProgramHeader &h) {
     return m;
 }
 
-__device__ __forceinline__ float bf16lo(uint32_t v) { return __uint_as_float(v << 16); }
-__device__ __forceinline__ float bf16hi(uint32_t v) { return __uint_as_float(v & 0xffff0000u); }
-
-__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d)
-                 : "memory");
-}
-
-// Address of the 16-byte unit holding operand columns [8*unit8, 8*unit8+8) of `row` (unit8 counts
-// 8-column units across the whole operand; chunk = unit8 / 8).
-__device__ __forceinline__ uint32_t a_unit_addr(uint32_t a_base, int row, int unit8) {
-    const int chunk = unit8 >> 3, u = unit8 & 7;
-    return a_base + chunk * kTcChunkBytes + row * 128 + ((u ^ (row & 7)) << 4);
-}
-
-template <int ACT>
-__device__ __forceinline__ float act_fast(float x) {
-    if (ACT == VOILA_ACT_RELU) return fmaxf(x, 0.0f);
-    if (ACT == VOILA_ACT_SILU) {
-        const float h = 0.5f * x;  // x * sigmoid(x) = h + h * tanh(h)
-        return fmaf(h, tanh_approx(h), h);
-    }
-    return x;
-}
-
-// One 64-column chunk of a hidden layer for this warp's 32 rows x 32 columns.
-template <int ACT>
-__device__ __forceinline__ void hidden_chunk(uint32_t taddr, const float *__restrict__ bias, uint32_t row_addr,
-                                             int row, int half) {
-    uint32_t v[32];
-    tmem_ld32(taddr, v);
-    float4 b[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) b[i] = __ldg(reinterpret_cast<const float4 *>(bias) + i);
-    tmem_ld_wait();
-    uint32_t o[16];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float y0 = act_fast<ACT>(__uint_as_float(v[4 * i + 0]) + b[i].x);
-        const float y1 = act_fast<ACT>(__uint_as_float(v[4 * i + 1]) + b[i].y);
-        const float y2 = act_fast<ACT>(__uint_as_float(v[4 * i + 2]) + b[i].z);
-        const float y3 = act_fast<ACT>(__uint_as_float(v[4 * i + 3]) + b[i].w);
-        o[2 * i] = pack_bf16x2(y0, y1);
-        o[2 * i + 1] = pack_bf16x2(y2, y3);
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int unit = half * 4 + u;
-        st_shared_v4(row_addr + ((unit ^ (row & 7)) << 4), o[4 * u], o[4 * u + 1], o[4 * u + 2], o[4 * u + 3]);
-    }
-}
-
-// Nz (<= 32, multiple of 8) standard normals of (seed; p, q, t, stream) packed as bf16 pairs.
-__device__ __forceinline__ void gen_noise(uint32_t (&nz)[16], uint64_t seed, uint32_t p, uint32_t q,
-                                          uint32_t t, uint32_t stream, int Nz) {
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        if (4 * b < Nz) {
-            float z[4];
-            normals4<true>(seed, p, q, t, stream, (uint32_t)b, z);
-            nz[2 * b] = pack_bf16x2(z[0], z[1]);
-            nz[2 * b + 1] = pack_bf16x2(z[2], z[3]);
-        }
-    }
-}
-
-// R(s, a) from the bf16 state for the non-quadratic reward kinds (R14).
-__device__ __forceinline__ float reward_from_state(const uint32_t *st, int S, int kind,
-                                                   const float *__restrict__ param) {
-    float acc = 0.0f;
-#pragma unroll
-    for (int c2 = 0; c2 < 32; ++c2) {
-        if (2 * c2 < S) {
-            const float s0 = bf16lo(st[c2]), s1 = bf16hi(st[c2]);
-            const float p0 = __ldg(param + 2 * c2), p1 = __ldg(param + 2 * c2 + 1);
-            if (kind == VOILA_R_NEG_L2_GOAL) {
-                acc = fmaf(s0 - p0, s0 - p0, acc);
-                acc = fmaf(s1 - p1, s1 - p1, acc);
-            } else {
-                acc = fmaf(p0, s0, acc);
-                acc = fmaf(p1, s1, acc);
-            }
-        }
-    }
-    return kind == VOILA_R_NEG_L2_GOAL ? -sqrtf(acc) : acc + __ldg(param + S);
-}
+using namespace tcc;
 
 __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRolloutParams p) {
     extern __shared__ uint8_t smem_raw[];
@@ -208,9 +130,15 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
         // ===== producer: weight tiles, in the program's issue order, once per step =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
+            long long tr_empty = 0;
+            const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
-                    mbar_wait(&empty[stage], phase ^ 1u);
+                    {
+                        TRACE_T0();
+                        mbar_wait(&empty[stage], phase ^ 1u);
+                        TRACE_ADD(tr_empty);
+                    }
                     const uint32_t bytes = T[i].bytes;
                     mbar_arrive_expect_tx(&full[stage], bytes);
                     bulk_g2s(smem + map.ring + stage * kTcStageBytes, p.wstream + T[i].src_off, bytes,
@@ -221,22 +149,37 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                     }
                 }
             }
+#ifdef VOILA_TC_TRACE
+            if (blockIdx.x == 0) {
+                g_tc_trace[0] = tr_empty;
+                g_tc_trace[1] = clock64() - tr_start;
+            }
+#endif
+            (void)tr_empty; (void)tr_start;
         }
     } else if (warp == 1) {
         // ===== MMA issuer =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
             int waited = -1, base = 1;
+            long long tr_evt = 0, tr_full = 0;
+            const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
                     const TcTile t = T[i];
                     const TcLayer &l = L[t.layer];
                     const int need = base + (int)t.need;
                     if (need > waited) {
+                        TRACE_T0();
                         mbar_wait(&evt[need & (kTcEvtRing - 1)], (uint32_t)(need / kTcEvtRing) & 1u);
+                        TRACE_ADD(tr_evt);
                         waited = need;
                     }
-                    mbar_wait(&full[stage], phase);
+                    {
+                        TRACE_T0();
+                        mbar_wait(&full[stage], phase);
+                        TRACE_ADD(tr_full);
+                    }
                     tc_fence_after();
                     const uint64_t ad = umma_desc_sw128(a_u32 + (uint32_t)t.kc * kTcChunkBytes);
                     const uint64_t bd = umma_desc_sw128(ring_u32 + stage * kTcStageBytes);
@@ -253,6 +196,14 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                 }
                 base += p.hdr.evt_per_step;
             }
+#ifdef VOILA_TC_TRACE
+            if (blockIdx.x == 0) {
+                g_tc_trace[2] = tr_evt;
+                g_tc_trace[3] = tr_full;
+                g_tc_trace[4] = clock64() - tr_start;
+            }
+#endif
+            (void)tr_evt; (void)tr_full; (void)tr_start;
         }
     } else if (warp >= 4) {
         // ===== epilogue warps =====
@@ -273,8 +224,12 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
             if (lane == 0) mbar_arrive(&evt[ev & (kTcEvtRing - 1)]);
             ++ev;
         };
+        long long tr_layer = 0;
+        const long long tr_start = clock64();
         auto wait_layer = [&]() {
+            TRACE_T0();
             mbar_wait(layer_done, ld_phase);
+            TRACE_ADD(tr_layer);
             ld_phase ^= 1u;
             tc_fence_after();
         };
@@ -494,6 +449,13 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                 }
             }
         }
+#ifdef VOILA_TC_TRACE
+        if (blockIdx.x == 0 && lane == 0) {
+            g_tc_trace[8 + 2 * ew] = tr_layer;
+            g_tc_trace[9 + 2 * ew] = clock64() - tr_start;
+        }
+#endif
+        (void)tr_layer; (void)tr_start;
     }
 
     tc_fence_before();
@@ -691,6 +653,9 @@ void *tc_create(const voila_model_desc *d, int sm_count, std::vector<void *> *al
     while (cols < max_n) cols *= 2;
     h->hdr.tmem_cols = cols;
     h->hdr.n_stages = 8;
+#ifdef VOILA_TC_TRACE
+    if (const char *e = getenv("VOILA_TC_STAGES")) h->hdr.n_stages = atoi(e);
+#endif
     while (h->hdr.n_stages > 2 && smem_map(h->hdr).total + 1024 > kMaxDynSmem) --h->hdr.n_stages;
     h->smem_bytes = smem_map(h->hdr).total + 1024;
     if (h->smem_bytes > kMaxDynSmem) {
@@ -757,3 +722,9 @@ cudaError_t launch_bu_propose_score_tc(void *, const ModelDev &, const BeliefArg
 }
 
 }  // namespace voila
+
+#ifdef VOILA_TC_TRACE
+extern "C" __attribute__((visibility("default"))) int voila_debug_tc_trace(unsigned long long *out32) {
+    return (int)cudaMemcpyFromSymbol(out32, voila::g_tc_trace, sizeof(unsigned long long) * 32);
+}
+#endif

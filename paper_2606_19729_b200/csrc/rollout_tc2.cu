@@ -1,0 +1,748 @@
+// rollout_tc2.cu -- CTA-pair (cta_group::2) tcgen05 path of libvoila (bf16 mode): the persistent
+// fused-MLP rollout kernel.  See tc2_program.h for the execution model.  A cluster of two CTAs
+// (two SMs) is persistent over (sequence, 256-particle block) work units; per CTA:
+//   warp 0    producer: TMA (cp.async.bulk.tensor, cta_group::2) streams this CTA's half of every
+//             weight tile L2 -> shared-memory ring, completing bytes on the LEADER's mbarrier
+//   warp 1    MMA issuer (leader CTA only): one thread issues tcgen05.mma.cta_group::2
+//             (M = 256, N = bn, K = 16, bf16 -> fp32 in both CTAs' TMEM), multicast commits
+//   warp 2    TMEM allocation
+//   warps 4-11 epilogue: tcgen05.ld accumulator block -> bias + activation -> bf16 -> operand
+//             buffer (in place), Philox noise, reward / return accumulation, observation witness.
+// The horizon loop never leaves the SMs: HBM sees the particle rows once per work unit and the
+// per-unit partial sums; weights come from L2, half a tile per CTA.
+#include <cuda.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "tc2_program.h"
+#include "tc_common.cuh"
+#include "voila_kernels.h"
+
+namespace voila {
+
+namespace {
+
+using namespace tcc;
+
+struct T2Params {
+    const float *bias;
+    const T2Layer *layers;
+    const T2Tile *tiles;
+    T2Header hdr;
+    const uint16_t *particles;  // [P][S] bf16
+    const int32_t *seqs;        // [Q][H]
+    const float *weights;       // [P] or nullptr
+    int P, Q, H;
+    uint64_t seed;
+    double *part_value;    // [Q][tiles_per_q]
+    double *part_witness;  // [Q][tiles_per_q][O] or nullptr
+    float *returns_out;
+    float *final_states_out;
+    int tiles_per_q, blocks_per_q, n_units;
+    int S, O, A, Nz;
+    float gamma;
+    int reward_kind;
+    const float *reward_param;
+    const float *action_cost;
+};
+
+struct Smem2 {
+    uint32_t a, ring, layers, tiles, bars, misc, total;
+};
+__host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
+    Smem2 m;
+    m.a = 0;
+    m.ring = m.a + (uint32_t)h.a_chunks * kT2ChunkBytes;
+    m.layers = m.ring + (uint32_t)h.n_stages * kT2StageBytes;
+    m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
+    m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2Tile) + 15u) & ~15u);
+    m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing) * 8;
+    m.total = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
+    return m;
+}
+
+// Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
+// in hidden layers, one 32-column half of every 64-column chunk.  Events are published on the
+// LEADER's mbarriers (remote arrive from the peer CTA).
+__device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
+                                            uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
+                                            int warp, int lane, uint32_t rank, int cluster_id, int n_clusters,
+                                            int n_my_units, int total_steps) {
+    const int n_layers = p.hdr.n_layers;
+    const uint32_t evt_cl = mapa_u32(smem_u32(evt), 0u);
+    {
+        // ===== epilogue warps =====
+        const int ew = warp - 4, qd = warp & 3, half = ew >> 2;
+        const int row = qd * 32 + lane;
+        const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
+        const int S = p.S, O = p.O, Nz = p.Nz;
+        const int in_units = p.hdr.in_chunks * 8;  // 8-column units of the step's input operand
+        uint32_t persist[64];  // half 0: packed bf16 state (32 words); half 1: fp32 witness (64 words)
+        uint32_t nz[16];
+        float G = 0.0f, disc = 1.0f, w_row = 0.0f;
+        int ev = 0, t = 0, unit_i = 0, q = 0, blk = 0, p_idx = 0;
+        bool valid = false;
+        uint32_t ld_seq = 0;
+
+        auto arrive_event = [&]() {
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(evt_cl + 8u * (uint32_t)(ev & (kT2EvtRing - 1)));
+            ++ev;
+        };
+        auto wait_layer = [&]() {
+            mbar_wait(&layer_done[ld_seq & (kT2AccRing - 1)], (ld_seq >> 3) & 1u);
+            ++ld_seq;
+            tc_fence_after();
+        };
+        auto load_unit = [&]() {
+            const int unit = cluster_id + unit_i * n_clusters;
+            q = unit / p.blocks_per_q;
+            blk = (unit - q * p.blocks_per_q) * 2 + (int)rank;  // 128-row tile index within the sequence
+            p_idx = blk * kT2Rows + row;
+            valid = p_idx < p.P;
+            w_row = valid ? (p.weights ? __ldg(p.weights + p_idx) : 1.0f) : 0.0f;
+            G = 0.0f;
+            disc = 1.0f;
+            t = 0;
+            if (half == 0) {
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                    if (8 * u < S && valid)
+                        v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)p_idx * S) + u);
+                    persist[4 * u] = v.x; persist[4 * u + 1] = v.y;
+                    persist[4 * u + 2] = v.z; persist[4 * u + 3] = v.w;
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 64; ++c) persist[c] = 0u;
+            }
+        };
+        // Writes the generator input [s ; w ; 0] of the next layer-1 into the operand buffer: the
+        // `state_half` warps write the state units, the other half the noise and padding units.
+        auto write_input = [&](int state_half, int noise_half) {
+            if (half == state_half) {
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (8 * u < S)
+                        st_shared_v4(a_unit_addr(a_u32, row, u), persist[4 * u], persist[4 * u + 1],
+                                     persist[4 * u + 2], persist[4 * u + 3]);
+            }
+            if (half == noise_half) {
+                const int u0 = S >> 3;
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (8 * u < Nz)
+                        st_shared_v4(a_unit_addr(a_u32, row, u0 + u), nz[4 * u], nz[4 * u + 1], nz[4 * u + 2],
+                                     nz[4 * u + 3]);
+                for (int u = u0 + (Nz >> 3); u < in_units; ++u)
+                    st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
+            }
+        };
+        auto step_reward = [&]() {  // non-quadratic reward kinds: R(s_t, a_t) from the state words
+            if (half == 0 && p.reward_kind != VOILA_R_NEG_QUADRATIC) {
+                float r = reward_from_state(persist, S, p.reward_kind, p.reward_param);
+                if (p.action_cost) r += __ldg(p.action_cost + __ldg(p.seqs + (size_t)q * p.H + t));
+                G = fmaf(disc, r, G);
+            }
+        };
+
+        if (n_my_units > 0) {
+            load_unit();
+            if (half == 0) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
+            write_input(0, 0);
+            step_reward();
+            fence_proxy_async_smem();
+            arrive_event();
+        }
+        for (int step = 0; step < total_steps; ++step) {
+            const int a_t = __ldg(p.seqs + (size_t)q * p.H + t);
+            for (int li = 0; li < n_layers; ++li) {
+                const T2Layer l = L[li];
+                const float *bias = p.bias + l.bias_off + (l.bias_per_action ? (size_t)a_t * l.n_pad : 0);
+                if (l.epi == T2_EPI_HIDDEN) {
+                    wait_layer();
+                    const int chunks = l.n_pad >> 6;
+                    for (int j = 0; j < chunks; ++j) {
+                        const uint32_t taddr = lane_taddr + (uint32_t)(64 * j + 32 * half);
+                        const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
+                        const float *bj = bias + 64 * j + 32 * half;
+                        if (l.act == VOILA_ACT_SILU) hidden_chunk<VOILA_ACT_SILU>(taddr, bj, row_addr, row, half);
+                        else if (l.act == VOILA_ACT_RELU) hidden_chunk<VOILA_ACT_RELU>(taddr, bj, row_addr, row, half);
+                        else hidden_chunk<VOILA_ACT_NONE>(taddr, bj, row_addr, row, half);
+                        fence_proxy_async_smem();
+                        tc_fence_before();
+                        arrive_event();
+                    }
+                } else if (l.epi == T2_EPI_REWARD) {
+                    wait_layer();
+                    if (half == 0) {
+                        float r = 0.0f;
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) {
+                            if (16 * g < (int)l.n_pad) {
+                                uint32_t v[16];
+                                tmem_ld16(lane_taddr + 16 * g, v);
+                                tmem_ld_wait();
+#pragma unroll
+                                for (int c = 0; c < 16; c += 2) {
+                                    const uint32_t sw = persist[(16 * g + c) >> 1];
+                                    r = fmaf(bf16lo(sw), __uint_as_float(v[c]), r);
+                                    r = fmaf(bf16hi(sw), __uint_as_float(v[c + 1]), r);
+                                }
+                            }
+                        }
+                        r = -r;
+                        if (p.action_cost) r += __ldg(p.action_cost + a_t);
+                        G = fmaf(disc, r, G);
+                    }
+                    tc_fence_before();
+                    arrive_event();
+                } else if (l.epi == T2_EPI_STATE) {
+                    // w_Z(t) is independent of the state: draw it while the output layer's MMAs run
+                    if (half == 1) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
+                    wait_layer();
+                    if (half == 0) {
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) {
+                            if (16 * g < (int)l.n_pad) {
+                                uint32_t v[16];
+                                tmem_ld16(lane_taddr + 16 * g, v);
+                                float4 b[4];
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) b[i] = __ldg(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                tmem_ld_wait();
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) {
+                                    persist[8 * g + 2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
+                                                                        __uint_as_float(v[4 * i + 1]) + b[i].y);
+                                    persist[8 * g + 2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
+                                                                            __uint_as_float(v[4 * i + 3]) + b[i].w);
+                                }
+                            }
+                        }
+                    }
+                    write_input(0, 1);
+                    fence_proxy_async_smem();
+                    tc_fence_before();
+                    arrive_event();
+                } else {  // T2_EPI_OBS: last layer of the step
+                    const bool last_step = (t == p.H - 1);
+                    if (half == 0 && !last_step)
+                        gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)(t + 1), kStreamRolloutT, Nz);
+                    wait_layer();
+                    if (half == 1) {
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) {
+                            if (16 * g < (int)l.n_pad) {
+                                uint32_t v[16];
+                                tmem_ld16(lane_taddr + 16 * g, v);
+                                float4 b[4];
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) b[i] = __ldg(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                tmem_ld_wait();
+#pragma unroll
+                                for (int i = 0; i < 4; ++i) {
+                                    const float o0 = __uint_as_float(v[4 * i]) + b[i].x, o1 = __uint_as_float(v[4 * i + 1]) + b[i].y;
+                                    const float o2 = __uint_as_float(v[4 * i + 2]) + b[i].z, o3 = __uint_as_float(v[4 * i + 3]) + b[i].w;
+                                    const int c0 = 16 * g + 4 * i;
+                                    persist[c0] = __float_as_uint(fmaf(disc, o0, __uint_as_float(persist[c0])));
+                                    persist[c0 + 1] = __float_as_uint(fmaf(disc, o1, __uint_as_float(persist[c0 + 1])));
+                                    persist[c0 + 2] = __float_as_uint(fmaf(disc, o2, __uint_as_float(persist[c0 + 2])));
+                                    persist[c0 + 3] = __float_as_uint(fmaf(disc, o3, __uint_as_float(persist[c0 + 3])));
+                                }
+                            }
+                        }
+                    }
+                    ++t;
+                    disc *= p.gamma;
+                    if (last_step) {
+                        // ---- work unit finished: per-(q, tile) weighted partial sums, fixed order ----
+                        if (half == 0) {
+                            double v = valid ? (double)w_row * (double)G : 0.0;
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                            if (lane == 0) red_g[qd] = v;
+                            if (valid && p.returns_out) p.returns_out[(size_t)q * p.P + p_idx] = G;
+                            if (valid && p.final_states_out) {
+                                float *fs = p.final_states_out + ((size_t)q * p.P + p_idx) * S;
+#pragma unroll
+                                for (int c2 = 0; c2 < 32; ++c2)
+                                    if (2 * c2 < S) {
+                                        fs[2 * c2] = bf16lo(persist[c2]);
+                                        fs[2 * c2 + 1] = bf16hi(persist[c2]);
+                                    }
+                            }
+                        } else if (p.part_witness) {
+#pragma unroll
+                            for (int c = 0; c < 64; ++c) {
+                                if (c < O) {
+                                    float x = w_row * __uint_as_float(persist[c]);
+#pragma unroll
+                                    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+                                    if (lane == 0) red_w[qd * 64 + c] = x;
+                                }
+                            }
+                        }
+                        named_bar_sync(1, 256);
+                        if (ew == 0 && lane == 0)
+                            p.part_value[(size_t)q * p.tiles_per_q + blk] = (red_g[0] + red_g[1]) + (red_g[2] + red_g[3]);
+                        if (ew == 4 && p.part_witness) {
+                            for (int c = lane; c < O; c += 32)
+                                p.part_witness[((size_t)q * p.tiles_per_q + blk) * O + c] =
+                                    ((double)red_w[c] + (double)red_w[64 + c]) +
+                                    ((double)red_w[128 + c] + (double)red_w[192 + c]);
+                        }
+                        named_bar_sync(1, 256);
+                        ++unit_i;
+                        if (unit_i < n_my_units) {
+                            load_unit();
+                            if (half == 0) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
+                        }
+                    }
+                    if (unit_i < n_my_units) {
+                        write_input(0, 0);
+                        step_reward();
+                    }
+                    fence_proxy_async_smem();
+                    tc_fence_before();
+                    arrive_event();
+                }
+            }
+        }
+    }
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
+    rollout_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw_u32 = smem_u32(smem_raw);
+    uint8_t *smem = smem_raw + (((raw_u32 + 1023u) & ~1023u) - raw_u32);
+    const Smem2 map = smem2_map(p.hdr);
+    T2Layer *L = reinterpret_cast<T2Layer *>(smem + map.layers);
+    T2Tile *T = reinterpret_cast<T2Tile *>(smem + map.tiles);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + map.bars);
+    uint64_t *empty = full + 8;
+    uint64_t *evt = empty + 8;
+    uint64_t *layer_done = evt + kT2EvtRing;
+    uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(smem + map.misc);
+    double *red_g = reinterpret_cast<double *>(smem + map.misc + 16);
+    float *red_w = reinterpret_cast<float *>(smem + map.misc + 16 + 4 * 8);
+    const uint32_t a_u32 = smem_u32(smem + map.a), ring_u32 = smem_u32(smem + map.ring);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int n_layers = p.hdr.n_layers, n_tiles = p.hdr.n_tiles, n_stages = p.hdr.n_stages;
+
+    // ---- one-time setup: program -> smem, zero the operand buffer, barriers, TMEM ----
+    {
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(p.layers);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(L);
+        for (int i = threadIdx.x; i < n_layers * (int)(sizeof(T2Layer) / 4); i += kT2Threads) dst[i] = src[i];
+        src = reinterpret_cast<const uint32_t *>(p.tiles);
+        dst = reinterpret_cast<uint32_t *>(T);
+        for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2Tile) / 4); i += kT2Threads) dst[i] = src[i];
+        uint4 *az = reinterpret_cast<uint4 *>(smem + map.a);
+        for (int i = threadIdx.x; i < p.hdr.a_chunks * kT2ChunkBytes / 16; i += kT2Threads)
+            az[i] = make_uint4(0u, 0u, 0u, 0u);
+        fence_proxy_async_smem();
+    }
+    if (warp == 0 && lane == 0) tma_prefetch_desc(&wmap);
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < 8; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 1);
+        }
+        for (int i = 0; i < kT2EvtRing; ++i) mbar_init(&evt[i], 16);  // 8 epilogue warps x 2 CTAs
+        for (int i = 0; i < kT2AccRing; ++i) mbar_init(&layer_done[i], 1);
+        fence_barrier_init();
+    }
+    if (warp == 2) {
+        tmem_alloc_2cta(tmem_ptr, (uint32_t)p.hdr.tmem_cols);
+        tmem_relinquish_2cta();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();  // the peer's barriers and TMEM exist before anything signals them
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    const int cluster_id = (int)blockIdx.x >> 1, n_clusters = (int)gridDim.x >> 1;
+    const int n_my_units = (p.n_units - cluster_id + n_clusters - 1) / n_clusters;
+    const int total_steps = n_my_units * p.H;
+
+    if (warp == 0) {
+        // ===== producer: this CTA's half of every weight tile, in issue order, once per step =====
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (int step = 0; step < total_steps; ++step) {
+                for (int i = 0; i < n_tiles; ++i) {
+                    const T2Tile t = T[i];
+                    mbar_wait(&empty[stage], phase ^ 1u);
+                    if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2u * kT2StageBytes);
+                    const int rows = (int)t.nk * (int)t.rows8 * 8;
+                    tma_load_2d_2cta(smem + map.ring + stage * kT2StageBytes, &wmap, &full[stage], 0,
+                                     (int32_t)t.src_row + (int32_t)rank * rows);
+                    if (++stage == (uint32_t)n_stages) {
+                        stage = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: leader CTA only =====
+        if (lane == 0 && rank == 0) {
+            uint32_t stage = 0, phase = 0;
+            int waited = -1, base = 1, blk_base = 0;
+            for (int step = 0; step < total_steps; ++step) {
+                T2Tile t = T[0];
+                for (int i = 0; i < n_tiles; ++i) {
+                    const T2Tile nxt = T[i + 1 < n_tiles ? i + 1 : 0];  // prefetch the next record
+                    const int need = base + (int)t.need;
+                    if (need > waited) {
+                        mbar_wait(&evt[need & (kT2EvtRing - 1)], (uint32_t)(need / kT2EvtRing) & 1u);
+                        waited = need;
+                    }
+                    mbar_wait(&full[stage], phase);
+                    tc_fence_after();
+                    const uint32_t d = tmem_base + (uint32_t)t.d_col16 * 16u;
+                    const uint32_t chunk_b = (uint32_t)t.rows8 * 1024u;  // bytes of one K chunk in the stage
+                    uint32_t acc = (t.flags & 1u) ? 0u : 1u;
+                    for (int c = 0; c < (int)t.nk; ++c) {
+                        const uint64_t ad = umma_desc_sw128(a_u32 + (uint32_t)(t.kc0 + c) * kT2ChunkBytes);
+                        const uint64_t bd = umma_desc_sw128(ring_u32 + stage * kT2StageBytes + c * chunk_b);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {  // 64-wide chunk = 4 x (K = 16); +32 bytes per K step
+                            umma_ss_2cta(d, ad + 2u * k, bd + 2u * k, t.idesc, acc);
+                            acc = 1u;
+                        }
+                    }
+                    umma_commit_2cta(&empty[stage], 3);
+                    if (t.flags & 2u) umma_commit_2cta(&layer_done[(blk_base + (int)t.blk) & (kT2AccRing - 1)], 3);
+                    if (++stage == (uint32_t)n_stages) {
+                        stage = 0;
+                        phase ^= 1u;
+                    }
+                    t = nxt;
+                }
+                base += p.hdr.evt_per_step;
+                blk_base += p.hdr.layers_per_step;
+            }
+        }
+    } else if (warp >= 4) {
+        t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, warp, lane, rank, cluster_id,
+                    n_clusters, n_my_units, total_steps);
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 2) tmem_dealloc_2cta(tmem_base, (uint32_t)p.hdr.tmem_cols);
+}
+
+}  // namespace
+
+// =====================================================================================
+// Host side: program construction (weight packing, block shapes, issue order), launcher
+// =====================================================================================
+namespace {
+
+constexpr size_t kMaxDynSmem2 = 232448;  // 227 KB per CTA on sm_100
+
+uint16_t h_bf16_bits(float x) {
+    uint32_t u;
+    std::memcpy(&u, &x, 4);
+    if ((u & 0x7f800000u) != 0x7f800000u) u += 0x7fffu + ((u >> 16) & 1u);
+    return (uint16_t)(u >> 16);
+}
+float h_bf16_round(float x) {
+    const uint32_t u = (uint32_t)h_bf16_bits(x) << 16;
+    float y;
+    std::memcpy(&y, &u, 4);
+    return y;
+}
+int rup(int x, int m) { return (x + m - 1) / m * m; }
+
+// Accumulator block widths of a hidden layer of width n (multiple of 64).  Narrow blocks first:
+// the next layer's MMAs may start as soon as the epilogue has drained the first block, and a
+// block's tiles all wait for the block's LAST column to be drained.
+std::vector<int> hidden_blocks(int n, int policy) {
+    std::vector<int> b;
+    int left = n;
+    if (policy == 1) {  // all 256
+        while (left >= 256) { b.push_back(256); left -= 256; }
+    } else if (policy == 2) {  // all 128
+        while (left >= 128) { b.push_back(128); left -= 128; }
+    } else {  // 128, 128, then 256s
+        for (int i = 0; i < 2 && left >= 128; ++i) { b.push_back(128); left -= 128; }
+        while (left >= 256) { b.push_back(256); left -= 256; }
+    }
+    while (left >= 128) { b.push_back(128); left -= 128; }
+    if (left > 0) b.push_back(left);  // 64
+    return b;
+}
+
+struct Builder2 {
+    std::vector<T2Layer> layers;
+    std::vector<T2Tile> tiles;
+    std::vector<uint8_t> wstream;  // rows of 128 bytes
+    std::vector<float> bias;
+    int evt = 0;
+    int col_free[512];
+    int a_ready[8];
+    int a_chunks = 1;
+    int policy = 0;
+
+    Builder2() {
+        for (int &c : col_free) c = -1;
+        for (int &a : a_ready) a = -1;
+    }
+
+    // W: [n0][k0] row-major fp32 ("algorithmic" column order); bias_rows x n0 biases.
+    void add_layer(const float *W, int n0, int k0, const float *b, int bias_rows, int epi, int act) {
+        T2Layer l{};
+        const bool hidden = epi == T2_EPI_HIDDEN;
+        const int n_pad = hidden ? n0 : rup(n0, 16);
+        const int kc_n = rup(k0, 64) / 64;
+        l.bias_off = (uint32_t)bias.size();
+        l.n_pad = (uint16_t)n_pad;
+        l.epi = (uint8_t)epi;
+        l.act = (uint8_t)act;
+        l.bias_per_action = bias_rows > 1;
+        for (int r = 0; r < bias_rows; ++r)
+            for (int j = 0; j < n_pad; ++j) bias.push_back((b && j < n0) ? b[(size_t)r * n0 + j] : 0.0f);
+        a_chunks = std::max(a_chunks, std::max(kc_n, hidden ? n_pad / 64 : 1));
+        const int li = (int)layers.size();
+        std::vector<int> blocks = hidden ? hidden_blocks(n_pad, policy) : std::vector<int>{n_pad};
+        l.bn = (uint16_t)blocks[0];
+        std::vector<T2Tile> lt;
+        int n_start = 0;
+        for (size_t bi = 0; bi < blocks.size(); ++bi) {
+            const int bn = blocks[bi], half = bn / 2;
+            const int nk_max = std::max(1, std::min(4, 128 / half));
+            int blk_need = -1;
+            for (int c = n_start; c < n_start + bn; ++c) blk_need = std::max(blk_need, col_free[c]);
+            for (int kc0 = 0; kc0 < kc_n; kc0 += nk_max) {
+                const int nk = std::min(nk_max, kc_n - kc0);
+                T2Tile t{};
+                t.src_row = (uint32_t)(wstream.size() / 128);
+                t.idesc = umma_idesc_bf16_m256((uint32_t)bn);
+                t.d_col16 = (uint8_t)(n_start / 16);
+                t.blk = (uint8_t)li;
+                t.kc0 = (uint8_t)kc0;
+                t.nk = (uint8_t)nk;
+                t.rows8 = (uint8_t)(half / 8);
+                int need = blk_need;
+                for (int c = 0; c < nk; ++c) need = std::max(need, a_ready[kc0 + c]);
+                t.need = (int16_t)need;
+                t.flags = (uint8_t)(bi << 4);  // scratch: block index, cleared below
+                // pack: CTA 0's rows then CTA 1's; per CTA chunk by chunk; 16-byte units XOR (row & 7)
+                const size_t base = wstream.size();
+                wstream.resize(base + (size_t)2 * nk * half * 128, 0);
+                for (int r = 0; r < 2; ++r)
+                    for (int c = 0; c < nk; ++c)
+                        for (int i = 0; i < half; ++i) {
+                            uint8_t *dst = wstream.data() + base + ((size_t)(r * nk + c) * half + i) * 128;
+                            const int row = n_start + r * half + i;
+                            for (int u = 0; u < 8; ++u)
+                                for (int e = 0; e < 8; ++e) {
+                                    const int k = (kc0 + c) * 64 + u * 8 + e;
+                                    const float v = (row < n0 && k < k0) ? W[(size_t)row * k0 + k] : 0.0f;
+                                    const uint16_t h = h_bf16_bits(v);
+                                    std::memcpy(dst + ((u ^ (i & 7)) * 16) + e * 2, &h, 2);
+                                }
+                        }
+                lt.push_back(t);
+            }
+            n_start += bn;
+        }
+        std::stable_sort(lt.begin(), lt.end(), [](const T2Tile &x, const T2Tile &y) { return x.need < y.need; });
+        bool seen[16] = {};
+        for (T2Tile &t : lt) {
+            const int bi = t.flags >> 4;
+            t.flags = seen[bi] ? 0 : 1;
+            seen[bi] = true;
+        }
+        lt.back().flags |= 2;  // the layer's last tile hands the accumulator to the epilogues
+        tiles.insert(tiles.end(), lt.begin(), lt.end());
+        layers.push_back(l);
+        if (hidden) {
+            for (int j = 0; j < n_pad / 64; ++j) {
+                for (int c = 64 * j; c < 64 * j + 64; ++c) col_free[c] = evt;
+                a_ready[j] = evt;
+                ++evt;
+            }
+        } else {
+            for (int c = 0; c < n_pad; ++c) col_free[c] = evt;
+            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE)
+                for (int &a : a_ready) a = evt;  // the next layer-1 input is written with this event
+            ++evt;
+        }
+    }
+};
+
+struct T2Handle {
+    T2Header hdr{};
+    void *d_wstream = nullptr, *d_bias = nullptr, *d_layers = nullptr, *d_tiles = nullptr;
+    size_t smem_bytes = 0;
+    int max_clusters = 0;
+    CUtensorMap wmap;
+};
+
+// Layer 1 of a generator sees the "algorithmic" input [s ; w] (K = S + Nz): the one-hot block is
+// folded into a per-action bias row b1 + W1[:, S + a] (R21).
+void add_generator2(Builder2 &pb, const voila_mlp &f, int S, int A, int Nz, int last_epi) {
+    for (int l = 0; l < f.n_layers; ++l) {
+        const int K = f.dims[l], N = f.dims[l + 1];
+        const bool last = l == f.n_layers - 1;
+        if (l == 0) {
+            const int k0 = S + Nz;
+            std::vector<float> W((size_t)N * k0), b((size_t)A * N);
+            for (int j = 0; j < N; ++j) {
+                for (int k = 0; k < S; ++k) W[(size_t)j * k0 + k] = f.W[0][(size_t)j * K + k];
+                for (int k = 0; k < Nz; ++k) W[(size_t)j * k0 + S + k] = f.W[0][(size_t)j * K + S + A + k];
+                for (int a = 0; a < A; ++a)
+                    b[(size_t)a * N + j] = f.b[0][j] + h_bf16_round(f.W[0][(size_t)j * K + S + a]);
+            }
+            pb.add_layer(W.data(), N, k0, b.data(), A, last ? last_epi : T2_EPI_HIDDEN, f.act);
+        } else {
+            pb.add_layer(f.W[l], N, K, f.b[l], 1, last ? last_epi : T2_EPI_HIDDEN, f.act);
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+bool tc2_supported(const voila_model_desc *d, std::string *why) { return tc_supported(d, why); }
+
+void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *allocs, std::string *err) {
+    const int S = d->state_dim, A = d->n_actions, Nz = d->noise_dim;
+    auto fail = [&](const std::string &m) -> void * {
+        if (err) *err = m;
+        return nullptr;
+    };
+    Builder2 pb;
+    if (const char *e = getenv("VOILA_T2_BLOCK_POLICY")) pb.policy = atoi(e);  // tuning knob (0, 1, 2)
+    if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
+        pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
+    add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
+    add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
+    if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles)
+        return fail("model too deep for the tcgen05 program tables");
+    // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
+    pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
+
+    T2Handle *h = new T2Handle();
+    h->hdr.n_layers = h->hdr.layers_per_step = (int)pb.layers.size();
+    h->hdr.n_tiles = (int)pb.tiles.size();
+    h->hdr.evt_per_step = pb.evt;
+    h->hdr.a_chunks = pb.a_chunks;
+    h->hdr.in_chunks = rup(S + Nz, 64) / 64;
+    int max_n = 32;
+    for (const T2Layer &l : pb.layers) max_n = std::max(max_n, (int)l.n_pad);
+    int cols = 32;
+    while (cols < max_n) cols *= 2;
+    h->hdr.tmem_cols = cols;
+    h->hdr.n_stages = 8;
+    if (const char *e = getenv("VOILA_T2_STAGES")) h->hdr.n_stages = std::max(2, std::min(8, atoi(e)));
+    while (h->hdr.n_stages > 2 && smem2_map(h->hdr).total + 1024 > kMaxDynSmem2) --h->hdr.n_stages;
+    h->smem_bytes = smem2_map(h->hdr).total + 1024;
+    if (h->smem_bytes > kMaxDynSmem2) {
+        delete h;
+        return fail("model does not fit the shared-memory budget of the tcgen05 pair kernel");
+    }
+    auto upload = [&](const void *src, size_t bytes, void **dst) -> bool {
+        if (cudaMalloc(dst, bytes) != cudaSuccess) return false;
+        allocs->push_back(*dst);
+        return cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
+    };
+    if (!upload(pb.wstream.data(), pb.wstream.size(), &h->d_wstream) ||
+        !upload(pb.bias.data(), pb.bias.size() * sizeof(float), &h->d_bias) ||
+        !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &h->d_layers) ||
+        !upload(pb.tiles.data(), pb.tiles.size() * sizeof(T2Tile), &h->d_tiles) ||
+        cudaFuncSetAttribute(rollout_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)h->smem_bytes) != cudaSuccess) {
+        const std::string m = cudaGetErrorString(cudaGetLastError());
+        delete h;
+        return fail(m);
+    }
+    // weight stream as a 2-D tensor [rows][64 bf16]; box = one ring stage (128 rows x 128 bytes).
+    // The tiles are pre-swizzled on the host, so the copy itself does not swizzle.
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        fn == nullptr || qres != cudaDriverEntryPointSuccess) {
+        delete h;
+        return fail("cuTensorMapEncodeTiled not available from the driver");
+    }
+    const cuuint64_t gdim[2] = {64, (cuuint64_t)(pb.wstream.size() / 128)};
+    const cuuint64_t gstride[1] = {128};
+    const cuuint32_t box[2] = {64, 128};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult cr = reinterpret_cast<EncodeTiledFn>(fn)(
+        &h->wmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, h->d_wstream, gdim, gstride, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) {
+        delete h;
+        return fail("cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)cr));
+    }
+    // how many CTA pairs can be resident at once (one CTA per SM; normally sm_count / 2)
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(sm_count & ~1));
+    cfg.blockDim = dim3(kT2Threads);
+    cfg.dynamicSmemBytes = h->smem_bytes;
+    int nc = 0;
+    if (cudaOccupancyMaxActiveClusters(&nc, rollout_tc2_kernel, &cfg) != cudaSuccess || nc < 1) {
+        cudaGetLastError();
+        nc = sm_count / 2;
+    }
+    h->max_clusters = std::min(nc, sm_count / 2);
+    return h;
+}
+
+void tc2_destroy(void *tc) { delete reinterpret_cast<T2Handle *>(tc); }
+
+cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
+                               std::string *kernel_name, int *n_launches) {
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    T2Params p{};
+    p.bias = reinterpret_cast<const float *>(h->d_bias);
+    p.layers = reinterpret_cast<const T2Layer *>(h->d_layers);
+    p.tiles = reinterpret_cast<const T2Tile *>(h->d_tiles);
+    p.hdr = h->hdr;
+    p.particles = reinterpret_cast<const uint16_t *>(a.particles);
+    p.seqs = a.action_seqs;
+    p.weights = a.weights;
+    p.P = a.P; p.Q = a.Q; p.H = a.H;
+    p.seed = a.seed;
+    p.part_value = a.part_value;
+    p.part_witness = a.part_witness;
+    p.returns_out = a.returns_out;
+    p.final_states_out = a.final_states_out;
+    p.blocks_per_q = (a.P + 2 * kT2Rows - 1) / (2 * kT2Rows);
+    p.tiles_per_q = a.tiles;  // = 2 * blocks_per_q (see rollout_tile_count)
+    p.n_units = p.blocks_per_q * a.Q;
+    p.S = m.S; p.O = m.O; p.A = m.A; p.Nz = m.Nz;
+    p.gamma = m.gamma;
+    p.reward_kind = m.reward.kind;
+    p.reward_param = m.reward.param;
+    p.action_cost = m.reward.action_cost;
+    const int clusters = std::min(h->max_clusters, p.n_units);
+    rollout_tc2_kernel<<<2 * clusters, kT2Threads, h->smem_bytes, st>>>(p, h->wmap);
+    if (kernel_name) *kernel_name = "rollout_tc2_kernel<tcgen05 cta_group::2 bf16>";
+    if (n_launches) *n_launches = 1;
+    return cudaGetLastError();
+}
+
+}  // namespace voila

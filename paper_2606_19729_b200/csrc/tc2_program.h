@@ -1,0 +1,67 @@
+// tc2_program.h -- the static program of the CTA-PAIR tcgen05 kernels (rollout_tc2.cu).
+//
+// Two CTAs of a cluster (two SMs of one TPC) own 256 rows (particles of ONE action sequence / of
+// the belief), 128 each.  Every tcgen05.mma is issued with cta_group::2 by the leader CTA: M = 256,
+// each CTA supplies its own 128 operand rows and HALF of the weight tile's output neurons, and
+// receives its 128 accumulator rows x N columns in its own TMEM.  Per CTA that halves both the
+// weight bytes streamed from L2 and the shared-memory operand reads per flop.
+//
+// As in tc_program.h the activations live in ONE operand buffer per CTA that every layer's
+// epilogue rewrites in place (64-column chunks, 16 KB, 128-byte-swizzle K-major) and the running
+// layer's accumulator lives in TMEM columns [0, N).  A weight tile may be issued once the epilogues
+// of BOTH CTAs have written the operand chunks it reads and drained the accumulator block it
+// overwrites; progress is published as numbered events on the leader's mbarriers (16 arrivals: 8
+// epilogue warps x 2 CTAs).  Accumulator blocks are handed to the epilogues one by one
+// (`acc_full` ring, multicast tcgen05.commit), so the epilogue of block n overlaps the MMAs of
+// block n+1.
+#pragma once
+#include <stdint.h>
+
+namespace voila {
+
+constexpr int kT2Rows = 128;              // rows per CTA (256 per pair)
+constexpr int kT2ChunkBytes = 128 * 128;  // one 64-column operand chunk
+constexpr int kT2StageBytes = 128 * 128;  // weight ring stage per CTA (TMA box: 128 rows x 128 B)
+constexpr int kT2MaxLayers = 24;
+constexpr int kT2MaxTiles = 512;
+constexpr int kT2EvtRing = 32;
+constexpr int kT2AccRing = 8;
+constexpr int kT2Threads = 384;  // warp 0 producer, 1 MMA issuer (leader), 2 TMEM, 3 spare, 4-11 epilogue
+
+enum T2Epi : int {
+    T2_EPI_HIDDEN = 0,    // y = act(D + bias) -> bf16 -> operand chunks (in place)
+    T2_EPI_REWARD = 1,    // rollout: u = M s ; r = -s^T u
+    T2_EPI_STATE = 2,     // rollout: s' = D + bias ; next operand = [s' ; w_Z]
+    T2_EPI_OBS = 3,       // rollout: o = D + bias -> witness ; next operand = [s' ; w_T]
+    T2_EPI_PROPOSAL = 4,  // belief: s' = D + bias -> proposals (HBM) ; next operand = [s']
+    T2_EPI_SCORE = 5      // belief: logit = <e, D + bias>/lambda + log w -> logits, running max
+};
+
+struct T2Layer {  // what the epilogue needs to know about a layer
+    uint32_t bias_off;  // float offset into the bias buffer
+    uint16_t n_pad;     // padded output width
+    uint16_t bn;        // accumulator block width (the N of this layer's MMAs)
+    uint8_t epi;        // T2Epi
+    uint8_t act;        // voila_act of a hidden layer
+    uint8_t bias_per_action;
+    uint8_t pad;
+};
+
+struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (16 bytes)
+    uint32_t src_row;  // first 128-byte row of the tile in the weight stream (CTA r: + r * rows)
+    uint32_t idesc;    // tcgen05 instruction descriptor (M = 256, N = bn)
+    uint8_t d_col16;   // first accumulator column of the block / 16
+    uint8_t blk;       // index of the block among the step's accumulator blocks (epilogue order)
+    int16_t need;      // event the tile waits for, relative to the step's first event
+    uint8_t kc0;       // first operand chunk
+    uint8_t nk;        // number of 64-wide K chunks held by the stage
+    uint8_t rows8;     // weight rows per CTA per chunk / 8 (= bn / 16)
+    uint8_t flags;     // bit 0: first tile of its block (overwrite); bit 1: last tile of its block
+};
+
+struct T2Header {
+    int n_layers, n_tiles, evt_per_step, a_chunks;
+    int tmem_cols, n_stages, in_chunks, layers_per_step;
+};
+
+}  // namespace voila

@@ -155,8 +155,13 @@ struct ProfScope {
     }
 };
 
+bool use_tc2(const voila_ctx *ctx) {
+    return ctx->prec == VOILA_PREC_BF16 && ctx->tc2 != nullptr &&
+           (ctx->kernel == VOILA_KERNEL_AUTO || ctx->kernel == VOILA_KERNEL_TCGEN05_PAIR);
+}
 bool use_tc(const voila_ctx *ctx) {
-    return ctx->prec == VOILA_PREC_BF16 && ctx->tc != nullptr && ctx->kernel != VOILA_KERNEL_FFMA;
+    return ctx->prec == VOILA_PREC_BF16 && ctx->tc != nullptr && ctx->kernel != VOILA_KERNEL_FFMA &&
+           !use_tc2(ctx);
 }
 
 }  // namespace
@@ -303,6 +308,12 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
                 voila_destroy(ctx);
                 return VOILA_ERR_CUDA;
             }
+            ctx->tc2 = tc2_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
+            if (!ctx->tc2) {
+                ctx->last_cuda_error = err;
+                voila_destroy(ctx);
+                return VOILA_ERR_CUDA;
+            }
         }
     }
     *out = ctx;
@@ -315,6 +326,7 @@ void voila_destroy(voila_ctx *ctx) {
         DeviceGuard guard(ctx->device);
         cudaDeviceSynchronize();
         if (ctx->tc) tc_destroy(ctx->tc);
+        if (ctx->tc2) tc2_destroy(ctx->tc2);
         for (auto &kind : ctx->prof_ev)
             for (auto &pair : kind)
                 for (auto &ev : pair)
@@ -356,8 +368,9 @@ voila_status voila_reserve(voila_ctx *ctx, int P, int Q, int H, int N) {
 }
 
 voila_status voila_set_kernel(voila_ctx *ctx, int kernel) {
-    if (!ctx || kernel < VOILA_KERNEL_AUTO || kernel > VOILA_KERNEL_TCGEN05) return VOILA_ERR_INVALID_ARG;
+    if (!ctx || kernel < VOILA_KERNEL_AUTO || kernel > VOILA_KERNEL_TCGEN05_PAIR) return VOILA_ERR_INVALID_ARG;
     if (kernel == VOILA_KERNEL_TCGEN05 && !ctx->tc) return VOILA_ERR_UNSUPPORTED;
+    if (kernel == VOILA_KERNEL_TCGEN05_PAIR && !ctx->tc2) return VOILA_ERR_UNSUPPORTED;
     ctx->kernel = kernel;
     return VOILA_OK;
 }
@@ -391,13 +404,19 @@ voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
     a.returns_out = returns_out;
     a.final_states_out = final_states_out;
     const int tile_rows = use_tc(ctx) ? 128 : kTileRows;
-    a.tiles = (P + tile_rows - 1) / tile_rows;
+    a.tiles = use_tc2(ctx) ? 2 * ((P + 255) / 256) : (P + tile_rows - 1) / tile_rows;
     double *wsum = reinterpret_cast<double *>(w + L.wsum);
 
     cudaError_t e = launch_weight_sum(weights, P, wsum, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 1;
-    if (use_tc(ctx)) {
+    if (use_tc2(ctx)) {
+        int n = 0;
+        ProfScope prof(ctx, VOILA_K_ROLLOUT, st);
+        e = launch_rollout_tc2(ctx->tc2, ctx->model, a, st, &ctx->last_rollout_kernel, &n);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += n;
+    } else if (use_tc(ctx)) {
         int n = 0;
         ProfScope prof(ctx, VOILA_K_ROLLOUT, st);
         e = launch_rollout_tc(ctx->tc, ctx->model, a, st, &ctx->last_rollout_kernel, &n);

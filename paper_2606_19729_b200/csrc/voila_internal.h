@@ -94,6 +94,8 @@ struct voila_ctx {
     size_t stage_bytes = 0;
     // tcgen05 path (opaque here; owned by rollout_tc.cu)
     void *tc = nullptr;
+    // CTA-pair tcgen05 path (owned by rollout_tc2.cu)
+    void *tc2 = nullptr;
     // profiling rings (voila_set_profiling): event pairs per kernel kind
     bool profiling = false;
     static constexpr int kProfRing = 256;

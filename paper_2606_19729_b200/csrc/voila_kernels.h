@@ -52,4 +52,12 @@ cudaError_t launch_rollout_tc(void *tc, const ModelDev &m, const RolloutArgs &a,
 cudaError_t launch_bu_propose_score_tc(void *tc, const ModelDev &m, const BeliefArgs &a,
                                        cudaStream_t st, int *n_launches);
 
+// ---- rollout_tc2.cu : CTA-pair (cta_group::2) tcgen05 path (bf16 mode) ----
+bool tc2_supported(const voila_model_desc *desc, std::string *why);
+void *tc2_create(const voila_model_desc *desc, int sm_count, std::vector<void *> *allocs,
+                 std::string *err);
+void tc2_destroy(void *tc2);
+cudaError_t launch_rollout_tc2(void *tc2, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
+                               std::string *kernel_name, int *n_launches);
+
 }  // namespace voila

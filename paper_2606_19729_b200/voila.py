@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
-KERNEL_AUTO, KERNEL_FFMA, KERNEL_TCGEN05 = 0, 1, 2
+KERNEL_AUTO, KERNEL_FFMA, KERNEL_TCGEN05, KERNEL_TCGEN05_PAIR = 0, 1, 2, 3
 PREC_FP32, PREC_BF16 = 0, 1
 
 # every symbol include/voila.h declares (tests check that the library exports all of them)

@@ -135,15 +135,18 @@ def _bf16_case(torch, oracle, cfg_idx, P, Q, H, kernel, seed=99, gain=1.0):
     return g, o, e
 
 
-@pytest.mark.parametrize("kernel_name", ["ffma", "tcgen05"])
-@pytest.mark.parametrize("cfg_idx,P,Q,H", [(2, 300, 6, 15), (3, 200, 3, 20), (5, 130, 2, 10)])
+@pytest.mark.parametrize("kernel_name", ["ffma", "tcgen05", "tcgen05_pair"])
+@pytest.mark.parametrize("cfg_idx,P,Q,H", [(2, 300, 6, 15), (3, 200, 3, 20), (5, 130, 2, 10), (5, 700, 3, 6)])
 def test_bf16_mode_within_north_star(torch_cuda, oracle, kernel_name, cfg_idx, P, Q, H):
     """bf16 mode against the fp32 oracle: relative 2e-2 on states, 1e-2 on value estimates."""
     import paper_2606_19729_b200 as vl
-    kernel = vl.KERNEL_FFMA if kernel_name == "ffma" else vl.KERNEL_TCGEN05
+    kernel = {"ffma": vl.KERNEL_FFMA, "tcgen05": vl.KERNEL_TCGEN05,
+              "tcgen05_pair": vl.KERNEL_TCGEN05_PAIR}[kernel_name]
     g, o, e = _bf16_case(torch_cuda, oracle, cfg_idx, P, Q, H, kernel)
     if kernel_name == "tcgen05":
-        assert "tc" in g["kernel"], g["kernel"]
+        assert "rollout_tc_kernel" in g["kernel"], g["kernel"]
+    if kernel_name == "tcgen05_pair":
+        assert "rollout_tc2_kernel" in g["kernel"], g["kernel"]
     assert_close(g["final_states"], o["final_states"], TOL_BF16_STATE, "final states")
     assert value_err(g["values"], o["values"]) <= TOL_BF16_VALUE
     assert value_err(g["returns"], o["returns"]) <= TOL_BF16_STATE
