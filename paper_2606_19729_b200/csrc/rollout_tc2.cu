@@ -29,7 +29,8 @@ namespace {
 using namespace tcc;
 
 struct T2Params {
-    const float *bias;
+    const float *bias;        // global: all bias rows (SiLU hidden layers pre-halved)
+    const float *sbias_init;  // image of the shared-memory bias table (action rows left empty)
     const T2Layer *layers;
     const T2Tile *tiles;
     T2Header hdr;
@@ -51,7 +52,7 @@ struct T2Params {
 };
 
 struct Smem2 {
-    uint32_t a, ring, layers, tiles, bars, misc, total;
+    uint32_t a, ring, layers, tiles, bars, misc, sbias, total;
 };
 __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     Smem2 m;
@@ -61,8 +62,40 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
     m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2Tile) + 15u) & ~15u);
     m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing) * 8;
-    m.total = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
+    m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
+    m.total = m.sbias + (((uint32_t)h.sbias_floats * 4u + 15u) & ~15u);
     return m;
+}
+
+// act(v + b) of a hidden layer.  SiLU layers carry PRE-HALVED biases: with h = (v + b) / 2,
+// x * sigmoid(x) = h + h * tanh(h): one FFMA, one MUFU.TANH, one FFMA per element.
+template <int ACT>
+__device__ __forceinline__ float act_biased(uint32_t v, float b) {
+    if (ACT == VOILA_ACT_SILU) {
+        const float h = fmaf(__uint_as_float(v), 0.5f, b);
+        return fmaf(h, tanh_approx(h), h);
+    }
+    const float x = __uint_as_float(v) + b;
+    return ACT == VOILA_ACT_RELU ? fmaxf(x, 0.0f) : x;
+}
+
+// 32 accumulator columns of this thread's row (already in registers) -> bias (shared memory,
+// broadcast reads) -> activation -> bf16 -> this warp's half of the 64-column operand chunk.
+template <int ACT>
+__device__ __forceinline__ void hidden_store(const uint32_t (&v)[32], const float *sb, uint32_t row_addr, int row,
+                                             int half) {
+    uint32_t o[16];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 b = *reinterpret_cast<const float4 *>(sb + 4 * i);
+        o[2 * i] = pack_bf16x2(act_biased<ACT>(v[4 * i], b.x), act_biased<ACT>(v[4 * i + 1], b.y));
+        o[2 * i + 1] = pack_bf16x2(act_biased<ACT>(v[4 * i + 2], b.z), act_biased<ACT>(v[4 * i + 3], b.w));
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int unit = half * 4 + u;
+        st_shared_v4(row_addr + ((unit ^ (row & 7)) << 4), o[4 * u], o[4 * u + 1], o[4 * u + 2], o[4 * u + 3]);
+    }
 }
 
 // Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
@@ -70,7 +103,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
 // LEADER's mbarriers (remote arrive from the peer CTA).
 __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                             uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
-                                            int warp, int lane, uint32_t rank, int cluster_id, int n_clusters,
+                                            float *sbias, int warp, int lane, uint32_t rank, int cluster_id, int n_clusters,
                                             int n_my_units, int total_steps) {
     const int n_layers = p.hdr.n_layers;
     const uint32_t evt_cl = mapa_u32(smem_u32(evt), 0u);
@@ -151,11 +184,39 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             }
         };
 
+        // Bias rows that depend on the action (one-hot block folded into the bias, R21):
+        // the rows of the NEXT step are fetched mid-step into registers and parked in the other
+        // half of a two-row slot of the shared-memory bias table at the end of the step.
+        const int tid_e = (int)threadIdx.x - 128;
+        float4 pa_reg[2] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
+        auto refresh_issue = [&](int q_next, int t_next) {
+            const int a_next = __ldg(p.seqs + (size_t)q_next * p.H + t_next);
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int li = p.hdr.pa_layer[i];
+                if (li >= 0 && 4 * tid_e < (int)L[li].n_pad)
+                    pa_reg[i] = __ldg(reinterpret_cast<const float4 *>(p.bias + L[li].bias_off +
+                                                                         (size_t)a_next * L[li].n_pad) + tid_e);
+            }
+        };
+        auto refresh_store = [&](int parity) {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int li = p.hdr.pa_layer[i];
+                if (li >= 0 && 4 * tid_e < (int)L[li].n_pad)
+                    *reinterpret_cast<float4 *>(sbias + L[li].sbias_off + parity * (int)L[li].n_pad + 4 * tid_e) =
+                        pa_reg[i];
+            }
+        };
+
         if (n_my_units > 0) {
             load_unit();
+            refresh_issue(q, 0);
             if (half == 0) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
             write_input(0, 0);
             step_reward();
+            refresh_store(0);
+            named_bar_sync(1, 256);
             fence_proxy_async_smem();
             arrive_event();
         }
@@ -163,20 +224,34 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             const int a_t = __ldg(p.seqs + (size_t)q * p.H + t);
             for (int li = 0; li < n_layers; ++li) {
                 const T2Layer l = L[li];
-                const float *bias = p.bias + l.bias_off + (l.bias_per_action ? (size_t)a_t * l.n_pad : 0);
+                const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
-                    wait_layer();
+                    // software-pipelined over the 64-column chunks: the TMEM load of chunk j+1 is in
+                    // flight while chunk j goes through bias / activation / pack / store / event
+                    uint32_t va[32], vb[32];
                     const int chunks = l.n_pad >> 6;
-                    for (int j = 0; j < chunks; ++j) {
-                        const uint32_t taddr = lane_taddr + (uint32_t)(64 * j + 32 * half);
+                    const uint32_t taddr0 = lane_taddr + (uint32_t)(32 * half);
+                    auto do_chunk = [&](const uint32_t (&v)[32], int j) {
                         const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
                         const float *bj = bias + 64 * j + 32 * half;
-                        if (l.act == VOILA_ACT_SILU) hidden_chunk<VOILA_ACT_SILU>(taddr, bj, row_addr, row, half);
-                        else if (l.act == VOILA_ACT_RELU) hidden_chunk<VOILA_ACT_RELU>(taddr, bj, row_addr, row, half);
-                        else hidden_chunk<VOILA_ACT_NONE>(taddr, bj, row_addr, row, half);
+                        if (l.act == VOILA_ACT_SILU) hidden_store<VOILA_ACT_SILU>(v, bj, row_addr, row, half);
+                        else if (l.act == VOILA_ACT_RELU) hidden_store<VOILA_ACT_RELU>(v, bj, row_addr, row, half);
+                        else hidden_store<VOILA_ACT_NONE>(v, bj, row_addr, row, half);
                         fence_proxy_async_smem();
                         tc_fence_before();
                         arrive_event();
+                    };
+                    wait_layer();
+                    tmem_ld32(taddr0, va);
+                    for (int j = 0; j < chunks; j += 2) {
+                        tmem_ld_wait();
+                        if (j + 1 < chunks) tmem_ld32(taddr0 + (uint32_t)(64 * (j + 1)), vb);
+                        do_chunk(va, j);
+                        if (j + 1 < chunks) {
+                            tmem_ld_wait();
+                            if (j + 2 < chunks) tmem_ld32(taddr0 + (uint32_t)(64 * (j + 2)), va);
+                            do_chunk(vb, j + 1);
+                        }
                     }
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
@@ -205,6 +280,9 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 } else if (l.epi == T2_EPI_STATE) {
                     // w_Z(t) is independent of the state: draw it while the output layer's MMAs run
                     if (half == 1) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
+                    if (t + 1 < p.H) refresh_issue(q, t + 1);
+                    else if (unit_i + 1 < n_my_units)
+                        refresh_issue((cluster_id + (unit_i + 1) * n_clusters) / p.blocks_per_q, 0);
                     wait_layer();
                     if (half == 0) {
 #pragma unroll
@@ -214,7 +292,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                 tmem_ld16(lane_taddr + 16 * g, v);
                                 float4 b[4];
 #pragma unroll
-                                for (int i = 0; i < 4; ++i) b[i] = __ldg(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
                                 tmem_ld_wait();
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) {
@@ -243,7 +321,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                 tmem_ld16(lane_taddr + 16 * g, v);
                                 float4 b[4];
 #pragma unroll
-                                for (int i = 0; i < 4; ++i) b[i] = __ldg(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
                                 tmem_ld_wait();
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) {
@@ -308,6 +386,8 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         write_input(0, 0);
                         step_reward();
                     }
+                    refresh_store((step + 1) & 1);
+                    named_bar_sync(1, 256);
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
@@ -332,6 +412,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(smem + map.misc);
     double *red_g = reinterpret_cast<double *>(smem + map.misc + 16);
     float *red_w = reinterpret_cast<float *>(smem + map.misc + 16 + 4 * 8);
+    float *sbias = reinterpret_cast<float *>(smem + map.sbias);
     const uint32_t a_u32 = smem_u32(smem + map.a), ring_u32 = smem_u32(smem + map.ring);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -346,6 +427,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
         src = reinterpret_cast<const uint32_t *>(p.tiles);
         dst = reinterpret_cast<uint32_t *>(T);
         for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2Tile) / 4); i += kT2Threads) dst[i] = src[i];
+        for (int i = threadIdx.x; i < p.hdr.sbias_floats; i += kT2Threads) sbias[i] = p.sbias_init[i];
         uint4 *az = reinterpret_cast<uint4 *>(smem + map.a);
         for (int i = threadIdx.x; i < p.hdr.a_chunks * kT2ChunkBytes / 16; i += kT2Threads)
             az[i] = make_uint4(0u, 0u, 0u, 0u);
@@ -375,6 +457,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     const int n_my_units = (p.n_units - cluster_id + n_clusters - 1) / n_clusters;
     const int total_steps = n_my_units * p.H;
 
+    // the epilogue warpgroups take the registers the producer / issuer warpgroup does not need
+    if (warp < 4) {
+    setmaxnreg_dec<56>();
     if (warp == 0) {
         // ===== producer: this CTA's half of every weight tile, in issue order, once per step =====
         if (lane == 0) {
@@ -434,8 +519,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
                 blk_base += p.hdr.layers_per_step;
             }
         }
-    } else if (warp >= 4) {
-        t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, warp, lane, rank, cluster_id,
+    }
+    } else {
+        setmaxnreg_inc<224>();
+        t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
                     n_clusters, n_my_units, total_steps);
     }
 
@@ -474,11 +561,11 @@ int rup(int x, int m) { return (x + m - 1) / m * m; }
 std::vector<int> hidden_blocks(int n, int policy) {
     std::vector<int> b;
     int left = n;
-    if (policy == 1) {  // all 256
+    if (policy == 0) {  // default: all 256 (N < 256 MMAs run below the tensor pipe's floor: A re-read)
         while (left >= 256) { b.push_back(256); left -= 256; }
     } else if (policy == 2) {  // all 128
         while (left >= 128) { b.push_back(128); left -= 128; }
-    } else {  // 128, 128, then 256s
+    } else {  // 1: 128, 128, then 256s
         for (int i = 0; i < 2 && left >= 128; ++i) { b.push_back(128); left -= 128; }
         while (left >= 256) { b.push_back(256); left -= 256; }
     }
@@ -491,7 +578,10 @@ struct Builder2 {
     std::vector<T2Layer> layers;
     std::vector<T2Tile> tiles;
     std::vector<uint8_t> wstream;  // rows of 128 bytes
-    std::vector<float> bias;
+    std::vector<float> bias;        // global: every bias row (SiLU hidden layers pre-halved)
+    std::vector<float> sbias_init;  // shared-memory table image: constant rows; 2 empty rows per action layer
+    int pa_layer[2] = {-1, -1};
+    bool too_many_pa = false;
     int evt = 0;
     int col_free[512];
     int a_ready[8];
@@ -514,10 +604,21 @@ struct Builder2 {
         l.epi = (uint8_t)epi;
         l.act = (uint8_t)act;
         l.bias_per_action = bias_rows > 1;
+        const float bscale = (hidden && act == VOILA_ACT_SILU) ? 0.5f : 1.0f;  // see act_biased()
         for (int r = 0; r < bias_rows; ++r)
-            for (int j = 0; j < n_pad; ++j) bias.push_back((b && j < n0) ? b[(size_t)r * n0 + j] : 0.0f);
+            for (int j = 0; j < n_pad; ++j)
+                bias.push_back((b && j < n0) ? bscale * b[(size_t)r * n0 + j] : 0.0f);
         a_chunks = std::max(a_chunks, std::max(kc_n, hidden ? n_pad / 64 : 1));
         const int li = (int)layers.size();
+        l.sbias_off = (uint32_t)sbias_init.size();
+        if (bias_rows > 1) {
+            sbias_init.resize(sbias_init.size() + 2 * (size_t)n_pad, 0.0f);
+            if (pa_layer[0] < 0) pa_layer[0] = li;
+            else if (pa_layer[1] < 0) pa_layer[1] = li;
+            else too_many_pa = true;
+        } else {
+            sbias_init.insert(sbias_init.end(), bias.end() - n_pad, bias.end());
+        }
         std::vector<int> blocks = hidden ? hidden_blocks(n_pad, policy) : std::vector<int>{n_pad};
         l.bn = (uint16_t)blocks[0];
         std::vector<T2Tile> lt;
@@ -588,7 +689,7 @@ struct Builder2 {
 
 struct T2Handle {
     T2Header hdr{};
-    void *d_wstream = nullptr, *d_bias = nullptr, *d_layers = nullptr, *d_tiles = nullptr;
+    void *d_wstream = nullptr, *d_bias = nullptr, *d_sbias = nullptr, *d_layers = nullptr, *d_tiles = nullptr;
     size_t smem_bytes = 0;
     int max_clusters = 0;
     CUtensorMap wmap;
@@ -637,7 +738,7 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
     add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
     add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
-    if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles)
+    if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa)
         return fail("model too deep for the tcgen05 program tables");
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
     pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
@@ -648,6 +749,9 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     h->hdr.evt_per_step = pb.evt;
     h->hdr.a_chunks = pb.a_chunks;
     h->hdr.in_chunks = rup(S + Nz, 64) / 64;
+    h->hdr.sbias_floats = (int)pb.sbias_init.size();
+    h->hdr.pa_layer[0] = pb.pa_layer[0];
+    h->hdr.pa_layer[1] = pb.pa_layer[1];
     int max_n = 32;
     for (const T2Layer &l : pb.layers) max_n = std::max(max_n, (int)l.n_pad);
     int cols = 32;
@@ -668,6 +772,7 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     };
     if (!upload(pb.wstream.data(), pb.wstream.size(), &h->d_wstream) ||
         !upload(pb.bias.data(), pb.bias.size() * sizeof(float), &h->d_bias) ||
+        !upload(pb.sbias_init.data(), pb.sbias_init.size() * sizeof(float), &h->d_sbias) ||
         !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &h->d_layers) ||
         !upload(pb.tiles.data(), pb.tiles.size() * sizeof(T2Tile), &h->d_tiles) ||
         cudaFuncSetAttribute(rollout_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -718,6 +823,7 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
     T2Params p{};
     p.bias = reinterpret_cast<const float *>(h->d_bias);
+    p.sbias_init = reinterpret_cast<const float *>(h->d_sbias);
     p.layers = reinterpret_cast<const T2Layer *>(h->d_layers);
     p.tiles = reinterpret_cast<const T2Tile *>(h->d_tiles);
     p.hdr = h->hdr;

@@ -38,7 +38,8 @@ enum T2Epi : int {
 };
 
 struct T2Layer {  // what the epilogue needs to know about a layer
-    uint32_t bias_off;  // float offset into the bias buffer
+    uint32_t bias_off;   // float offset into the global bias buffer (per-action layers: A rows)
+    uint32_t sbias_off;  // float offset into the shared-memory bias table (per-action layers: 2 rows)
     uint16_t n_pad;     // padded output width
     uint16_t bn;        // accumulator block width (the N of this layer's MMAs)
     uint8_t epi;        // T2Epi
@@ -62,6 +63,9 @@ struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block 
 struct T2Header {
     int n_layers, n_tiles, evt_per_step, a_chunks;
     int tmem_cols, n_stages, in_chunks, layers_per_step;
+    int sbias_floats;     // size of the shared-memory bias table
+    int pa_layer[2];      // layers whose bias row depends on the action (-1: none)
+    int reserved;
 };
 
 }  // namespace voila
