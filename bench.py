@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-DEFAULT_CONFIG = 2
+DEFAULT_CONFIG = 5  # the largest config: the one north_star's >= 50 %-of-peak target is stated on
 METRIC = "rollout_steps_per_sec"
 UNIT = "particle*sequence*depth steps/s"
 
@@ -191,7 +191,12 @@ def run_voila(args):
     parts = ctx.to_particles(inp.particles)
     bu_parts = parts if chain else ctx.to_particles(inp.bu_particles)
     seqs = torch.from_numpy(inp.action_seqs).to(dev)
-    obs_all = torch.from_numpy(synth.observations_for_steps(cfg, args.warmup + args.steps + 1)).to(dev)
+    # one observation per planning step; rows padded to 16 bytes (the C ABI wants aligned pointers)
+    obs_np = synth.observations_for_steps(cfg, args.warmup + args.steps + 1)
+    o_pad = (cfg.O + 3) // 4 * 4
+    obs_buf = torch.zeros(obs_np.shape[0], o_pad, dtype=torch.float32, device=dev)
+    obs_buf[:, :cfg.O] = torch.from_numpy(obs_np).to(dev)
+    obs_all = [obs_buf[k, :cfg.O] for k in range(obs_np.shape[0])]
     bu_w = None if inp.bu_weights is None else torch.from_numpy(inp.bu_weights).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
     stream = torch.cuda.current_stream(dev)
@@ -256,7 +261,7 @@ def run_voila(args):
     h_parts = parts.cpu().pin_memory()
     h_bu = h_parts if chain else bu_parts.cpu().pin_memory()
     h_seqs = torch.from_numpy(inp.action_seqs).pin_memory()
-    h_obs = obs_all.cpu().pin_memory()
+    h_obs = obs_buf.cpu().pin_memory()
     h_w = None if bu_w is None else bu_w.cpu().pin_memory()
     h_vals = torch.empty(Q, dtype=torch.float32).pin_memory()
     h_pout = torch.empty_like(h_bu).pin_memory()
@@ -267,7 +272,7 @@ def run_voila(args):
 
     def e2e_step(k):
         ctx.voila_rollout_values_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals)
-        ctx.voila_belief_update_host(h_bu, inp.bu_action, h_obs[k % h_obs.shape[0]], h_w,
+        ctx.voila_belief_update_host(h_bu, inp.bu_action, h_obs[k % h_obs.shape[0], :cfg.O], h_w,
                                      seed0 + 2 * k + 1, h_pout, None, h_anc, h_le, h_st)
 
     e2e_step(0)

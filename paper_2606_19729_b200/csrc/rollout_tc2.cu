@@ -28,6 +28,17 @@ namespace {
 
 using namespace tcc;
 
+// Optional wait-cycle trace (build with -DVOILA_T2_TRACE): where the producer, the MMA issuer and
+// the epilogue warps of cluster 0 spend their time waiting.  Read with voila_debug_t2_trace().
+#ifdef VOILA_T2_TRACE
+__device__ unsigned long long g_t2_trace[64];
+#define T2_TRACE_T0() const long long _t0 = clock64()
+#define T2_TRACE_ADD(var) var += clock64() - _t0
+#else
+#define T2_TRACE_T0()
+#define T2_TRACE_ADD(var)
+#endif
+
 struct T2Params {
     const float *bias;        // global: all bias rows (SiLU hidden layers pre-halved)
     const float *sbias_init;  // image of the shared-memory bias table (action rows left empty)
@@ -61,7 +72,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     m.layers = m.ring + (uint32_t)h.n_stages * kT2StageBytes;
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
     m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2Tile) + 15u) & ~15u);
-    m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing) * 8;
+    m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing + kT2FreeRing) * 8;
     m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
     m.total = m.sbias + (((uint32_t)h.sbias_floats * 4u + 15u) & ~15u);
     return m;
@@ -119,7 +130,10 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         float G = 0.0f, disc = 1.0f, w_row = 0.0f;
         int ev = 0, t = 0, unit_i = 0, q = 0, blk = 0, p_idx = 0;
         bool valid = false;
-        uint32_t ld_seq = 0;
+        long long tr_layer = 0, tr_free = 0, tr_bar = 0;
+        const long long tr_start = clock64();
+        uint32_t ld_seq = 0, free_seq = 0;
+        uint64_t *cfree = layer_done + kT2AccRing;
 
         auto arrive_event = [&]() {
             __syncwarp();
@@ -127,7 +141,9 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             ++ev;
         };
         auto wait_layer = [&]() {
+            T2_TRACE_T0();
             mbar_wait(&layer_done[ld_seq & (kT2AccRing - 1)], (ld_seq >> 3) & 1u);
+            T2_TRACE_ADD(tr_layer);
             ++ld_seq;
             tc_fence_after();
         };
@@ -212,7 +228,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         if (n_my_units > 0) {
             load_unit();
             refresh_issue(q, 0);
-            if (half == 0) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
+            if (half == 0) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
             write_input(0, 0);
             step_reward();
             refresh_store(0);
@@ -231,7 +247,19 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     uint32_t va[32], vb[32];
                     const int chunks = l.n_pad >> 6;
                     const uint32_t taddr0 = lane_taddr + (uint32_t)(32 * half);
+                    int free_have = 0;
                     auto do_chunk = [&](const uint32_t (&v)[32], int j) {
+                        if (j < (int)l.wait_chunks) {  // in-place store: the last block must have read chunk j
+                            const int need_free = j / (int)l.free_nk + 1;
+                            while (free_have < need_free) {
+                                T2_TRACE_T0();
+                                mbar_wait(&cfree[free_seq & (kT2FreeRing - 1)], (free_seq >> 3) & 1u);
+                                T2_TRACE_ADD(tr_free);
+                                ++free_seq;
+                                ++free_have;
+                            }
+                            tc_fence_after();
+                        }
                         const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
                         const float *bj = bias + 64 * j + 32 * half;
                         if (l.act == VOILA_ACT_SILU) hidden_store<VOILA_ACT_SILU>(v, bj, row_addr, row, half);
@@ -241,15 +269,20 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         tc_fence_before();
                         arrive_event();
                     };
-                    wait_layer();
-                    tmem_ld32(taddr0, va);
+                    // accumulator blocks are handed over one by one: chunk c may be loaded once the
+                    // block it belongs to has been committed (l.blk_mask: chunks that start a block)
+                    auto fetch = [&](int c, uint32_t (&buf)[32]) {
+                        if ((l.blk_mask >> c) & 1u) wait_layer();
+                        tmem_ld32(taddr0 + (uint32_t)(64 * c), buf);
+                    };
+                    fetch(0, va);
                     for (int j = 0; j < chunks; j += 2) {
                         tmem_ld_wait();
-                        if (j + 1 < chunks) tmem_ld32(taddr0 + (uint32_t)(64 * (j + 1)), vb);
+                        if (j + 1 < chunks) fetch(j + 1, vb);
                         do_chunk(va, j);
                         if (j + 1 < chunks) {
                             tmem_ld_wait();
-                            if (j + 2 < chunks) tmem_ld32(taddr0 + (uint32_t)(64 * (j + 2)), va);
+                            if (j + 2 < chunks) fetch(j + 2, va);
                             do_chunk(vb, j + 1);
                         }
                     }
@@ -279,7 +312,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     arrive_event();
                 } else if (l.epi == T2_EPI_STATE) {
                     // w_Z(t) is independent of the state: draw it while the output layer's MMAs run
-                    if (half == 1) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
+                    if (half == 1) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
                     if (t + 1 < p.H) refresh_issue(q, t + 1);
                     else if (unit_i + 1 < n_my_units)
                         refresh_issue((cluster_id + (unit_i + 1) * n_clusters) / p.blocks_per_q, 0);
@@ -311,7 +344,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 } else {  // T2_EPI_OBS: last layer of the step
                     const bool last_step = (t == p.H - 1);
                     if (half == 0 && !last_step)
-                        gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)(t + 1), kStreamRolloutT, Nz);
+                        gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)(t + 1), kStreamRolloutT, Nz);
                     wait_layer();
                     if (half == 1) {
 #pragma unroll
@@ -379,7 +412,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         ++unit_i;
                         if (unit_i < n_my_units) {
                             load_unit();
-                            if (half == 0) gen_noise(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
+                            if (half == 0) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
                         }
                     }
                     if (unit_i < n_my_units) {
@@ -387,13 +420,27 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         step_reward();
                     }
                     refresh_store((step + 1) & 1);
-                    named_bar_sync(1, 256);
+                    {
+                        T2_TRACE_T0();
+                        named_bar_sync(1, 256);
+                        T2_TRACE_ADD(tr_bar);
+                    }
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
                 }
             }
         }
+#ifdef VOILA_T2_TRACE
+        if (cluster_id == 0 && lane == 0) {
+            unsigned long long *o = g_t2_trace + 16 + ((int)rank * 8 + ew) * 3;
+            o[0] = tr_layer;
+            o[1] = tr_free;
+            o[2] = tr_bar;
+            if (ew == 0 && rank == 0) g_t2_trace[15] = clock64() - tr_start;
+        }
+#endif
+        (void)tr_layer; (void)tr_free; (void)tr_bar; (void)tr_start;
     }
 }
 
@@ -440,7 +487,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
             mbar_init(&empty[s], 1);
         }
         for (int i = 0; i < kT2EvtRing; ++i) mbar_init(&evt[i], 16);  // 8 epilogue warps x 2 CTAs
-        for (int i = 0; i < kT2AccRing; ++i) mbar_init(&layer_done[i], 1);
+        for (int i = 0; i < kT2AccRing + kT2FreeRing; ++i) mbar_init(&layer_done[i], 1);  // + cfree ring
         fence_barrier_init();
     }
     if (warp == 2) {
@@ -464,10 +511,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
         // ===== producer: this CTA's half of every weight tile, in issue order, once per step =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
+            long long tr_empty = 0;
+            const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
                     const T2Tile t = T[i];
-                    mbar_wait(&empty[stage], phase ^ 1u);
+                    {
+                        T2_TRACE_T0();
+                        mbar_wait(&empty[stage], phase ^ 1u);
+                        T2_TRACE_ADD(tr_empty);
+                    }
                     if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2u * kT2StageBytes);
                     const int rows = (int)t.nk * (int)t.rows8 * 8;
                     tma_load_2d_2cta(smem + map.ring + stage * kT2StageBytes, &wmap, &full[stage], 0,
@@ -478,22 +531,39 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
                     }
                 }
             }
+#ifdef VOILA_T2_TRACE
+            if (cluster_id == 0) {
+                g_t2_trace[(int)rank * 2] = tr_empty;
+                g_t2_trace[(int)rank * 2 + 1] = clock64() - tr_start;
+            }
+#endif
+            (void)tr_empty; (void)tr_start;
         }
     } else if (warp == 1) {
         // ===== MMA issuer: leader CTA only =====
         if (lane == 0 && rank == 0) {
             uint32_t stage = 0, phase = 0;
             int waited = -1, base = 1, blk_base = 0;
+            uint32_t free_seq = 0;
+            uint64_t *cfree = layer_done + kT2AccRing;
+            long long tr_evt = 0, tr_full = 0;
+            const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 T2Tile t = T[0];
                 for (int i = 0; i < n_tiles; ++i) {
                     const T2Tile nxt = T[i + 1 < n_tiles ? i + 1 : 0];  // prefetch the next record
                     const int need = base + (int)t.need;
                     if (need > waited) {
+                        T2_TRACE_T0();
                         mbar_wait(&evt[need & (kT2EvtRing - 1)], (uint32_t)(need / kT2EvtRing) & 1u);
+                        T2_TRACE_ADD(tr_evt);
                         waited = need;
                     }
-                    mbar_wait(&full[stage], phase);
+                    {
+                        T2_TRACE_T0();
+                        mbar_wait(&full[stage], phase);
+                        T2_TRACE_ADD(tr_full);
+                    }
                     tc_fence_after();
                     const uint32_t d = tmem_base + (uint32_t)t.d_col16 * 16u;
                     const uint32_t chunk_b = (uint32_t)t.rows8 * 1024u;  // bytes of one K chunk in the stage
@@ -508,6 +578,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
                         }
                     }
                     umma_commit_2cta(&empty[stage], 3);
+                    if (t.flags & 4u) {
+                        umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
+                        ++free_seq;
+                    }
                     if (t.flags & 2u) umma_commit_2cta(&layer_done[(blk_base + (int)t.blk) & (kT2AccRing - 1)], 3);
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
@@ -516,8 +590,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
                     t = nxt;
                 }
                 base += p.hdr.evt_per_step;
-                blk_base += p.hdr.layers_per_step;
+                blk_base += p.hdr.blocks_per_step;
             }
+#ifdef VOILA_T2_TRACE
+            if (cluster_id == 0) {
+                g_t2_trace[4] = tr_evt;
+                g_t2_trace[5] = tr_full;
+                g_t2_trace[6] = clock64() - tr_start;
+            }
+#endif
+            (void)tr_evt; (void)tr_full; (void)tr_start;
         }
     }
     } else {
@@ -561,6 +643,8 @@ int rup(int x, int m) { return (x + m - 1) / m * m; }
 std::vector<int> hidden_blocks(int n, int policy) {
     std::vector<int> b;
     int left = n;
+    if (policy == 0 && n <= 256) policy = 2;  // a 256-wide layer as two 128 blocks: the epilogue of the
+                                              // first overlaps the MMAs of the second (measured, CFG3)
     if (policy == 0) {  // default: all 256 (N < 256 MMAs run below the tensor pipe's floor: A re-read)
         while (left >= 256) { b.push_back(256); left -= 256; }
     } else if (policy == 2) {  // all 128
@@ -582,10 +666,12 @@ struct Builder2 {
     std::vector<float> sbias_init;  // shared-memory table image: constant rows; 2 empty rows per action layer
     int pa_layer[2] = {-1, -1};
     bool too_many_pa = false;
+    bool bad_order = false;
     int evt = 0;
     int col_free[512];
     int a_ready[8];
     int a_chunks = 1;
+    int n_blocks = 0;  // accumulator blocks of the step so far (each is handed to the epilogues on its own)
     int policy = 0;
 
     Builder2() {
@@ -620,7 +706,6 @@ struct Builder2 {
             sbias_init.insert(sbias_init.end(), bias.end() - n_pad, bias.end());
         }
         std::vector<int> blocks = hidden ? hidden_blocks(n_pad, policy) : std::vector<int>{n_pad};
-        l.bn = (uint16_t)blocks[0];
         std::vector<T2Tile> lt;
         int n_start = 0;
         for (size_t bi = 0; bi < blocks.size(); ++bi) {
@@ -634,7 +719,7 @@ struct Builder2 {
                 t.src_row = (uint32_t)(wstream.size() / 128);
                 t.idesc = umma_idesc_bf16_m256((uint32_t)bn);
                 t.d_col16 = (uint8_t)(n_start / 16);
-                t.blk = (uint8_t)li;
+                t.blk = (uint8_t)(n_blocks + (int)bi);
                 t.kc0 = (uint8_t)kc0;
                 t.nk = (uint8_t)nk;
                 t.rows8 = (uint8_t)(half / 8);
@@ -664,12 +749,41 @@ struct Builder2 {
         }
         std::stable_sort(lt.begin(), lt.end(), [](const T2Tile &x, const T2Tile &y) { return x.need < y.need; });
         bool seen[16] = {};
-        for (T2Tile &t : lt) {
-            const int bi = t.flags >> 4;
-            t.flags = seen[bi] ? 0 : 1;
+        int last_of[16];
+        for (size_t i = 0; i < lt.size(); ++i) {
+            const int bi = lt[i].flags >> 4;
+            lt[i].flags = seen[bi] ? 0 : 1;
             seen[bi] = true;
+            last_of[bi] = (int)i;
         }
-        lt.back().flags |= 2;  // the layer's last tile hands the accumulator to the epilogues
+        // the last tile of every block hands that block of the accumulator to the epilogues
+        for (size_t bi = 0; bi < blocks.size(); ++bi) lt[last_of[bi]].flags |= 2;
+        {
+            int c = 0;
+            for (size_t bi = 0; bi < blocks.size(); ++bi) {
+                if (hidden) l.blk_mask |= (uint8_t)(1u << c);
+                c += blocks[bi] / 64;
+            }
+        }
+        n_blocks += (int)blocks.size();
+        if (hidden && blocks.size() > 1) {
+            const int last_bi = (int)blocks.size() - 1, last_half = blocks[last_bi] / 2;
+            const int nk_last = std::max(1, std::min(4, 128 / last_half));
+            const int early = (n_pad - blocks[last_bi]) / 64;
+            l.free_nk = (uint8_t)nk_last;
+            l.wait_chunks = (uint8_t)std::min(early, kc_n);
+            int prev_kc0 = -1, n_sig = 0;
+            for (T2Tile &t : lt) {
+                if ((int)t.blk != n_blocks - 1) continue;
+                if ((int)t.kc0 <= prev_kc0) bad_order = true;  // signals must arrive in chunk order
+                prev_kc0 = t.kc0;
+                if ((int)t.kc0 < (int)l.wait_chunks) {
+                    t.flags |= 4;
+                    ++n_sig;
+                }
+            }
+            if (n_sig > kT2FreeRing) bad_order = true;
+        }
         tiles.insert(tiles.end(), lt.begin(), lt.end());
         layers.push_back(l);
         if (hidden) {
@@ -738,13 +852,14 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
     add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
     add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
-    if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa)
+    if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa || pb.bad_order)
         return fail("model too deep for the tcgen05 program tables");
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
     pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
 
     T2Handle *h = new T2Handle();
-    h->hdr.n_layers = h->hdr.layers_per_step = (int)pb.layers.size();
+    h->hdr.n_layers = (int)pb.layers.size();
+    h->hdr.blocks_per_step = pb.n_blocks;
     h->hdr.n_tiles = (int)pb.tiles.size();
     h->hdr.evt_per_step = pb.evt;
     h->hdr.a_chunks = pb.a_chunks;
@@ -852,3 +967,9 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
 }
 
 }  // namespace voila
+
+#ifdef VOILA_T2_TRACE
+extern "C" __attribute__((visibility("default"))) int voila_debug_t2_trace(unsigned long long *out64) {
+    return (int)cudaMemcpyFromSymbol(out64, voila::g_t2_trace, sizeof(unsigned long long) * 64);
+}
+#endif

@@ -12,8 +12,10 @@
 // of BOTH CTAs have written the operand chunks it reads and drained the accumulator block it
 // overwrites; progress is published as numbered events on the leader's mbarriers (16 arrivals: 8
 // epilogue warps x 2 CTAs).  Accumulator blocks are handed to the epilogues one by one
-// (`acc_full` ring, multicast tcgen05.commit), so the epilogue of block n overlaps the MMAs of
-// block n+1.
+// (`layer_done` ring, multicast tcgen05.commit), so the epilogue of block n overlaps the MMAs of
+// block n+1.  Because the operand buffer is rewritten in place, the epilogue of an earlier block
+// may store output chunk c only after the LAST block's tile that reads operand chunk c has
+// retired: those tiles commit "operand chunk free" signals (`cfree` ring) in chunk order.
 #pragma once
 #include <stdint.h>
 
@@ -26,6 +28,7 @@ constexpr int kT2MaxLayers = 24;
 constexpr int kT2MaxTiles = 512;
 constexpr int kT2EvtRing = 32;
 constexpr int kT2AccRing = 8;
+constexpr int kT2FreeRing = 8;
 constexpr int kT2Threads = 384;  // warp 0 producer, 1 MMA issuer (leader), 2 TMEM, 3 spare, 4-11 epilogue
 
 enum T2Epi : int {
@@ -41,28 +44,32 @@ struct T2Layer {  // what the epilogue needs to know about a layer
     uint32_t bias_off;   // float offset into the global bias buffer (per-action layers: A rows)
     uint32_t sbias_off;  // float offset into the shared-memory bias table (per-action layers: 2 rows)
     uint16_t n_pad;     // padded output width
-    uint16_t bn;        // accumulator block width (the N of this layer's MMAs)
+    uint8_t free_nk;    // K chunks per tile of the layer's LAST accumulator block (see wait_chunks)
+    uint8_t wait_chunks;  // output chunks [0, wait_chunks) belong to earlier blocks and overwrite operand
+                          // chunks the last block's MMAs still read: chunk c may be stored once
+                          // c / free_nk + 1 "operand chunk free" signals of this layer have arrived
     uint8_t epi;        // T2Epi
     uint8_t act;        // voila_act of a hidden layer
     uint8_t bias_per_action;
-    uint8_t pad;
+    uint8_t blk_mask;   // hidden layers: bit c set = 64-column chunk c is the first of an accumulator block
 };
 
 struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (16 bytes)
     uint32_t src_row;  // first 128-byte row of the tile in the weight stream (CTA r: + r * rows)
     uint32_t idesc;    // tcgen05 instruction descriptor (M = 256, N = bn)
     uint8_t d_col16;   // first accumulator column of the block / 16
-    uint8_t blk;       // index of the block among the step's accumulator blocks (epilogue order)
+    uint8_t blk;       // index of the accumulator block among the step's blocks (epilogue order)
     int16_t need;      // event the tile waits for, relative to the step's first event
     uint8_t kc0;       // first operand chunk
     uint8_t nk;        // number of 64-wide K chunks held by the stage
     uint8_t rows8;     // weight rows per CTA per chunk / 8 (= bn / 16)
-    uint8_t flags;     // bit 0: first tile of its block (overwrite); bit 1: last tile of its block
+    uint8_t flags;     // bit 0: first tile of its block (overwrite); bit 1: last tile of its block;
+                       // bit 2: commit an "operand chunk free" signal after this tile
 };
 
 struct T2Header {
     int n_layers, n_tiles, evt_per_step, a_chunks;
-    int tmem_cols, n_stages, in_chunks, layers_per_step;
+    int tmem_cols, n_stages, in_chunks, blocks_per_step;  // accumulator blocks (hand-offs) per step
     int sbias_floats;     // size of the shared-memory bias table
     int pa_layer[2];      // layers whose bias row depends on the action (-1: none)
     int reserved;

@@ -78,6 +78,29 @@ __device__ __forceinline__ void gen_noise(uint32_t (&nz)[16], uint64_t seed, uin
     }
 }
 
+// Eight normals (Philox blocks 2u and 2u+1) packed as one 16-byte operand unit.  Deliberately NOT
+// inlined: the Philox rounds + Box-Muller of a block are ~160 instructions, and the pair kernel
+// draws noise at several places of its epilogue; one copy keeps the kernel inside the instruction
+// cache (the inlined form was 3/4 of the kernel's SASS).
+static __device__ __noinline__ uint4 noise_unit8(uint64_t seed, uint32_t p, uint32_t q, uint32_t t, uint32_t stream,
+                                          uint32_t u) {
+    float z[8];
+    normals4<true>(seed, p, q, t, stream, 2u * u, z);
+    normals4<true>(seed, p, q, t, stream, 2u * u + 1u, z + 4);
+    return make_uint4(pack_bf16x2(z[0], z[1]), pack_bf16x2(z[2], z[3]), pack_bf16x2(z[4], z[5]),
+                      pack_bf16x2(z[6], z[7]));
+}
+__device__ __forceinline__ void gen_noise_call(uint32_t (&nz)[16], uint64_t seed, uint32_t p, uint32_t q,
+                                               uint32_t t, uint32_t stream, int Nz) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        if (8 * u < Nz) {
+            const uint4 v = noise_unit8(seed, p, q, t, stream, (uint32_t)u);
+            nz[4 * u] = v.x; nz[4 * u + 1] = v.y; nz[4 * u + 2] = v.z; nz[4 * u + 3] = v.w;
+        }
+    }
+}
+
 // R(s, a) from the bf16 state for the non-quadratic reward kinds (R14).
 __device__ __forceinline__ float reward_from_state(const uint32_t *st, int S, int kind,
                                                    const float *__restrict__ param) {
