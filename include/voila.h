@@ -207,6 +207,8 @@ voila_status voila_belief_update_host(voila_ctx *ctx, const void *particles, int
  * since creation, and the name / launch geometry of the last rollout kernel. */
 uint64_t voila_launch_count(const voila_ctx *ctx);
 const char *voila_last_rollout_kernel(const voila_ctx *ctx);
+/* Name of the propose+score kernel the last voila_belief_update launched. */
+const char *voila_last_belief_kernel(const voila_ctx *ctx);
 
 /* Kernel timing for bench.py's roofline line.  When profiling is on, the library brackets each
  * launch of its main kernels with CUDA events on the caller's stream (a ring of 256 pairs per

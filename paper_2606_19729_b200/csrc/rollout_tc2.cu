@@ -60,6 +60,15 @@ struct T2Params {
     int reward_kind;
     const float *reward_param;
     const float *action_cost;
+    // belief-update program (propose + score): one unit = 256 particles, one step per unit
+    int bu_action;
+    const float *bu_e;        // f(o), [d]
+    uint16_t *bu_proposals;   // [N][S] bf16
+    float *bu_logits;         // [N]
+    int *bu_max_ordered;      // [1]
+    double *bu_part_wsum;     // [(N + 31) / 32]: prior-weight sums per 32 particles
+    float inv_lambda;
+    int d;
 };
 
 struct Smem2 {
@@ -109,6 +118,83 @@ __device__ __forceinline__ void hidden_store(const uint32_t (&v)[32], const floa
     }
 }
 
+// Synchronisation state of one epilogue warp: the numbered events it publishes on the leader's
+// mbarriers, and its positions in the accumulator hand-off and operand-chunk-free rings.
+struct EpiSync {
+    uint32_t evt_cl;       // cluster address of the leader's event ring
+    uint64_t *layer_done;  // accumulator hand-off ring (this CTA's copy; multicast commits)
+    uint64_t *cfree;       // operand-chunk-free ring
+    int ev = 0;
+    uint32_t ld_seq = 0, free_seq = 0;
+    int lane;
+    long long tr_layer = 0, tr_free = 0, tr_bar = 0;  // wait-cycle trace (VOILA_T2_TRACE)
+
+    __device__ __forceinline__ void arrive_event() {
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(evt_cl + 8u * (uint32_t)(ev & (kT2EvtRing - 1)));
+        ++ev;
+    }
+    __device__ __forceinline__ void wait_layer() {
+        T2_TRACE_T0();
+        mbar_wait(&layer_done[ld_seq & (kT2AccRing - 1)], (ld_seq >> 3) & 1u);
+        T2_TRACE_ADD(tr_layer);
+        ++ld_seq;
+        tc_fence_after();
+    }
+    __device__ __forceinline__ void wait_chunk_free() {
+        T2_TRACE_T0();
+        mbar_wait(&cfree[free_seq & (kT2FreeRing - 1)], (free_seq >> 3) & 1u);
+        T2_TRACE_ADD(tr_free);
+        ++free_seq;
+    }
+};
+
+// Epilogue of a hidden layer for this warp's 32 rows x one 32-column half of every 64-column chunk:
+// software-pipelined over the chunks (the TMEM load of chunk j+1 is in flight while chunk j goes
+// through bias / activation / pack / store / event).
+__device__ __forceinline__ void epi_hidden_layer(EpiSync &es, const T2Layer &l, const float *bias, uint32_t a_u32,
+                                                 uint32_t lane_taddr, int row, int half) {
+    uint32_t va[32], vb[32];
+    const int chunks = l.n_pad >> 6;
+    const uint32_t taddr0 = lane_taddr + (uint32_t)(32 * half);
+    int free_have = 0;
+    auto do_chunk = [&](const uint32_t (&v)[32], int j) {
+        if (j < (int)l.wait_chunks) {  // in-place store: the last block must have read chunk j
+            const int need_free = j / (int)l.free_nk + 1;
+            while (free_have < need_free) {
+                es.wait_chunk_free();
+                ++free_have;
+            }
+            tc_fence_after();
+        }
+        const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
+        const float *bj = bias + 64 * j + 32 * half;
+        if (l.act == VOILA_ACT_SILU) hidden_store<VOILA_ACT_SILU>(v, bj, row_addr, row, half);
+        else if (l.act == VOILA_ACT_RELU) hidden_store<VOILA_ACT_RELU>(v, bj, row_addr, row, half);
+        else hidden_store<VOILA_ACT_NONE>(v, bj, row_addr, row, half);
+        fence_proxy_async_smem();
+        tc_fence_before();
+        es.arrive_event();
+    };
+    // accumulator blocks are handed over one by one: chunk c may be loaded once the block it
+    // belongs to has been committed (l.blk_mask: chunks that start a block)
+    auto fetch = [&](int c, uint32_t (&buf)[32]) {
+        if ((l.blk_mask >> c) & 1u) es.wait_layer();
+        tmem_ld32(taddr0 + (uint32_t)(64 * c), buf);
+    };
+    fetch(0, va);
+    for (int j = 0; j < chunks; j += 2) {
+        tmem_ld_wait();
+        if (j + 1 < chunks) fetch(j + 1, vb);
+        do_chunk(va, j);
+        if (j + 1 < chunks) {
+            tmem_ld_wait();
+            if (j + 2 < chunks) fetch(j + 2, va);
+            do_chunk(vb, j + 1);
+        }
+    }
+}
+
 // Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
 // in hidden layers, one 32-column half of every 64-column chunk.  Events are published on the
 // LEADER's mbarriers (remote arrive from the peer CTA).
@@ -128,25 +214,16 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         uint32_t persist[64];  // half 0: packed bf16 state (32 words); half 1: fp32 witness (64 words)
         uint32_t nz[16];
         float G = 0.0f, disc = 1.0f, w_row = 0.0f;
-        int ev = 0, t = 0, unit_i = 0, q = 0, blk = 0, p_idx = 0;
+        int t = 0, unit_i = 0, q = 0, blk = 0, p_idx = 0;
         bool valid = false;
-        long long tr_layer = 0, tr_free = 0, tr_bar = 0;
         const long long tr_start = clock64();
-        uint32_t ld_seq = 0, free_seq = 0;
-        uint64_t *cfree = layer_done + kT2AccRing;
-
-        auto arrive_event = [&]() {
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(evt_cl + 8u * (uint32_t)(ev & (kT2EvtRing - 1)));
-            ++ev;
-        };
-        auto wait_layer = [&]() {
-            T2_TRACE_T0();
-            mbar_wait(&layer_done[ld_seq & (kT2AccRing - 1)], (ld_seq >> 3) & 1u);
-            T2_TRACE_ADD(tr_layer);
-            ++ld_seq;
-            tc_fence_after();
-        };
+        EpiSync es;
+        es.evt_cl = evt_cl;
+        es.layer_done = layer_done;
+        es.cfree = layer_done + kT2AccRing;
+        es.lane = lane;
+        auto arrive_event = [&]() { es.arrive_event(); };
+        auto wait_layer = [&]() { es.wait_layer(); };
         auto load_unit = [&]() {
             const int unit = cluster_id + unit_i * n_clusters;
             q = unit / p.blocks_per_q;
@@ -242,50 +319,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 const T2Layer l = L[li];
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
-                    // software-pipelined over the 64-column chunks: the TMEM load of chunk j+1 is in
-                    // flight while chunk j goes through bias / activation / pack / store / event
-                    uint32_t va[32], vb[32];
-                    const int chunks = l.n_pad >> 6;
-                    const uint32_t taddr0 = lane_taddr + (uint32_t)(32 * half);
-                    int free_have = 0;
-                    auto do_chunk = [&](const uint32_t (&v)[32], int j) {
-                        if (j < (int)l.wait_chunks) {  // in-place store: the last block must have read chunk j
-                            const int need_free = j / (int)l.free_nk + 1;
-                            while (free_have < need_free) {
-                                T2_TRACE_T0();
-                                mbar_wait(&cfree[free_seq & (kT2FreeRing - 1)], (free_seq >> 3) & 1u);
-                                T2_TRACE_ADD(tr_free);
-                                ++free_seq;
-                                ++free_have;
-                            }
-                            tc_fence_after();
-                        }
-                        const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
-                        const float *bj = bias + 64 * j + 32 * half;
-                        if (l.act == VOILA_ACT_SILU) hidden_store<VOILA_ACT_SILU>(v, bj, row_addr, row, half);
-                        else if (l.act == VOILA_ACT_RELU) hidden_store<VOILA_ACT_RELU>(v, bj, row_addr, row, half);
-                        else hidden_store<VOILA_ACT_NONE>(v, bj, row_addr, row, half);
-                        fence_proxy_async_smem();
-                        tc_fence_before();
-                        arrive_event();
-                    };
-                    // accumulator blocks are handed over one by one: chunk c may be loaded once the
-                    // block it belongs to has been committed (l.blk_mask: chunks that start a block)
-                    auto fetch = [&](int c, uint32_t (&buf)[32]) {
-                        if ((l.blk_mask >> c) & 1u) wait_layer();
-                        tmem_ld32(taddr0 + (uint32_t)(64 * c), buf);
-                    };
-                    fetch(0, va);
-                    for (int j = 0; j < chunks; j += 2) {
-                        tmem_ld_wait();
-                        if (j + 1 < chunks) fetch(j + 1, vb);
-                        do_chunk(va, j);
-                        if (j + 1 < chunks) {
-                            tmem_ld_wait();
-                            if (j + 2 < chunks) fetch(j + 2, va);
-                            do_chunk(vb, j + 1);
-                        }
-                    }
+                    epi_hidden_layer(es, l, bias, a_u32, lane_taddr, row, half);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
                     if (half == 0) {
@@ -423,7 +457,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     {
                         T2_TRACE_T0();
                         named_bar_sync(1, 256);
-                        T2_TRACE_ADD(tr_bar);
+                        T2_TRACE_ADD(es.tr_bar);
                     }
                     fence_proxy_async_smem();
                     tc_fence_before();
@@ -434,18 +468,197 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
 #ifdef VOILA_T2_TRACE
         if (cluster_id == 0 && lane == 0) {
             unsigned long long *o = g_t2_trace + 16 + ((int)rank * 8 + ew) * 3;
-            o[0] = tr_layer;
-            o[1] = tr_free;
-            o[2] = tr_bar;
+            o[0] = es.tr_layer;
+            o[1] = es.tr_free;
+            o[2] = es.tr_bar;
             if (ew == 0 && rank == 0) g_t2_trace[15] = clock64() - tr_start;
         }
 #endif
-        (void)tr_layer; (void)tr_free; (void)tr_bar; (void)tr_start;
+        (void)tr_start;
     }
 }
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
-    rollout_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+// Epilogue role of the belief-update program: per 256-particle unit
+//   input [s_i ; w_i] -> f_T hidden layers -> PROPOSAL: s'_i = D + b -> bf16 -> proposals (HBM),
+//   operand = [s'_i] -> g hidden layers -> SCORE: l_i = <e, D + b>, L_i = log w_i + l_i / lambda
+//   -> logits, ordered-int running maximum, prior-weight partial sums.
+// P = N and H = 1 in T2Params; the action is the same for every particle, so the action-dependent
+// bias rows are parked once in slot 0 of the shared-memory bias table.
+__device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
+                                               uint64_t *evt, uint64_t *layer_done, float *sbias, int warp, int lane,
+                                               uint32_t rank, int cluster_id, int n_clusters, int n_my_units) {
+    const int n_layers = p.hdr.n_layers;
+    const int ew = warp - 4, qd = warp & 3, half = ew >> 2;
+    const int row = qd * 32 + lane;
+    const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
+    const int S = p.S, Nz = p.Nz;
+    const int in_units = p.hdr.in_chunks * 8;   // f_T input operand, 8-column units
+    const int g_units = p.hdr.g_in_chunks * 8;  // g input operand
+    const float *e_s = sbias + p.hdr.e_off;
+    uint32_t persist[32];  // packed bf16 state of this thread's particle (half 0)
+    uint32_t nz[16];
+    int unit_i = 0, i_idx = 0;
+    bool valid = false;
+    EpiSync es;
+    es.evt_cl = mapa_u32(smem_u32(evt), 0u);
+    es.layer_done = layer_done;
+    es.cfree = layer_done + kT2AccRing;
+    es.lane = lane;
+
+    // one-time: action rows of the bias table (slot 0), e = f(o)
+    {
+        const int tid_e = (int)threadIdx.x - 128;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int li = p.hdr.pa_layer[i];
+            if (li >= 0)
+                for (int c = tid_e; c < (int)L[li].n_pad; c += 256)
+                    sbias[L[li].sbias_off + c] = __ldg(p.bias + L[li].bias_off + (size_t)p.bu_action * L[li].n_pad + c);
+        }
+        for (int c = tid_e; c < p.hdr.e_pad; c += 256) sbias[p.hdr.e_off + c] = c < p.d ? __ldg(p.bu_e + c) : 0.0f;
+    }
+
+    auto load_unit = [&]() {
+        const int unit = cluster_id + unit_i * n_clusters;
+        i_idx = (unit * 2 + (int)rank) * kT2Rows + row;
+        valid = i_idx < p.P;
+        if (half == 0) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (8 * u < S && valid) v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)i_idx * S) + u);
+                persist[4 * u] = v.x; persist[4 * u + 1] = v.y;
+                persist[4 * u + 2] = v.z; persist[4 * u + 3] = v.w;
+            }
+            gen_noise_call(nz, p.seed, (uint32_t)i_idx, 0u, 0u, kStreamBeliefT, Nz);
+        }
+    };
+    auto write_ft_input = [&]() {  // [s ; w ; 0]
+        if (half == 0) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (8 * u < S)
+                    st_shared_v4(a_unit_addr(a_u32, row, u), persist[4 * u], persist[4 * u + 1], persist[4 * u + 2],
+                                 persist[4 * u + 3]);
+            const int u0 = S >> 3;
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (8 * u < Nz)
+                    st_shared_v4(a_unit_addr(a_u32, row, u0 + u), nz[4 * u], nz[4 * u + 1], nz[4 * u + 2], nz[4 * u + 3]);
+            for (int u = u0 + (Nz >> 3); u < in_units; ++u) st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
+        }
+    };
+
+    if (n_my_units > 0) {
+        load_unit();
+        write_ft_input();
+        named_bar_sync(1, 256);  // also orders the bias-table writes above before their first use
+        fence_proxy_async_smem();
+        es.arrive_event();
+    }
+    for (int step = 0; step < n_my_units; ++step) {
+        for (int li = 0; li < n_layers; ++li) {
+            const T2Layer l = L[li];
+            const float *bias = sbias + l.sbias_off;
+            if (l.epi == T2_EPI_HIDDEN) {
+                epi_hidden_layer(es, l, bias, a_u32, lane_taddr, row, half);
+            } else if (l.epi == T2_EPI_PROPOSAL) {
+                es.wait_layer();
+                if (half == 0) {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        if (16 * g < (int)l.n_pad) {
+                            uint32_t v[16];
+                            tmem_ld16(lane_taddr + 16 * g, v);
+                            float4 b[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                persist[8 * g + 2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
+                                                                    __uint_as_float(v[4 * i + 1]) + b[i].y);
+                                persist[8 * g + 2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
+                                                                        __uint_as_float(v[4 * i + 3]) + b[i].w);
+                            }
+                        }
+                    }
+                    // the stored particle is what the filter carries forward: bf16(s')
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (8 * u < S) {
+                            st_shared_v4(a_unit_addr(a_u32, row, u), persist[4 * u], persist[4 * u + 1],
+                                         persist[4 * u + 2], persist[4 * u + 3]);
+                            if (valid)
+                                *(reinterpret_cast<uint4 *>(p.bu_proposals + (size_t)i_idx * S) + u) =
+                                    make_uint4(persist[4 * u], persist[4 * u + 1], persist[4 * u + 2], persist[4 * u + 3]);
+                        }
+                } else {
+                    for (int u = S >> 3; u < g_units; ++u) st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
+                }
+                fence_proxy_async_smem();
+                tc_fence_before();
+                es.arrive_event();
+            } else {  // T2_EPI_SCORE: last layer of the unit
+                float w = 1.0f, lw = 0.0f;
+                if (half == 0 && p.weights) {
+                    w = valid ? __ldg(p.weights + i_idx) : 0.0f;
+                    lw = w > 0.0f ? logf(w) : -INFINITY;
+                }
+                es.wait_layer();
+                if (half == 0) {
+                    float ell = 0.0f;
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        if (16 * g < (int)l.n_pad) {
+                            uint32_t v[16];
+                            tmem_ld16(lane_taddr + 16 * g, v);
+                            float4 b[4], e4[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                e4[i] = *(reinterpret_cast<const float4 *>(e_s + 16 * g) + i);
+                            }
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                ell = fmaf(e4[i].x, __uint_as_float(v[4 * i]) + b[i].x, ell);
+                                ell = fmaf(e4[i].y, __uint_as_float(v[4 * i + 1]) + b[i].y, ell);
+                                ell = fmaf(e4[i].z, __uint_as_float(v[4 * i + 2]) + b[i].z, ell);
+                                ell = fmaf(e4[i].w, __uint_as_float(v[4 * i + 3]) + b[i].w, ell);
+                            }
+                        }
+                    }
+                    const float Lg = lw + ell * p.inv_lambda;
+                    int ord = float_to_ordered(valid ? Lg : -INFINITY);
+                    if (valid) p.bu_logits[i_idx] = Lg;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) ord = max(ord, __shfl_xor_sync(0xffffffffu, ord, o));
+                    double ws = valid ? (double)w : 0.0;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
+                    const int i0 = i_idx - lane;  // first particle of this warp's 32 rows
+                    if (lane == 0 && i0 < p.P) {
+                        atomicMax(p.bu_max_ordered, ord);
+                        p.bu_part_wsum[i0 >> 5] = ws;
+                    }
+                }
+                ++unit_i;
+                if (unit_i < n_my_units) {
+                    load_unit();
+                    write_ft_input();
+                }
+                named_bar_sync(1, 256);
+                fence_proxy_async_smem();
+                tc_fence_before();
+                es.arrive_event();
+            }
+        }
+    }
+}
+
+template <bool BELIEF>
+__device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &wmap) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw_u32 = smem_u32(smem_raw);
     uint8_t *smem = smem_raw + (((raw_u32 + 1023u) & ~1023u) - raw_u32);
@@ -604,14 +817,27 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     }
     } else {
         setmaxnreg_inc<224>();
-        t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
-                    n_clusters, n_my_units, total_steps);
+        if (BELIEF)
+            t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
+                           n_my_units);
+        else
+            t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
+                        n_clusters, n_my_units, total_steps);
     }
 
     tc_fence_before();
     __syncthreads();
     cluster_sync_all();
     if (warp == 2) tmem_dealloc_2cta(tmem_base, (uint32_t)p.hdr.tmem_cols);
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
+    rollout_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    tc2_body<false>(p, wmap);
+}
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
+    belief_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    tc2_body<true>(p, wmap);
 }
 
 }  // namespace
@@ -801,12 +1027,20 @@ struct Builder2 {
     }
 };
 
-struct T2Handle {
+
+// One static program resident on the device: tables, packed weight stream, its tensor map.
+struct T2Program {
     T2Header hdr{};
     void *d_wstream = nullptr, *d_bias = nullptr, *d_sbias = nullptr, *d_layers = nullptr, *d_tiles = nullptr;
     size_t smem_bytes = 0;
     int max_clusters = 0;
     CUtensorMap wmap;
+};
+
+struct T2Handle {
+    T2Program roll;    // rollout: [reward] + f_T + f_Z per step
+    T2Program belief;  // belief update: f_T + g per 256-particle unit
+    bool has_belief = false;
 };
 
 // Layer 1 of a generator sees the "algorithmic" input [s ; w] (K = S + Nz): the one-hot block is
@@ -836,112 +1070,161 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
                                   CUtensorMapFloatOOBfill);
 
-}  // namespace
-
-bool tc2_supported(const voila_model_desc *d, std::string *why) { return tc_supported(d, why); }
-
-void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *allocs, std::string *err) {
-    const int S = d->state_dim, A = d->n_actions, Nz = d->noise_dim;
-    auto fail = [&](const std::string &m) -> void * {
-        if (err) *err = m;
-        return nullptr;
-    };
-    Builder2 pb;
-    if (const char *e = getenv("VOILA_T2_BLOCK_POLICY")) pb.policy = atoi(e);  // tuning knob (0, 1, 2)
-    if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
-        pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
-    add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
-    add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
+// Sizes the program, uploads its tables and weight stream, encodes the tensor map, queries how
+// many CTA pairs of `kernel` can be resident.  Returns an empty string on success.
+template <typename Kernel>
+std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chunks, int sm_count,
+                           std::vector<void *> *allocs) {
     if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa || pb.bad_order)
-        return fail("model too deep for the tcgen05 program tables");
+        return "model too deep for the tcgen05 program tables";
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
     pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
-
-    T2Handle *h = new T2Handle();
-    h->hdr.n_layers = (int)pb.layers.size();
-    h->hdr.blocks_per_step = pb.n_blocks;
-    h->hdr.n_tiles = (int)pb.tiles.size();
-    h->hdr.evt_per_step = pb.evt;
-    h->hdr.a_chunks = pb.a_chunks;
-    h->hdr.in_chunks = rup(S + Nz, 64) / 64;
-    h->hdr.sbias_floats = (int)pb.sbias_init.size();
-    h->hdr.pa_layer[0] = pb.pa_layer[0];
-    h->hdr.pa_layer[1] = pb.pa_layer[1];
+    g.hdr.n_layers = (int)pb.layers.size();
+    g.hdr.blocks_per_step = pb.n_blocks;
+    g.hdr.n_tiles = (int)pb.tiles.size();
+    g.hdr.evt_per_step = pb.evt;
+    g.hdr.a_chunks = pb.a_chunks;
+    g.hdr.in_chunks = in_chunks;
+    g.hdr.sbias_floats = (int)pb.sbias_init.size();
+    g.hdr.pa_layer[0] = pb.pa_layer[0];
+    g.hdr.pa_layer[1] = pb.pa_layer[1];
     int max_n = 32;
     for (const T2Layer &l : pb.layers) max_n = std::max(max_n, (int)l.n_pad);
     int cols = 32;
     while (cols < max_n) cols *= 2;
-    h->hdr.tmem_cols = cols;
-    h->hdr.n_stages = 8;
-    if (const char *e = getenv("VOILA_T2_STAGES")) h->hdr.n_stages = std::max(2, std::min(8, atoi(e)));
-    while (h->hdr.n_stages > 2 && smem2_map(h->hdr).total + 1024 > kMaxDynSmem2) --h->hdr.n_stages;
-    h->smem_bytes = smem2_map(h->hdr).total + 1024;
-    if (h->smem_bytes > kMaxDynSmem2) {
-        delete h;
-        return fail("model does not fit the shared-memory budget of the tcgen05 pair kernel");
-    }
+    g.hdr.tmem_cols = cols;
+    g.hdr.n_stages = 8;
+    if (const char *e = getenv("VOILA_T2_STAGES")) g.hdr.n_stages = std::max(2, std::min(8, atoi(e)));
+    while (g.hdr.n_stages > 2 && smem2_map(g.hdr).total + 1024 > kMaxDynSmem2) --g.hdr.n_stages;
+    g.smem_bytes = smem2_map(g.hdr).total + 1024;
+    if (g.smem_bytes > kMaxDynSmem2) return "model does not fit the shared-memory budget of the tcgen05 pair kernel";
     auto upload = [&](const void *src, size_t bytes, void **dst) -> bool {
         if (cudaMalloc(dst, bytes) != cudaSuccess) return false;
         allocs->push_back(*dst);
         return cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
     };
-    if (!upload(pb.wstream.data(), pb.wstream.size(), &h->d_wstream) ||
-        !upload(pb.bias.data(), pb.bias.size() * sizeof(float), &h->d_bias) ||
-        !upload(pb.sbias_init.data(), pb.sbias_init.size() * sizeof(float), &h->d_sbias) ||
-        !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &h->d_layers) ||
-        !upload(pb.tiles.data(), pb.tiles.size() * sizeof(T2Tile), &h->d_tiles) ||
-        cudaFuncSetAttribute(rollout_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)h->smem_bytes) != cudaSuccess) {
-        const std::string m = cudaGetErrorString(cudaGetLastError());
-        delete h;
-        return fail(m);
-    }
+    if (!upload(pb.wstream.data(), pb.wstream.size(), &g.d_wstream) ||
+        !upload(pb.bias.data(), pb.bias.size() * sizeof(float), &g.d_bias) ||
+        !upload(pb.sbias_init.data(), pb.sbias_init.size() * sizeof(float), &g.d_sbias) ||
+        !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &g.d_layers) ||
+        !upload(pb.tiles.data(), pb.tiles.size() * sizeof(T2Tile), &g.d_tiles) ||
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem_bytes) != cudaSuccess)
+        return cudaGetErrorString(cudaGetLastError());
     // weight stream as a 2-D tensor [rows][64 bf16]; box = one ring stage (128 rows x 128 bytes).
     // The tiles are pre-swizzled on the host, so the copy itself does not swizzle.
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
-        fn == nullptr || qres != cudaDriverEntryPointSuccess) {
-        delete h;
-        return fail("cuTensorMapEncodeTiled not available from the driver");
-    }
+        fn == nullptr || qres != cudaDriverEntryPointSuccess)
+        return "cuTensorMapEncodeTiled not available from the driver";
     const cuuint64_t gdim[2] = {64, (cuuint64_t)(pb.wstream.size() / 128)};
     const cuuint64_t gstride[1] = {128};
     const cuuint32_t box[2] = {64, 128};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult cr = reinterpret_cast<EncodeTiledFn>(fn)(
-        &h->wmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, h->d_wstream, gdim, gstride, box, estr,
+        &g.wmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, g.d_wstream, gdim, gstride, box, estr,
         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (cr != CUDA_SUCCESS) {
-        delete h;
-        return fail("cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)cr));
-    }
+    if (cr != CUDA_SUCCESS) return "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)cr);
     // how many CTA pairs can be resident at once (one CTA per SM; normally sm_count / 2)
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(sm_count & ~1));
     cfg.blockDim = dim3(kT2Threads);
-    cfg.dynamicSmemBytes = h->smem_bytes;
+    cfg.dynamicSmemBytes = g.smem_bytes;
     int nc = 0;
-    if (cudaOccupancyMaxActiveClusters(&nc, rollout_tc2_kernel, &cfg) != cudaSuccess || nc < 1) {
+    if (cudaOccupancyMaxActiveClusters(&nc, kernel, &cfg) != cudaSuccess || nc < 1) {
         cudaGetLastError();
         nc = sm_count / 2;
     }
-    h->max_clusters = std::min(nc, sm_count / 2);
+    g.max_clusters = std::min(nc, sm_count / 2);
+    return std::string();
+}
+
+}  // namespace
+
+bool tc2_supported(const voila_model_desc *d, std::string *why) { return tc_supported(d, why); }
+
+namespace {
+// The state tower g fits the belief program when its hidden widths are MMA-block shaped and the
+// embedding fits eight 16-column accumulator groups.
+bool tower_fits_tc2(const voila_model_desc *d) {
+    const voila_mlp &g = d->lik_state;
+    if (g.n_layers < 2 || g.n_layers > 6) return false;
+    if (g.dims[0] != d->state_dim + (d->lik_action_cond ? d->n_actions : 0)) return false;
+    for (int l = 1; l < g.n_layers; ++l)
+        if (g.dims[l] % 64 != 0 || g.dims[l] > 512) return false;
+    return g.dims[g.n_layers] >= 1 && g.dims[g.n_layers] <= 128;
+}
+}  // namespace
+
+void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *allocs, std::string *err) {
+    const int S = d->state_dim, A = d->n_actions, Nz = d->noise_dim;
+    int policy = 0;
+    if (const char *e = getenv("VOILA_T2_BLOCK_POLICY")) policy = atoi(e);  // tuning knob (0, 1, 2)
+    T2Handle *h = new T2Handle();
+    {
+        Builder2 pb;
+        pb.policy = policy;
+        if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
+            pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
+        add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
+        add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
+        const std::string m = finish_program(pb, h->roll, rollout_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+        if (!m.empty()) {
+            if (err) *err = m;
+            delete h;
+            return nullptr;
+        }
+    }
+    if (tower_fits_tc2(d)) {
+        // belief-update program: proposal s' = f_T(s, a, w), then the state tower g(s') and the score
+        Builder2 pb;
+        pb.policy = policy;
+        add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
+        const voila_mlp &g = d->lik_state;
+        if (d->lik_action_cond) {
+            add_generator2(pb, g, S, A, 0, T2_EPI_SCORE);
+        } else {
+            for (int l = 0; l < g.n_layers; ++l)
+                pb.add_layer(g.W[l], g.dims[l + 1], g.dims[l], g.b[l], 1,
+                             l == g.n_layers - 1 ? T2_EPI_SCORE : T2_EPI_HIDDEN, g.act);
+        }
+        const int dd = g.dims[g.n_layers];
+        h->belief.hdr.g_in_chunks = rup(S, 64) / 64;
+        h->belief.hdr.e_pad = rup(dd, 16);
+        h->belief.hdr.e_off = (int)pb.sbias_init.size();
+        pb.sbias_init.resize(pb.sbias_init.size() + (size_t)h->belief.hdr.e_pad, 0.0f);
+        const std::string m = finish_program(pb, h->belief, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+        h->has_belief = m.empty();  // otherwise the CUDA-core propose+score kernel serves the belief update
+    }
     return h;
 }
 
 void tc2_destroy(void *tc) { delete reinterpret_cast<T2Handle *>(tc); }
 
+bool tc2_has_belief(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_belief; }
+
+namespace {
+T2Params base_params(const T2Program &g, const ModelDev &m) {
+    T2Params p{};
+    p.bias = reinterpret_cast<const float *>(g.d_bias);
+    p.sbias_init = reinterpret_cast<const float *>(g.d_sbias);
+    p.layers = reinterpret_cast<const T2Layer *>(g.d_layers);
+    p.tiles = reinterpret_cast<const T2Tile *>(g.d_tiles);
+    p.hdr = g.hdr;
+    p.S = m.S; p.O = m.O; p.A = m.A; p.Nz = m.Nz;
+    p.gamma = m.gamma;
+    p.reward_kind = m.reward.kind;
+    p.reward_param = m.reward.param;
+    p.action_cost = m.reward.action_cost;
+    return p;
+}
+}  // namespace
+
 cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
                                std::string *kernel_name, int *n_launches) {
-    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
-    T2Params p{};
-    p.bias = reinterpret_cast<const float *>(h->d_bias);
-    p.sbias_init = reinterpret_cast<const float *>(h->d_sbias);
-    p.layers = reinterpret_cast<const T2Layer *>(h->d_layers);
-    p.tiles = reinterpret_cast<const T2Tile *>(h->d_tiles);
-    p.hdr = h->hdr;
+    const T2Program &g = reinterpret_cast<const T2Handle *>(tc)->roll;
+    T2Params p = base_params(g, m);
     p.particles = reinterpret_cast<const uint16_t *>(a.particles);
     p.seqs = a.action_seqs;
     p.weights = a.weights;
@@ -954,14 +1237,34 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     p.blocks_per_q = (a.P + 2 * kT2Rows - 1) / (2 * kT2Rows);
     p.tiles_per_q = a.tiles;  // = 2 * blocks_per_q (see rollout_tile_count)
     p.n_units = p.blocks_per_q * a.Q;
-    p.S = m.S; p.O = m.O; p.A = m.A; p.Nz = m.Nz;
-    p.gamma = m.gamma;
-    p.reward_kind = m.reward.kind;
-    p.reward_param = m.reward.param;
-    p.action_cost = m.reward.action_cost;
-    const int clusters = std::min(h->max_clusters, p.n_units);
-    rollout_tc2_kernel<<<2 * clusters, kT2Threads, h->smem_bytes, st>>>(p, h->wmap);
+    const int clusters = std::min(g.max_clusters, p.n_units);
+    rollout_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (kernel_name) *kernel_name = "rollout_tc2_kernel<tcgen05 cta_group::2 bf16>";
+    if (n_launches) *n_launches = 1;
+    return cudaGetLastError();
+}
+
+// Belief update, propose + score on the CTA-pair tcgen05 program.
+// part_wsum gets one entry per 32 particles.
+cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const BeliefArgs &a, cudaStream_t st,
+                                        int *n_launches) {
+    const T2Program &g = reinterpret_cast<const T2Handle *>(tc)->belief;
+    T2Params p = base_params(g, m);
+    p.particles = reinterpret_cast<const uint16_t *>(a.particles);
+    p.weights = a.weights;
+    p.P = a.N; p.Q = 1; p.H = 1;
+    p.seed = a.seed;
+    p.n_units = (a.N + 2 * kT2Rows - 1) / (2 * kT2Rows);
+    p.bu_action = a.action;
+    p.bu_e = a.e;
+    p.bu_proposals = reinterpret_cast<uint16_t *>(a.proposals);
+    p.bu_logits = a.logits;
+    p.bu_max_ordered = a.max_ordered;
+    p.bu_part_wsum = a.part_wsum;
+    p.inv_lambda = 1.0f / m.lambda;
+    p.d = m.mlp[3].dims[m.mlp[3].n_layers];
+    const int clusters = std::min(g.max_clusters, p.n_units);
+    belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (n_launches) *n_launches = 1;
     return cudaGetLastError();
 }

@@ -72,7 +72,8 @@ struct T2Header {
     int tmem_cols, n_stages, in_chunks, blocks_per_step;  // accumulator blocks (hand-offs) per step
     int sbias_floats;     // size of the shared-memory bias table
     int pa_layer[2];      // layers whose bias row depends on the action (-1: none)
-    int reserved;
+    int g_in_chunks;      // belief program: operand chunks of the state tower's input
+    int e_off, e_pad;     // belief program: f(o) in the shared-memory table (float offset, padded length)
 };
 
 }  // namespace voila

@@ -206,6 +206,9 @@ uint64_t voila_launch_count(const voila_ctx *ctx) { return ctx ? ctx->launches :
 const char *voila_last_rollout_kernel(const voila_ctx *ctx) {
     return ctx ? ctx->last_rollout_kernel.c_str() : "";
 }
+const char *voila_last_belief_kernel(const voila_ctx *ctx) {
+    return ctx ? ctx->last_belief_kernel.c_str() : "";
+}
 
 voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **out) {
     if (!desc || !out) return VOILA_ERR_INVALID_ARG;
@@ -488,7 +491,15 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
     a.max_ordered = sb.max_ordered;
     a.part_wsum = sb.part_wsum;
     int n_parts = (N + kTileRows - 1) / kTileRows;
-    if (use_tc(ctx) && tc_has_belief(ctx->tc)) {
+    if (use_tc2(ctx) && tc2_has_belief(ctx->tc2)) {
+        int n = 0;
+        ProfScope prof(ctx, VOILA_K_PROPOSE, st);
+        e = launch_bu_propose_score_tc2(ctx->tc2, ctx->model, a, st, &n);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += n;
+        n_parts = (N + 31) / 32;
+        ctx->last_belief_kernel = "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
+    } else if (use_tc(ctx) && tc_has_belief(ctx->tc)) {
         int n = 0;
         ProfScope prof(ctx, VOILA_K_PROPOSE, st);
         e = launch_bu_propose_score_tc(ctx->tc, ctx->model, a, st, &n);
@@ -500,6 +511,7 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
         e = launch_bu_propose_score_ffma(ctx->model, a, bf16, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e);
         ctx->launches += 1;
+        ctx->last_belief_kernel = bf16 ? "bu_propose_score_ffma_kernel<bf16>" : "bu_propose_score_ffma_kernel<fp32>";
     }
     {
         ProfScope prof(ctx, VOILA_K_SCAN, st);

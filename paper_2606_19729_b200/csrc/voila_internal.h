@@ -103,6 +103,7 @@ struct voila_ctx {
     int prof_n[4] = {0, 0, 0, 0};
     uint64_t launches = 0;
     std::string last_rollout_kernel;
+    std::string last_belief_kernel;
     std::string last_cuda_error;
     // host copies needed for validation
     int S = 0, O = 0, A = 0, Nz = 0, d = 0;

@@ -57,7 +57,11 @@ bool tc2_supported(const voila_model_desc *desc, std::string *why);
 void *tc2_create(const voila_model_desc *desc, int sm_count, std::vector<void *> *allocs,
                  std::string *err);
 void tc2_destroy(void *tc2);
+bool tc2_has_belief(const void *tc2);  // the belief-update propose+score program was built too
 cudaError_t launch_rollout_tc2(void *tc2, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
                                std::string *kernel_name, int *n_launches);
+// writes one prior-weight partial sum per 32 particles into a.part_wsum
+cudaError_t launch_bu_propose_score_tc2(void *tc2, const ModelDev &m, const BeliefArgs &a,
+                                        cudaStream_t st, int *n_launches);
 
 }  // namespace voila

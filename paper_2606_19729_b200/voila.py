@@ -24,7 +24,7 @@ EXPORTS = [
     "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update",
     "voila_resample_systematic", "voila_mlp_forward", "voila_best_action",
     "voila_rollout_values_host",
-    "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel",
+    "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read",
 ]
@@ -97,6 +97,8 @@ def load_library():
     lib.voila_launch_count.restype = u64
     lib.voila_last_rollout_kernel.argtypes = [vp]
     lib.voila_last_rollout_kernel.restype = C.c_char_p
+    lib.voila_last_belief_kernel.argtypes = [vp]
+    lib.voila_last_belief_kernel.restype = C.c_char_p
     lib.voila_status_string.argtypes = [i32]
     lib.voila_status_string.restype = C.c_char_p
     lib.voila_last_cuda_error.argtypes = [vp]
@@ -217,6 +219,9 @@ class Voila:
 
     def voila_launch_count(self) -> int:
         return int(self.lib.voila_launch_count(self._h))
+
+    def voila_last_belief_kernel(self) -> str:
+        return self.lib.voila_last_belief_kernel(self._h).decode()
 
     def voila_last_rollout_kernel(self) -> str:
         return self.lib.voila_last_rollout_kernel(self._h).decode()

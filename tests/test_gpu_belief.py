@@ -21,7 +21,7 @@ def torch_cuda():
 def _gpu_bu(torch, model, particles, action, obs, weights, seed, prec, kernel=0):
     import paper_2606_19729_b200 as vl
     ctx = vl.Voila(model, device=0, prec=prec)
-    if kernel == vl.KERNEL_TCGEN05 and not ctx.voila_tcgen05_supported():
+    if kernel in (vl.KERNEL_TCGEN05, vl.KERNEL_TCGEN05_PAIR) and not ctx.voila_tcgen05_supported():
         ctx.close()
         pytest.skip("tcgen05 path does not support these dims")
     ctx.voila_set_kernel(kernel)
@@ -30,6 +30,8 @@ def _gpu_bu(torch, model, particles, action, obs, weights, seed, prec, kernel=0)
     w = None if weights is None else torch.from_numpy(weights).cuda()
     out = ctx.voila_belief_update(parts, action, o, w, seed)
     torch.cuda.synchronize()
+    if kernel == vl.KERNEL_TCGEN05_PAIR:  # the tensor-core program really ran (no silent CUDA-core fallback)
+        assert ctx.voila_last_belief_kernel().startswith("belief_tc2_kernel")
     res = {k: t2n(v) if v.dtype != torch.int32 else v.cpu().numpy() for k, v in out.items()}
     ctx.close()
     return res
@@ -84,11 +86,12 @@ def test_belief_update_action_conditioned_tower(torch_cuda, oracle):
     _check_bu(oracle, model, inp.bu_particles, 3, inp.observation, None, 5, g, TOL_FP32, False)
 
 
-@pytest.mark.parametrize("kernel_name", ["ffma", "tcgen05"])
-@pytest.mark.parametrize("cfg_idx,N", [(2, 1024), (3, 2048), (4, 5000), (5, 700)])
+@pytest.mark.parametrize("kernel_name", ["ffma", "tcgen05", "pair"])
+@pytest.mark.parametrize("cfg_idx,N", [(2, 1024), (3, 2048), (4, 5000), (5, 700), (3, 1), (4, 255), (4, 257),
+                                       (5, 40_001)])
 def test_belief_update_bf16(torch_cuda, oracle, kernel_name, cfg_idx, N):
     import paper_2606_19729_b200 as vl
-    kernel = vl.KERNEL_FFMA if kernel_name == "ffma" else vl.KERNEL_TCGEN05
+    kernel = {"ffma": vl.KERNEL_FFMA, "tcgen05": vl.KERNEL_TCGEN05, "pair": vl.KERNEL_TCGEN05_PAIR}[kernel_name]
     cfg = synth.CONFIGS[cfg_idx]
     model = synth.make_model(cfg, prec=synth.PREC_BF16)
     inp = synth.make_inputs(cfg, N=N, P=8, Q=1, H=1)
@@ -96,6 +99,25 @@ def test_belief_update_bf16(torch_cuda, oracle, kernel_name, cfg_idx, N):
                 synth.PREC_BF16, kernel)
     _check_bu(oracle, model, inp.bu_particles, 1, inp.observation, inp.bu_weights, 31, g,
               TOL_BF16_STATE, True)
+
+
+def test_belief_update_bf16_pair_variants(torch_cuda, oracle):
+    """CTA-pair tcgen05 propose+score program: action-conditioned tower (one-hot folded into the
+    bias of g's first layer), uniform prior (weights = NULL), another action and seed."""
+    import paper_2606_19729_b200 as vl
+    cfg = synth.CONFIGS[3]
+    for cond, use_w, action, seed in [(1, False, 5, 99), (0, False, 0, 3), (1, True, 15, 1 << 40)]:
+        model = synth.make_model(cfg, prec=synth.PREC_BF16, lik_action_cond=cond)
+        inp = synth.make_inputs(cfg, N=1500, P=8, Q=1, H=1)
+        w = None
+        if use_w:
+            w = np.exp(2.0 * np.random.default_rng(4).standard_normal(1500)).astype(np.float32)
+            w[::7] = 0.0
+        g = _gpu_bu(torch_cuda, model, inp.bu_particles, action, inp.observation, w, seed, synth.PREC_BF16,
+                    vl.KERNEL_TCGEN05_PAIR)
+        _check_bu(oracle, model, inp.bu_particles, action, inp.observation, w, seed, g, TOL_BF16_STATE, True)
+        if use_w:
+            assert not np.any(np.isin(g["ancestors"], np.nonzero(w == 0)[0]))
 
 
 def test_belief_update_degenerate_weights(torch_cuda):
