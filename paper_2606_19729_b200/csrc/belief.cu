@@ -2,13 +2,15 @@
 // (O5-O7; PAPER.md:77 "before resampling", :128 only relative weights matter, :137).
 //
 //   weight_scan    v_i = exp(L_i - m) (max-shifted), q_i = floor(v_i 2^32) as
-//                  uint64, inclusive scan C_i in ONE pass: warp shuffles inside a 2048-element tile,
-//                  decoupled look-back across tiles.  Integer addition is associative, so the CDF is
+//                  uint64, inclusive scan C_i in ONE pass: warp shuffles inside a 4096-element tile,
+//                  block-wide decoupled look-back across tiles (512 predecessors per round).  Integer addition is associative, so the CDF is
 //                  independent of tiling and the resampled indices are bit-exact (reading R6).
 //   bu_finalize    W = C_{N-1}, comb offset U = (x0 W) >> 32 from one Philox word, log evidence,
 //                  degenerate-weight status.
-//   resample_gather  i_k = min{ i : N C_i > k W + U } by binary search with 128-bit compares
-//                  (the 8 N-byte CDF is L2 resident), then coalesced vectorised row gathers.
+//   resample_gather  i_k = min{ i : N C_i > k W + U } with 128-bit compares: ancestors are
+//                  non-decreasing in k, so a CTA brackets its 256 outputs with two searches of the
+//                  L2-resident CDF, stages that CDF segment in shared memory and searches there;
+//                  then coalesced vectorised row gathers.
 // HBM-bound; no tensor-core work here.
 #include "voila_device.cuh"
 #include "voila_kernels.h"
@@ -18,7 +20,7 @@ namespace voila {
 namespace {
 
 typedef unsigned long long u64;
-constexpr int kScanThreads = 256;
+constexpr int kScanThreads = 512;
 constexpr int kItems = kScanTile / kScanThreads;  // 8
 constexpr unsigned kFlagEmpty = 0u, kFlagAggregate = 1u, kFlagInclusive = 2u;
 
@@ -34,8 +36,92 @@ __global__ void bu_init_kernel(ScanBuffers sb, int tiles) {
     }
 }
 
-__device__ __forceinline__ unsigned ld_flag(const unsigned *p) {
-    return *reinterpret_cast<const volatile unsigned *>(p);
+// bu_init + the observation tower e = f(o) for ONE observation:
+// a chain of GEMVs, so one CTA; the K range of every layer is split over kObsThreads / N thread
+// groups (coalesced reads of the k-major weights, independent loads), partial sums meet in shared
+// memory.  bf16 mode rounds the operands like every other kernel of the library.
+constexpr int kObsThreads = 1024;
+constexpr int kObsMaxWidth = 1024;
+template <bool EMU>
+__global__ void __launch_bounds__(kObsThreads) bu_init_obs_kernel(ScanBuffers sb, int tiles, MlpDev f,
+                                                                  const float *__restrict__ obs, float *e_out) {
+    __shared__ float xs[2][kObsMaxWidth];
+    __shared__ float part[kObsThreads];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < tiles; i += kObsThreads) sb.tile_flag[i] = kFlagEmpty;
+    if (tid == 0) {
+        ScanState z;
+        z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.pad = 0;
+        *sb.state = z;
+        *sb.max_ordered = (int)0x80000000;
+    }
+    // pull every layer's weights towards L2 now: the layers below then pay L2, not HBM, latency
+    for (int l = 0; l < f.n_layers; ++l) {
+        const size_t lines = ((size_t)f.dims[l] * f.dims[l + 1] * sizeof(float) + 127) / 128;
+        const char *w = reinterpret_cast<const char *>(f.Wt[l]);
+        for (size_t i = tid; i < lines; i += kObsThreads) asm volatile("prefetch.global.L2 [%0];" ::"l"(w + i * 128));
+    }
+    for (int k = tid; k < f.dims[0]; k += kObsThreads) xs[0][k] = EMU ? bf16_round(obs[k]) : obs[k];
+    __syncthreads();
+    int cur = 0;
+    for (int l = 0; l < f.n_layers; ++l) {
+        const int K = f.dims[l], N = f.dims[l + 1];
+        const bool last = l == f.n_layers - 1;
+        // G groups of N threads; group g sums k = g, g + G, ...
+        int G = kObsThreads / N;
+        if (G < 1) G = 1;
+        if (G > K) G = K;
+        const float *__restrict__ Wt = f.Wt[l];
+        for (int j0 = 0; j0 < N; j0 += kObsThreads) {  // one pass unless N > kObsThreads
+            const int g = tid / N, j = j0 + tid - g * N;
+            float acc = 0.0f;
+            if (g < G && j < N) {
+                // batches of 8 predicated loads in flight (a plain unrolled loop serialises them
+                // behind its exit tests)
+                const int per = (K + G - 1) / G;
+                for (int kk = 0; kk < per; kk += 8) {
+                    float w[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int k = g + (kk + u) * G;
+                        w[u] = k < K ? __ldg(Wt + (size_t)k * N + j) : 0.0f;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int k = g + (kk + u) * G;
+                        acc = fmaf(w[u], k < K ? xs[cur][k] : 0.0f, acc);
+                    }
+                }
+            }
+            part[tid] = acc;
+            __syncthreads();
+            if (tid < N - j0 && tid < kObsThreads) {
+                const int jj = j0 + tid;
+                float t = 0.0f;
+                for (int gg = 0; gg < G; ++gg) t += part[gg * N + tid];
+                t += __ldg(f.b[l] + jj);
+                if (!last) {
+                    t = act_apply(t, f.act);
+                    if (EMU) t = bf16_round(t);
+                    xs[cur ^ 1][jj] = t;
+                } else {
+                    e_out[jj] = t;
+                }
+            }
+            __syncthreads();
+        }
+        cur ^= 1;
+    }
+}
+
+__device__ __forceinline__ unsigned ld_flag(const unsigned *p) {  // acquire: orders the value load after it
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_flag(unsigned *p, unsigned v) {  // release: the value store is visible first
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ u64 ld_u64_volatile(const u64 *p) {
     return *reinterpret_cast<const volatile u64 *>(p);
@@ -52,14 +138,15 @@ template <bool FROM_LOGITS>
 __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers sb,
                                                                    const float *__restrict__ in, int N,
                                                                    float *post_weights_out) {
-    __shared__ unsigned tile_s;
-    __shared__ u64 warp_tot[kScanThreads / 32];
-    __shared__ u64 excl_s;
-    __shared__ double dsum[kScanThreads / 32];
+    constexpr int kWarpsS = kScanThreads / 32;
+    __shared__ u64 warp_tot[kWarpsS];
+    __shared__ u64 look_tot[kWarpsS];
+    __shared__ int look_first[kWarpsS];
+    __shared__ double dsum[kWarpsS];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) tile_s = atomicAdd(&sb.state->tile_counter, 1u);  // ticket: tiles start in order
-    __syncthreads();
-    const int tile = (int)tile_s;
+    // Tile = CTA index: a look-back only waits for lower-numbered CTAs, which the hardware
+    // dispatches first (the same assumption CUB's single-pass scan makes).
+    const int tile = (int)blockIdx.x;
     const int base = tile * kScanTile + tid * kItems;
 
     float m = 0.0f;
@@ -105,63 +192,64 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
     __syncthreads();
     u64 warp_prefix = 0, agg = 0;
 #pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
+    for (int w = 0; w < kWarpsS; ++w) {
         if (w < warp) warp_prefix += warp_tot[w];
         agg += warp_tot[w];
     }
     const u64 thread_excl = warp_prefix + (incl - run);
 
-    if (warp == 0) {
-        u64 excl = 0;
+    // publish this tile's aggregate (tile 0: its inclusive prefix) before looking back
+    if (tid == 0) {
         if (tile == 0) {
-            if (lane == 0) {
-                sb.tile_incl[0] = agg;
-                __threadfence();
-                *reinterpret_cast<volatile unsigned *>(sb.tile_flag) = kFlagInclusive;
-            }
+            sb.tile_incl[0] = agg;
+            st_flag(sb.tile_flag, kFlagInclusive);
         } else {
-            if (lane == 0) {
-                sb.tile_agg[tile] = agg;
-                __threadfence();
-                *reinterpret_cast<volatile unsigned *>(sb.tile_flag + tile) = kFlagAggregate;
-            }
-            // decoupled look-back, 32 predecessors per round
-            int j = tile - 1;
-            while (true) {
-                const int idx = j - lane;
-                unsigned f;
-                do {
-                    f = idx >= 0 ? ld_flag(sb.tile_flag + idx) : kFlagInclusive;
-                } while (__any_sync(0xffffffffu, f == kFlagEmpty));
-                __threadfence();
-                u64 val = 0;
-                if (idx >= 0) val = ld_u64_volatile(f == kFlagInclusive ? sb.tile_incl + idx : sb.tile_agg + idx);
-                const unsigned inc_mask = __ballot_sync(0xffffffffu, f == kFlagInclusive);
-                const int first = inc_mask ? (__ffs(inc_mask) - 1) : 32;
-                u64 contrib = (lane <= first) ? val : 0ull;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
-                excl += contrib;
-                if (inc_mask) break;
-                j -= 32;
-            }
-            if (lane == 0) {
-                sb.tile_incl[tile] = excl + agg;
-                __threadfence();
-                *reinterpret_cast<volatile unsigned *>(sb.tile_flag + tile) = kFlagInclusive;
-            }
+            sb.tile_agg[tile] = agg;
+            st_flag(sb.tile_flag + tile, kFlagAggregate);
         }
-        if (lane == 0) {
-            excl_s = excl;
-            double t = 0.0;
+        double t = 0.0;
 #pragma unroll
-            for (int w = 0; w < kScanThreads / 32; ++w) t += dsum[w];
-            sb.tile_sumv[tile] = t;
-            if (tile == (N + kScanTile - 1) / kScanTile - 1) sb.state->total_q = excl + agg;
-        }
+        for (int w = 0; w < kWarpsS; ++w) t += dsum[w];
+        sb.tile_sumv[tile] = t;
     }
-    __syncthreads();
-    const u64 off = excl_s + thread_excl;
+    // Decoupled look-back, one predecessor per THREAD and round (kScanThreads per round): when all
+    // tiles of a launch are co-resident nobody owns an inclusive prefix early, and a 32-wide
+    // look-back would walk tiles/32 dependent rounds of L2 latency; this walks tiles/512.
+    // Every predecessor holds a smaller ticket, i.e. has started: the spin cannot deadlock.
+    u64 excl = 0;
+    for (int j = tile - 1; j >= 0; j -= kScanThreads) {
+        const int idx = j - tid;
+        unsigned f = kFlagInclusive;
+        u64 val = 0;
+        if (idx >= 0) {
+            while ((f = ld_flag(sb.tile_flag + idx)) == kFlagEmpty) __nanosleep(40);
+            val = ld_u64_volatile(f == kFlagInclusive ? sb.tile_incl + idx : sb.tile_agg + idx);
+        }
+        // nearest predecessor (smallest tid) that already owns an inclusive prefix
+        const unsigned inc_mask = __ballot_sync(0xffffffffu, f == kFlagInclusive);
+        if (lane == 0) look_first[warp] = inc_mask ? warp * 32 + (__ffs(inc_mask) - 1) : kScanThreads;
+        __syncthreads();
+        int first = kScanThreads;
+#pragma unroll
+        for (int w = kWarpsS - 1; w >= 0; --w)
+            if (look_first[w] < kScanThreads) first = look_first[w];
+        u64 contrib = (tid <= first) ? val : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
+        if (lane == 0) look_tot[warp] = contrib;
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < kWarpsS; ++w) excl += look_tot[w];
+        if (first < kScanThreads) break;  // uniform: every thread read the same look_first[]
+    }
+    if (tid == 0) {
+        if (tile > 0) {
+            sb.tile_incl[tile] = excl + agg;
+            st_flag(sb.tile_flag + tile, kFlagInclusive);
+        }
+        if (tile == (N + kScanTile - 1) / kScanTile - 1) sb.state->total_q = excl + agg;
+    }
+    const u64 off = excl + thread_excl;
     if (base + kItems <= N) {
         ulonglong2 *dst = reinterpret_cast<ulonglong2 *>(sb.cdf + base);
 #pragma unroll
@@ -181,31 +269,41 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
     }
 }
 
-__global__ void bu_finalize_kernel(ScanBuffers sb, int N, int tiles, int n_wsum_parts, int has_prior,
-                                   int from_logits, uint64_t seed, float *log_evidence_out,
-                                   int32_t *dev_status_out) {
-    __shared__ double sh[256];
+constexpr int kFinThreads = 1024;
+
+// block sum of doubles, fixed order (bit-reproducible): 8 independent loads per thread and round
+__device__ __forceinline__ double fin_block_sum(const double *__restrict__ v, int n, double *sh) {
     const int tid = threadIdx.x;
     double acc = 0.0;
-    for (int i = tid; i < tiles; i += 256) acc += sb.tile_sumv[i];
+    int i = tid;
+    for (; i + 7 * kFinThreads < n; i += 8 * kFinThreads) {
+        double t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t[u] = v[i + u * kFinThreads];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc += t[u];
+    }
+    for (; i < n; i += kFinThreads) acc += v[i];
     sh[tid] = acc;
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
+    for (int o = kFinThreads / 2; o > 0; o >>= 1) {
         if (tid < o) sh[tid] += sh[tid + o];
         __syncthreads();
     }
-    const double sum_v = sh[0];
+    const double r = sh[0];
     __syncthreads();
-    acc = 0.0;
-    if (has_prior) for (int i = tid; i < n_wsum_parts; i += 256) acc += sb.part_wsum[i];
-    sh[tid] = acc;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if (tid < o) sh[tid] += sh[tid + o];
-        __syncthreads();
-    }
+    return r;
+}
+
+__global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb, int N, int tiles, int n_wsum_parts,
+                                                                  int has_prior, int from_logits, uint64_t seed,
+                                                                  float *log_evidence_out, int32_t *dev_status_out) {
+    __shared__ double sh[kFinThreads];
+    const int tid = threadIdx.x;
+    const double sum_v = fin_block_sum(sb.tile_sumv, tiles, sh);
+    const double sum_wp = has_prior ? fin_block_sum(sb.part_wsum, n_wsum_parts, sh) : 0.0;
     if (tid == 0) {
-        const double sum_w = has_prior ? sh[0] : (double)N;
+        const double sum_w = has_prior ? sum_wp : (double)N;
         const u64 W = sb.state->total_q;
         float m = 0.0f;
         int status = 0;
@@ -242,44 +340,112 @@ template <> struct VecT<8> { typedef uint2 type; };
 template <> struct VecT<4> { typedef uint32_t type; };
 template <> struct VecT<2> { typedef uint16_t type; };
 
+constexpr int kSegMax = 2048;  // CDF samples staged per CTA (16 KB)
+
+// first i in [lo, hi] with N*C_i > rhs (the answer is known to lie in the range): one thread
+__device__ __forceinline__ int comb_search_global(const u64 *__restrict__ cdf, u64 Nn, int lo, int hi, u64 rhs_hi,
+                                                  u64 rhs_lo) {
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (comb_below(Nn, __ldg(cdf + mid), rhs_hi, rhs_lo)) hi = mid;
+        else lo = mid + 1;
+    }
+    return lo;
+}
+
+// The same search by a whole warp, 32 probes per round: log32(N) dependent rounds of L2 latency
+// instead of log2(N) (4 instead of 20 at N = 2^20).  All lanes return the answer.
+__device__ __forceinline__ int comb_search_warp(const u64 *__restrict__ cdf, u64 Nn, int lo, int hi, u64 rhs_hi,
+                                                u64 rhs_lo, int lane) {
+    while (lo < hi) {
+        const long long span = (long long)hi - lo + 1;
+        const long long step = (span + 31) / 32;
+        long long p = (long long)lo + (lane + 1) * step - 1;
+        if (p > hi) p = hi;
+        const bool above = comb_below(Nn, __ldg(cdf + p), rhs_hi, rhs_lo);  // answer <= p
+        const unsigned mask = __ballot_sync(0xffffffffu, above);             // lane 31 probes hi: mask != 0
+        const int f = __ffs(mask) - 1;
+        const long long p_f = __shfl_sync(0xffffffffu, p, f);
+        const long long p_prev = __shfl_sync(0xffffffffu, p, f > 0 ? f - 1 : 0);
+        if (f > 0) lo = (int)p_prev + 1;
+        hi = (int)p_f;
+    }
+    return lo;
+}
+
 template <int VEC>
 __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, int N,
                                                               const uint8_t *__restrict__ proposals,
                                                               int row_bytes, uint8_t *particles_out,
                                                               float *weights_out, int32_t *ancestors_out) {
     __shared__ int anc_s[256];
-    const int tid = threadIdx.x;
+    __shared__ int range_s[2];
+    __shared__ u64 seg[kSegMax];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k0 = blockIdx.x * 256, k = k0 + tid;
+    const int rows = min(256, N - k0);
     const ScanState st = *sb.state;
-    if (k < N) {
+    const u64 W = st.total_q, U = st.offset_u;
+    u64 rhs_lo = (u64)k * W, rhs_hi = __umul64hi((u64)k, W);
+    rhs_lo += U;
+    rhs_hi += (rhs_lo < U) ? 1ull : 0ull;
+    if (st.status == 0) {
+        // Ancestors are non-decreasing in k: bracket the CTA's outputs with the ancestors of its
+        // first and last output (warps 0 and 1, one cooperative search each).
+        if (warp < 2) {
+            const int kk = warp == 0 ? k0 : k0 + rows - 1;
+            u64 r_lo = (u64)kk * W, r_hi = __umul64hi((u64)kk, W);
+            r_lo += U;
+            r_hi += (r_lo < U) ? 1ull : 0ull;
+            // the answer exists: k*W + U < N*W = N*C_{N-1}
+            const int a = comb_search_warp(sb.cdf, (u64)N, 0, N - 1, r_hi, r_lo, lane);
+            if (lane == 0) range_s[warp] = a;
+        }
+        __syncthreads();
+        const int a_lo = range_s[0], a_hi = range_s[1];
+        const int len = a_hi - a_lo + 1;
+        // stage the segment [a_lo, a_hi] in shared memory, every s-th entry when it is longer than
+        // kSegMax (sample g = last entry of group g): search the samples, then inside one group
+        const int s_ = (len + kSegMax - 1) / kSegMax;
+        const int cnt = (len + s_ - 1) / s_;
+        for (int i = tid; i < cnt; i += 256) {
+            const long long pos = (long long)a_lo + (long long)(i + 1) * s_ - 1;
+            seg[i] = __ldg(sb.cdf + (pos < a_hi ? pos : a_hi));
+        }
+        __syncthreads();
         int a = k;
-        if (st.status == 0) {
-            const u64 W = st.total_q, U = st.offset_u;
-            u64 rhs_lo = (u64)k * W, rhs_hi = __umul64hi((u64)k, W);
-            rhs_lo += U;
-            rhs_hi += (rhs_lo < U) ? 1ull : 0ull;
-            int lo = 0, hi = N - 1;  // the answer exists: k*W + U < N*W = N*C_{N-1}
+        if (k < N) {
+            int lo = 0, hi = cnt - 1;
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
-                if (comb_below((u64)N, __ldg(sb.cdf + mid), rhs_hi, rhs_lo)) hi = mid;
+                if (comb_below((u64)N, seg[mid], rhs_hi, rhs_lo)) hi = mid;
                 else lo = mid + 1;
             }
-            a = lo;
+            a = a_lo + lo;
+            if (s_ > 1) {
+                const long long g_lo = (long long)a_lo + (long long)lo * s_;
+                long long g_hi = g_lo + s_ - 1;
+                if (g_hi > a_hi) g_hi = a_hi;
+                a = comb_search_global(sb.cdf, (u64)N, (int)g_lo, (int)g_hi, rhs_hi, rhs_lo);
+            }
         }
         anc_s[tid] = a;
-        if (ancestors_out) ancestors_out[k] = a;
+    } else {
+        anc_s[tid] = k;  // degenerate weights: identity
+    }
+    if (k < N) {
+        if (ancestors_out) ancestors_out[k] = anc_s[tid];
         if (weights_out) weights_out[k] = 1.0f / (float)N;
     }
     __syncthreads();
     if (particles_out) {
         typedef typename VecT<VEC>::type V;
-        const int rows = min(256, N - k0);
         const int cpr = row_bytes / VEC;
         const int total = rows * cpr;
         for (int c = tid; c < total; c += 256) {
             const int j = c / cpr, off = c - j * cpr;
             const V val = *reinterpret_cast<const V *>(proposals + (size_t)anc_s[j] * row_bytes + (size_t)off * VEC);
-            *reinterpret_cast<V *>(particles_out + (size_t)(k0 + j) * row_bytes + (size_t)off * VEC) = val;
+            __stcs(reinterpret_cast<V *>(particles_out + (size_t)(k0 + j) * row_bytes + (size_t)off * VEC), val);
         }
     }
 }
@@ -289,6 +455,20 @@ __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, in
 cudaError_t launch_bu_init(const ScanBuffers &sb, int N, cudaStream_t st) {
     const int tiles = scan_tiles(N);
     bu_init_kernel<<<(tiles + 255) / 256, 256, 0, st>>>(sb, tiles);
+    return cudaGetLastError();
+}
+
+bool obs_tower_fits(const MlpDev &f) {
+    for (int l = 0; l <= f.n_layers; ++l)
+        if (f.dims[l] > kObsMaxWidth) return false;
+    return true;
+}
+
+cudaError_t launch_bu_init_obs(const ScanBuffers &sb, int N, const MlpDev &f, const float *obs, float *e_out,
+                               bool bf16, cudaStream_t st) {
+    const int tiles = scan_tiles(N);
+    if (bf16) bu_init_obs_kernel<true><<<1, kObsThreads, 0, st>>>(sb, tiles, f, obs, e_out);
+    else bu_init_obs_kernel<false><<<1, kObsThreads, 0, st>>>(sb, tiles, f, obs, e_out);
     return cudaGetLastError();
 }
 
@@ -305,7 +485,7 @@ cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, b
                                cudaStream_t st) {
     // n_wsum_parts < 0 marks the stage-level resampler (weights given directly, no logits)
     const int from_logits = n_wsum_parts >= 0;
-    bu_finalize_kernel<<<1, 256, 0, st>>>(sb, N, scan_tiles(N), n_wsum_parts < 0 ? 0 : n_wsum_parts,
+    bu_finalize_kernel<<<1, kFinThreads, 0, st>>>(sb, N, scan_tiles(N), n_wsum_parts < 0 ? 0 : n_wsum_parts,
                                           has_prior ? 1 : 0, from_logits, seed, log_evidence_out,
                                           dev_status_out);
     return cudaGetLastError();

@@ -472,12 +472,19 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
     const bool bf16 = ctx->prec == VOILA_PREC_BF16;
     float *e_dev = reinterpret_cast<float *>(w + L.e);
 
-    cudaError_t e = launch_bu_init(sb, N, st);
-    if (e != cudaSuccess) return cuda_fail(ctx, e);
-    // e = f(o): the observation tower, once (one row through the generic MLP kernel)
-    e = launch_mlp_forward_ffma(ctx->model, 2, observation, 1, e_dev, bf16, st);
-    if (e != cudaSuccess) return cuda_fail(ctx, e);
-    ctx->launches += 2;
+    // scan bookkeeping reset + e = f(o): the observation tower, once
+    cudaError_t e;
+    if (obs_tower_fits(ctx->model.mlp[2])) {
+        e = launch_bu_init_obs(sb, N, ctx->model.mlp[2], observation, e_dev, bf16, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 1;
+    } else {
+        e = launch_bu_init(sb, N, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        e = launch_mlp_forward_ffma(ctx->model, 2, observation, 1, e_dev, bf16, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 2;
+    }
 
     BeliefArgs a{};
     a.particles = particles;

@@ -18,7 +18,7 @@ cudaError_t launch_bu_propose_score_ffma(const ModelDev &m, const BeliefArgs &a,
                                          cudaStream_t st);
 
 // ---- belief.cu : normalise, uint64 decoupled-lookback scan, systematic resample + gather ----
-constexpr int kScanTile = 2048;
+constexpr int kScanTile = 4096;
 struct ScanBuffers {
     ScanState *state;
     unsigned int *tile_flag;           // [tiles]
@@ -31,6 +31,10 @@ struct ScanBuffers {
 };
 inline int scan_tiles(int N) { return (N + kScanTile - 1) / kScanTile; }
 cudaError_t launch_bu_init(const ScanBuffers &sb, int N, cudaStream_t st);
+// bu_init fused with the observation tower e = f(o) (one observation): one launch, one CTA
+bool obs_tower_fits(const MlpDev &f);
+cudaError_t launch_bu_init_obs(const ScanBuffers &sb, int N, const MlpDev &f, const float *obs, float *e_out,
+                               bool bf16, cudaStream_t st);
 // from_logits: v_i = exp(L_i - max) (belief update) ; else v_i = in[i] (stage-level resampler)
 cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bool from_logits,
                                float *post_weights_out, cudaStream_t st);
