@@ -759,7 +759,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             int waited = -1, base = 1, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
-            long long tr_evt = 0, tr_full = 0;
+            long long tr_evt = 0, tr_full = 0, tr_mma = 0, tr_commit = 0;
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 T2Tile t = T[0];
@@ -781,6 +781,9 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                     const uint32_t d = tmem_base + (uint32_t)t.d_col16 * 16u;
                     const uint32_t chunk_b = (uint32_t)t.rows8 * 1024u;  // bytes of one K chunk in the stage
                     uint32_t acc = (t.flags & 1u) ? 0u : 1u;
+#ifdef VOILA_T2_TRACE
+                    const long long tm0 = clock64();
+#endif
                     for (int c = 0; c < (int)t.nk; ++c) {
                         const uint64_t ad = umma_desc_sw128(a_u32 + (uint32_t)(t.kc0 + c) * kT2ChunkBytes);
                         const uint64_t bd = umma_desc_sw128(ring_u32 + stage * kT2StageBytes + c * chunk_b);
@@ -790,12 +793,19 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                             acc = 1u;
                         }
                     }
+#ifdef VOILA_T2_TRACE
+                    const long long tm1 = clock64();
+                    tr_mma += tm1 - tm0;
+#endif
                     umma_commit_2cta(&empty[stage], 3);
                     if (t.flags & 4u) {
                         umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
                         ++free_seq;
                     }
                     if (t.flags & 2u) umma_commit_2cta(&layer_done[(blk_base + (int)t.blk) & (kT2AccRing - 1)], 3);
+#ifdef VOILA_T2_TRACE
+                    tr_commit += clock64() - tm1;
+#endif
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
@@ -810,9 +820,11 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                 g_t2_trace[4] = tr_evt;
                 g_t2_trace[5] = tr_full;
                 g_t2_trace[6] = clock64() - tr_start;
+                g_t2_trace[7] = tr_mma;
+                g_t2_trace[8] = tr_commit;
             }
 #endif
-            (void)tr_evt; (void)tr_full; (void)tr_start;
+            (void)tr_evt; (void)tr_full; (void)tr_start; (void)tr_mma; (void)tr_commit;
         }
     }
     } else {
