@@ -314,6 +314,11 @@ def run_voila(args):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": None,
                 "peak_kind": "fp32 FFMA: SMs x 128 lanes x 2 flop x max SM clock (CUDA-core kernel)"}
+    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (inputs are
+    # read once and stay in L2; the horizon loop never touches HBM): profiles/r01c_rollout_tc2_cfg5.md
+    if cfg.name.startswith("cfg5") and "rollout_tc2" in ctx.voila_last_rollout_kernel():
+        roof["traffic"] = 4374272
+        roof["traffic_from"] = "profiles/r01c_rollout_tc2_cfg5.md (ncu --set full, Q=37 launch of the same shapes)"
     roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
                  "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
                  "share_of_step": k_ms / ms_per_step})
@@ -325,6 +330,12 @@ def run_voila(args):
               "propose_score_us": 1e3 * float(np.mean(kt[1])) if kt[1] else None,
               "scan_us": 1e3 * float(np.mean(kt[2])) if kt[2] else None,
               "resample_gather_us": 1e3 * float(np.mean(kt[3])) if kt[3] else None}
+    if kt[1] and ctx.prec == vl.PREC_BF16 and "tc2" in ctx.voila_last_belief_kernel():
+        tf = N * synth.flops_per_belief_particle(model) / (np.mean(kt[1]) * 1e-3) / 1e12
+        belief["propose_score_roofline"] = {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"],
+                                            "unit": "TFLOP/s", "frac": tf / peaks["bf16_burst"],
+                                            "kernel": ctx.voila_last_belief_kernel(),
+                                            "flop_per_particle": synth.flops_per_belief_particle(model)}
     if kt[3]:
         gbs = bytes_resample / (np.mean(kt[3]) * 1e-3) / 1e9
         belief["resample_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"],

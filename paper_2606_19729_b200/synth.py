@@ -225,3 +225,17 @@ def flops_per_rollout_step(model: ModelSpec, algorithmic: bool = True) -> int:
                 k -= model.A
             tot += 2 * k * f.dims[l + 1]
     return tot
+
+
+def flops_per_belief_particle(model: ModelSpec, algorithmic: bool = True) -> int:
+    """2*MAC of one proposal f_T plus one state-tower g evaluation and the score dot product
+    (SURVEY 8a R7-R8); `algorithmic` folds one-hot action blocks into first-layer biases."""
+    tot = 0
+    towers = [(model.f_T, True), (model.lik_state, bool(model.lik_action_cond))]
+    for f, has_onehot in towers:
+        for l in range(f.n_layers):
+            k = f.dims[l]
+            if l == 0 and algorithmic and has_onehot:
+                k -= model.A
+            tot += 2 * k * f.dims[l + 1]
+    return tot + 2 * model.lik_state.dims[-1]
