@@ -166,9 +166,8 @@ def run_voila(args):
     import paper_2606_19729_b200 as vl
     from paper_2606_19729_b200 import synth
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2606_19729_b200 import replicas
+    rank, local, world = replicas.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -200,7 +199,7 @@ def run_voila(args):
     bu_w = None if inp.bu_weights is None else torch.from_numpy(inp.bu_weights).to(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
     stream = torch.cuda.current_stream(dev)
-    seed0 = 20260619
+    seed0 = replicas.replica_seed(20260619, rank, 0, 0)  # replicas draw different noise
 
     state = {"parts": parts, "bu_parts": bu_parts}
 
@@ -246,15 +245,12 @@ def run_voila(args):
     roll_ms = [a.elapsed_time(b) for a, b, _ in ev]
     bu_ms = [b.elapsed_time(c) for _, b, c in ev]
     total_ms = float(sum(roll_ms) + sum(bu_ms))
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = replicas.max_over_ranks(total_ms, dist, dev)  # the job is as slow as its slowest replica
     kt = [ctx.voila_profile_read(w) for w in range(4)]
     ctx.voila_set_profiling(False)
     assert int(bu["status"].item()) == 0 and bool(torch.isfinite(out["values"]).all())
     ms_per_step = total_ms / args.steps
-    value = world * P * Q * H / (ms_per_step * 1e-3)
+    value = replicas.whole_job_value(P * Q * H, world, ms_per_step)
 
     # ---- end to end through the host-buffer C-ABI entry points (pinned host memory) ----
     esize = 2 if ctx.prec == vl.PREC_BF16 else 4
@@ -284,10 +280,7 @@ def run_voila(args):
         e2e_step(k + 1)
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, dist, dev)
     h2d = P * cfg.S * esize + Q * H * 4 + N * cfg.S * esize + cfg.O * 4 + (N * 4 if h_w is not None else 0)
     d2h = Q * 4 + N * cfg.S * esize + N * 4 + 8
     e2e = {"value": world * P * Q * H * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
