@@ -753,8 +753,9 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             (void)tr_empty; (void)tr_start;
         }
     } else if (warp == 1) {
-        // ===== MMA issuer: leader CTA only =====
-        if (lane == 0 && rank == 0) {
+        // ===== MMA issuer: leader CTA only.  The whole warp walks the tile program (waits are
+        // warp-uniform); one elected lane issues the MMAs and commits. =====
+        if (rank == 0) {
             uint32_t stage = 0, phase = 0;
             int waited = -1, base = 1, blk_base = 0;
             uint32_t free_seq = 0;
@@ -778,6 +779,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                         T2_TRACE_ADD(tr_full);
                     }
                     tc_fence_after();
+                    if (elect_one_sync()) {
                     const uint32_t d = tmem_base + (uint32_t)t.d_col16 * 16u;
                     const uint32_t chunk_b = (uint32_t)t.rows8 * 1024u;  // bytes of one K chunk in the stage
                     uint32_t acc = (t.flags & 1u) ? 0u : 1u;
@@ -798,14 +800,14 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                     tr_mma += tm1 - tm0;
 #endif
                     umma_commit_2cta(&empty[stage], 3);
-                    if (t.flags & 4u) {
-                        umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
-                        ++free_seq;
-                    }
+                    if (t.flags & 4u) umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
                     if (t.flags & 2u) umma_commit_2cta(&layer_done[(blk_base + (int)t.blk) & (kT2AccRing - 1)], 3);
 #ifdef VOILA_T2_TRACE
                     tr_commit += clock64() - tm1;
 #endif
+                    }
+                    __syncwarp();
+                    if (t.flags & 4u) ++free_seq;
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
@@ -816,7 +818,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                 blk_base += p.hdr.blocks_per_step;
             }
 #ifdef VOILA_T2_TRACE
-            if (cluster_id == 0) {
+            if (cluster_id == 0 && elect_one_sync()) {
                 g_t2_trace[4] = tr_evt;
                 g_t2_trace[5] = tr_full;
                 g_t2_trace[6] = clock64() - tr_start;
