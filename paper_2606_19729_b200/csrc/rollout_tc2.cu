@@ -99,23 +99,49 @@ __device__ __forceinline__ float act_biased(uint32_t v, float b) {
     return ACT == VOILA_ACT_RELU ? fmaxf(x, 0.0f) : x;
 }
 
-// 32 accumulator columns of this thread's row (already in registers) -> bias (shared memory,
-// broadcast reads) -> activation -> bf16 -> this warp's half of the 64-column operand chunk.
-template <int ACT>
-__device__ __forceinline__ void hidden_store(const uint32_t (&v)[32], const float *sb, uint32_t row_addr, int row,
-                                             int half) {
-    uint32_t o[16];
+// Per-thread constants of the hidden-layer epilogue, computed once and pinned in registers (the
+// asm barrier keeps the compiler from re-deriving them from %tid / cvta in every chunk, which was
+// ~40 % of the chunk's instructions).
+struct EpiConst {
+    uint32_t st_base;   // shared address of this row in operand chunk 0
+    uint32_t sw[4];     // swizzled byte offsets of this warp's four 16-byte units inside a row
+    uint32_t taddr0;    // TMEM address of this warp's lane quadrant + column half
+    uint32_t sbias_u32; // shared address of the bias table + this warp's column half
+};
+__device__ __forceinline__ uint32_t pin_reg(uint32_t v) {
+    asm volatile("mov.b32 %0, %0;" : "+r"(v));
+    return v;
+}
+__device__ __forceinline__ EpiConst make_epi_const(uint32_t a_u32, uint32_t lane_taddr, const float *sbias, int row,
+                                                   int half) {
+    EpiConst c;
+    c.st_base = pin_reg(a_u32 + (uint32_t)row * 128u);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float4 b = *reinterpret_cast<const float4 *>(sb + 4 * i);
+    for (int u = 0; u < 4; ++u) c.sw[u] = (uint32_t)(((half * 4 + u) ^ (row & 7)) << 4);
+    c.taddr0 = pin_reg(lane_taddr + (uint32_t)(32 * half));
+    c.sbias_u32 = pin_reg(smem_u32(sbias) + (uint32_t)(32 * half) * 4u);
+    return c;
+}
+__device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+// 16 accumulator columns of this thread's row (already in registers) -> bias (shared memory,
+// broadcast reads) -> activation -> bf16 -> two 16-byte units of the 64-column operand chunk.
+template <int ACT>
+__device__ __forceinline__ void hidden_store16(const uint32_t (&v)[16], uint32_t bias_u32, uint32_t row_addr,
+                                               uint32_t sw0, uint32_t sw1) {
+    uint32_t o[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float4 b = ld_shared_f4(bias_u32 + 16u * i);
         o[2 * i] = pack_bf16x2(act_biased<ACT>(v[4 * i], b.x), act_biased<ACT>(v[4 * i + 1], b.y));
         o[2 * i + 1] = pack_bf16x2(act_biased<ACT>(v[4 * i + 2], b.z), act_biased<ACT>(v[4 * i + 3], b.w));
     }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int unit = half * 4 + u;
-        st_shared_v4(row_addr + ((unit ^ (row & 7)) << 4), o[4 * u], o[4 * u + 1], o[4 * u + 2], o[4 * u + 3]);
-    }
+    st_shared_v4(row_addr + sw0, o[0], o[1], o[2], o[3]);
+    st_shared_v4(row_addr + sw1, o[4], o[5], o[6], o[7]);
 }
 
 // Synchronisation state of one epilogue warp: the numbered events it publishes on the leader's
@@ -151,48 +177,55 @@ struct EpiSync {
 
 // Epilogue of a hidden layer for this warp's 32 rows x one 32-column half of every 64-column chunk:
 // software-pipelined over the chunks (the TMEM load of chunk j+1 is in flight while chunk j goes
-// through bias / activation / pack / store / event).
-__device__ __forceinline__ void epi_hidden_layer(EpiSync &es, const T2Layer &l, const float *bias, uint32_t a_u32,
-                                                 uint32_t lane_taddr, int row, int half) {
-    uint32_t va[32], vb[32];
+// through bias / activation / pack / store / event).  One instantiation per activation, so the
+// chunk loop carries no dispatch.
+template <int ACT>
+__device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, uint32_t bias_u32, const EpiConst &ec) {
+    // 16-column pieces, double-buffered: the TMEM load of piece k+1 is in flight while piece k goes
+    // through bias / activation / pack / store (32 live accumulator registers instead of 64)
+    uint32_t va[16], vb[16];
     const int chunks = l.n_pad >> 6;
-    const uint32_t taddr0 = lane_taddr + (uint32_t)(32 * half);
+    const int wait_chunks = l.wait_chunks, free_nk = l.free_nk;
+    const uint32_t blk_mask = l.blk_mask;
     int free_have = 0;
-    auto do_chunk = [&](const uint32_t (&v)[32], int j) {
-        if (j < (int)l.wait_chunks) {  // in-place store: the last block must have read chunk j
-            const int need_free = j / (int)l.free_nk + 1;
+    // accumulator blocks are handed over one by one: a chunk may be loaded once the block it
+    // belongs to has been committed (blk_mask: chunks that start a block)
+    if (blk_mask & 1u) es.wait_layer();
+    tmem_ld16(ec.taddr0, va);
+    for (int j = 0; j < chunks; ++j) {
+        const uint32_t row_addr = ec.st_base + (uint32_t)j * kT2ChunkBytes;
+        const uint32_t bj = bias_u32 + 256u * (uint32_t)j;
+        tmem_ld_wait();
+        tmem_ld16(ec.taddr0 + (uint32_t)(64 * j + 16), vb);
+        if (j < wait_chunks) {  // in-place store: the last block must have read chunk j
+            const int need_free = j / free_nk + 1;
             while (free_have < need_free) {
                 es.wait_chunk_free();
                 ++free_have;
             }
             tc_fence_after();
         }
-        const uint32_t row_addr = a_u32 + j * kT2ChunkBytes + row * 128;
-        const float *bj = bias + 64 * j + 32 * half;
-        if (l.act == VOILA_ACT_SILU) hidden_store<VOILA_ACT_SILU>(v, bj, row_addr, row, half);
-        else if (l.act == VOILA_ACT_RELU) hidden_store<VOILA_ACT_RELU>(v, bj, row_addr, row, half);
-        else hidden_store<VOILA_ACT_NONE>(v, bj, row_addr, row, half);
+        hidden_store16<ACT>(va, bj, row_addr, ec.sw[0], ec.sw[1]);
+        tmem_ld_wait();
+        // the next chunk may belong to a block that is still being accumulated: then publish this
+        // chunk first and wait afterwards (one un-overlapped TMEM load per block, not per chunk)
+        const bool next_blk = (j + 1 < chunks) && ((blk_mask >> (j + 1)) & 1u);
+        if (j + 1 < chunks && !next_blk) tmem_ld16(ec.taddr0 + (uint32_t)(64 * (j + 1)), va);
+        hidden_store16<ACT>(vb, bj + 64u, row_addr, ec.sw[2], ec.sw[3]);
         fence_proxy_async_smem();
         tc_fence_before();
         es.arrive_event();
-    };
-    // accumulator blocks are handed over one by one: chunk c may be loaded once the block it
-    // belongs to has been committed (l.blk_mask: chunks that start a block)
-    auto fetch = [&](int c, uint32_t (&buf)[32]) {
-        if ((l.blk_mask >> c) & 1u) es.wait_layer();
-        tmem_ld32(taddr0 + (uint32_t)(64 * c), buf);
-    };
-    fetch(0, va);
-    for (int j = 0; j < chunks; j += 2) {
-        tmem_ld_wait();
-        if (j + 1 < chunks) fetch(j + 1, vb);
-        do_chunk(va, j);
-        if (j + 1 < chunks) {
-            tmem_ld_wait();
-            if (j + 2 < chunks) fetch(j + 2, va);
-            do_chunk(vb, j + 1);
+        if (next_blk) {
+            es.wait_layer();
+            tmem_ld16(ec.taddr0 + (uint32_t)(64 * (j + 1)), va);
         }
     }
+}
+__device__ __forceinline__ void epi_hidden_layer(EpiSync &es, const T2Layer &l, int bias_float_off, const EpiConst &ec) {
+    const uint32_t bias_u32 = ec.sbias_u32 + 4u * (uint32_t)bias_float_off;
+    if (l.act == VOILA_ACT_SILU) epi_hidden_loop<VOILA_ACT_SILU>(es, l, bias_u32, ec);
+    else if (l.act == VOILA_ACT_RELU) epi_hidden_loop<VOILA_ACT_RELU>(es, l, bias_u32, ec);
+    else epi_hidden_loop<VOILA_ACT_NONE>(es, l, bias_u32, ec);
 }
 
 // Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
@@ -224,6 +257,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         es.lane = lane;
         auto arrive_event = [&]() { es.arrive_event(); };
         auto wait_layer = [&]() { es.wait_layer(); };
+        const EpiConst ec = make_epi_const(a_u32, lane_taddr, sbias, row, half);
         auto load_unit = [&]() {
             const int unit = cluster_id + unit_i * n_clusters;
             q = unit / p.blocks_per_q;
@@ -319,7 +353,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 const T2Layer l = L[li];
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
-                    epi_hidden_layer(es, l, bias, a_u32, lane_taddr, row, half);
+                    epi_hidden_layer(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ec);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
                     if (half == 0) {
@@ -504,6 +538,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
     es.layer_done = layer_done;
     es.cfree = layer_done + kT2AccRing;
     es.lane = lane;
+    const EpiConst ec = make_epi_const(a_u32, lane_taddr, sbias, row, half);
 
     // one-time: action rows of the bias table (slot 0), e = f(o)
     {
@@ -561,7 +596,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             const T2Layer l = L[li];
             const float *bias = sbias + l.sbias_off;
             if (l.epi == T2_EPI_HIDDEN) {
-                epi_hidden_layer(es, l, bias, a_u32, lane_taddr, row, half);
+                epi_hidden_layer(es, l, (int)l.sbias_off, ec);
             } else if (l.epi == T2_EPI_PROPOSAL) {
                 es.wait_layer();
                 if (half == 0) {
