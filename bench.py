@@ -203,9 +203,18 @@ def run_voila(args):
 
     state = {"parts": parts, "bu_parts": bu_parts}
 
+    def pick_action(values):
+        """CFG5 protocol: the executed action is the first action of argmax_q V_q, taken
+        on the device (`voila_best_action`); the 4-byte read-back is the planner's output.  CFG1-4
+        update with the fixed action of the config."""
+        if not chain:
+            return inp.bu_action
+        _, ba = ctx.voila_best_action(values, seqs)
+        return int(ba.item())
+
     def step(k):
         out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * k, want_witness=True)
-        bu = ctx.voila_belief_update(state["bu_parts"], inp.bu_action, obs_all[k], bu_w,
+        bu = ctx.voila_belief_update(state["bu_parts"], pick_action(out["values"]), obs_all[k], bu_w,
                                      seed0 + 2 * k + 1, want_debug=False)
         if chain:
             state["parts"] = state["bu_parts"] = bu["particles"]
@@ -232,7 +241,7 @@ def run_voila(args):
         ev[k][0].record(stream)
         out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * (k + args.warmup))
         ev[k][1].record(stream)
-        bu = ctx.voila_belief_update(state["bu_parts"], inp.bu_action, obs_all[k + args.warmup], bu_w,
+        bu = ctx.voila_belief_update(state["bu_parts"], pick_action(out["values"]), obs_all[k + args.warmup], bu_w,
                                      seed0 + 2 * (k + args.warmup) + 1, want_debug=False)
         ev[k][2].record(stream)
         if chain:
@@ -268,7 +277,8 @@ def run_voila(args):
 
     def e2e_step(k):
         ctx.voila_rollout_values_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals)
-        ctx.voila_belief_update_host(h_bu, inp.bu_action, h_obs[k % h_obs.shape[0], :cfg.O], h_w,
+        a_exec = int(h_seqs[int(np.argmax(h_vals.numpy())), 0]) if chain else inp.bu_action  # ties -> lowest q
+        ctx.voila_belief_update_host(h_bu, a_exec, h_obs[k % h_obs.shape[0], :cfg.O], h_w,
                                      seed0 + 2 * k + 1, h_pout, None, h_anc, h_le, h_st)
 
     e2e_step(0)

@@ -158,8 +158,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
             (void)tr_empty; (void)tr_start;
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
+        // ===== MMA issuer: the warp walks the tile program converged (waits are warp-uniform); one
+        // elected lane issues, so each tcgen05.mma / commit is ONE instruction (no ELECT loop) =====
+        {
             uint32_t stage = 0, phase = 0;
             int waited = -1, base = 1;
             long long tr_evt = 0, tr_full = 0;
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                         TRACE_ADD(tr_full);
                     }
                     tc_fence_after();
+                    if (elect_one_sync()) {
                     const uint64_t ad = umma_desc_sw128(a_u32 + (uint32_t)t.kc * kTcChunkBytes);
                     const uint64_t bd = umma_desc_sw128(ring_u32 + stage * kTcStageBytes);
                     const uint32_t d = tmem_base + (uint32_t)t.n * l.bn;
@@ -189,6 +191,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                         umma_ss(d, ad + 2u * k, bd + 2u * k, l.idesc, (t.first && k == 0) ? 0u : 1u);
                     umma_commit(&empty[stage]);
                     if (t.last) umma_commit(layer_done);
+                    }
+                    __syncwarp();
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
@@ -197,7 +201,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
                 base += p.hdr.evt_per_step;
             }
 #ifdef VOILA_TC_TRACE
-            if (blockIdx.x == 0) {
+            if (blockIdx.x == 0 && lane == 0) {
                 g_tc_trace[2] = tr_evt;
                 g_tc_trace[3] = tr_full;
                 g_tc_trace[4] = clock64() - tr_start;

@@ -210,3 +210,22 @@ def test_rollout_argument_errors(torch_cuda):
                                   C.c_void_p(vals.data_ptr()), None, None, None, None)
     assert rc == 1  # misaligned
     ctx.close()
+
+
+def test_best_action_matches_argmax(torch_cuda):
+    """voila_best_action: q* = argmax_q V_q with ties to the lowest q and NaN never winning; the
+    returned action is action_seqs[q*][0] (root action selection, include/voila.h)."""
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    ctx = vl.Voila(synth.make_model(synth.CONFIGS[1]))
+    rng = np.random.default_rng(11)
+    for Q, H in [(1, 1), (7, 3), (1000, 10), (4096, 30), (100_003, 2)]:
+        v = rng.standard_normal(Q).astype(np.float32)
+        seqs = rng.integers(0, 4, size=(Q, H), dtype=np.int32)
+        if Q > 6:
+            v[[3, 5]] = v.max() + 1.0          # a tie: the lower index must win
+            v[1] = np.nan                      # NaN never wins
+        bq, ba = ctx.voila_best_action(torch.from_numpy(v).cuda(), torch.from_numpy(seqs).cuda())
+        ref = int(np.nanargmax(v))
+        assert int(bq.item()) == ref and int(ba.item()) == int(seqs[ref, 0])
+    ctx.close()
