@@ -202,6 +202,9 @@ def run_voila(args):
     seed0 = replicas.replica_seed(20260619, rank, 0, 0)  # replicas draw different noise
 
     state = {"parts": parts, "bu_parts": bu_parts}
+    # belief-update outputs are allocated once and reused (two sets: the chained configs feed the
+    # resampled particles back in, and the output must not alias the input)
+    bu_bufs = [ctx.belief_update_buffers(bu_parts, want_debug=False) for _ in range(2)]
 
     def pick_action(values):
         """CFG5 protocol: the executed action is the first action of argmax_q V_q, taken
@@ -215,7 +218,7 @@ def run_voila(args):
     def step(k):
         out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * k, want_witness=True)
         bu = ctx.voila_belief_update(state["bu_parts"], pick_action(out["values"]), obs_all[k], bu_w,
-                                     seed0 + 2 * k + 1, want_debug=False)
+                                     seed0 + 2 * k + 1, want_debug=False, out=bu_bufs[k & 1])
         if chain:
             state["parts"] = state["bu_parts"] = bu["particles"]
         return out, bu
@@ -242,7 +245,8 @@ def run_voila(args):
         out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * (k + args.warmup))
         ev[k][1].record(stream)
         bu = ctx.voila_belief_update(state["bu_parts"], pick_action(out["values"]), obs_all[k + args.warmup], bu_w,
-                                     seed0 + 2 * (k + args.warmup) + 1, want_debug=False)
+                                     seed0 + 2 * (k + args.warmup) + 1, want_debug=False,
+                                     out=bu_bufs[(k + args.warmup) & 1])
         ev[k][2].record(stream)
         if chain:
             state["parts"] = state["bu_parts"] = bu["particles"]

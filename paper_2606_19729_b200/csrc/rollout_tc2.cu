@@ -15,6 +15,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -517,11 +518,14 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
 //   operand = [s'_i] -> g hidden layers -> SCORE: l_i = <e, D + b>, L_i = log w_i + l_i / lambda
 //   -> logits, ordered-int running maximum, prior-weight partial sums.
 // P = N and H = 1 in T2Params; the action is the same for every particle, so the action-dependent
-// bias rows are parked once in slot 0 of the shared-memory bias table.
+// bias rows are parked once in slot 0 of the shared-memory bias table.  Rows stream HBM -> operand
+// buffer -> HBM: no per-row register state, so a TWO-SLOT program (hdr.n_slots == 2: narrow models)
+// keeps two units in flight, each layer record naming its slot; the epilogue of one unit then
+// overlaps the MMAs of the other.
 __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                                uint64_t *evt, uint64_t *layer_done, float *sbias, int warp, int lane,
                                                uint32_t rank, int cluster_id, int n_clusters, int n_my_units) {
-    const int n_layers = p.hdr.n_layers;
+    const int n_layers = p.hdr.n_layers, n_slots = p.hdr.n_slots;
     const int ew = warp - 4, qd = warp & 3, half = ew >> 2;
     const int row = qd * 32 + lane;
     const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
@@ -529,10 +533,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
     const int in_units = p.hdr.in_chunks * 8;   // f_T input operand, 8-column units
     const int g_units = p.hdr.g_in_chunks * 8;  // g input operand
     const float *e_s = sbias + p.hdr.e_off;
-    uint32_t persist[32];  // packed bf16 state of this thread's particle (half 0)
-    uint32_t nz[16];
-    int unit_i = 0, i_idx = 0;
-    bool valid = false;
+    int unit_i = 0;
     EpiSync es;
     es.evt_cl = mapa_u32(smem_u32(evt), 0u);
     es.layer_done = layer_done;
@@ -553,88 +554,100 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
         for (int c = tid_e; c < p.hdr.e_pad; c += 256) sbias[p.hdr.e_off + c] = c < p.d ? __ldg(p.bu_e + c) : 0.0f;
     }
 
-    auto load_unit = [&]() {
-        const int unit = cluster_id + unit_i * n_clusters;
-        i_idx = (unit * 2 + (int)rank) * kT2Rows + row;
-        valid = i_idx < p.P;
-        if (half == 0) {
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                if (8 * u < S && valid) v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)i_idx * S) + u);
-                persist[4 * u] = v.x; persist[4 * u + 1] = v.y;
-                persist[4 * u + 2] = v.z; persist[4 * u + 3] = v.w;
-            }
-            gen_noise_call(nz, p.seed, (uint32_t)i_idx, 0u, 0u, kStreamBeliefT, Nz);
-        }
+    // particle index of this thread's row in (unit, slot)
+    auto row_index = [&](int unit_local, int slot) {
+        const int unit = cluster_id + unit_local * n_clusters;
+        return ((unit * n_slots + slot) * 2 + (int)rank) * kT2Rows + row;
     };
-    auto write_ft_input = [&]() {  // [s ; w ; 0]
-        if (half == 0) {
+    // f_T input [s_i ; w_i ; 0] of a row straight into the slot's operand chunks (half 0 warps)
+    auto load_input = [&](int unit_local, int slot, uint32_t a_slot) {
+        if (half != 0) return;
+        const int i_idx = row_index(unit_local, slot);
+        const bool valid = i_idx < p.P;
 #pragma unroll
-            for (int u = 0; u < 8; ++u)
-                if (8 * u < S)
-                    st_shared_v4(a_unit_addr(a_u32, row, u), persist[4 * u], persist[4 * u + 1], persist[4 * u + 2],
-                                 persist[4 * u + 3]);
-            const int u0 = S >> 3;
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (8 * u < Nz)
-                    st_shared_v4(a_unit_addr(a_u32, row, u0 + u), nz[4 * u], nz[4 * u + 1], nz[4 * u + 2], nz[4 * u + 3]);
-            for (int u = u0 + (Nz >> 3); u < in_units; ++u) st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
+        for (int u = 0; u < 8; ++u) {
+            if (8 * u < S) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (valid) v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)i_idx * S) + u);
+                st_shared_v4(a_unit_addr(a_slot, row, u), v.x, v.y, v.z, v.w);
+            }
         }
+        const int u0 = S >> 3;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (8 * u < Nz) {
+                const uint4 v = noise_unit8(p.seed, (uint32_t)i_idx, 0u, 0u, kStreamBeliefT, (uint32_t)u);
+                st_shared_v4(a_unit_addr(a_slot, row, u0 + u), v.x, v.y, v.z, v.w);
+            }
+        }
+        for (int u = u0 + (Nz >> 3); u < in_units; ++u) st_shared_v4(a_unit_addr(a_slot, row, u), 0u, 0u, 0u, 0u);
     };
 
     if (n_my_units > 0) {
-        load_unit();
-        write_ft_input();
-        named_bar_sync(1, 256);  // also orders the bias-table writes above before their first use
-        fence_proxy_async_smem();
-        es.arrive_event();
+        for (int s = 0; s < n_slots; ++s) {  // one initial event per slot (hdr.init_events)
+            load_input(0, s, a_u32 + (uint32_t)(s * p.hdr.slot_chunks) * kT2ChunkBytes);
+            named_bar_sync(1, 256);  // also orders the bias-table writes above before their first use
+            fence_proxy_async_smem();
+            es.arrive_event();
+        }
     }
     for (int step = 0; step < n_my_units; ++step) {
         for (int li = 0; li < n_layers; ++li) {
             const T2Layer l = L[li];
+            const int slot = l.slot;
             const float *bias = sbias + l.sbias_off;
+            const uint32_t a_slot = a_u32 + (uint32_t)l.chunk_off * kT2ChunkBytes;
+            const uint32_t taddr = lane_taddr + (uint32_t)l.col_off;
             if (l.epi == T2_EPI_HIDDEN) {
-                epi_hidden_layer(es, l, (int)l.sbias_off, ec);
+                EpiConst ecs = ec;
+                ecs.st_base += (uint32_t)l.chunk_off * kT2ChunkBytes;
+                ecs.taddr0 += (uint32_t)l.col_off;
+                epi_hidden_layer(es, l, (int)l.sbias_off, ecs);
             } else if (l.epi == T2_EPI_PROPOSAL) {
+                const int i_idx = row_index(step, slot);
+                const bool valid = i_idx < p.P;
                 es.wait_layer();
                 if (half == 0) {
+                    // the stored particle is what the filter carries forward: bf16(s'); 16 columns
+                    // at a time: TMEM -> + bias -> bf16 -> operand buffer (g's input) and HBM
 #pragma unroll
                     for (int g = 0; g < 4; ++g) {
                         if (16 * g < (int)l.n_pad) {
-                            uint32_t v[16];
-                            tmem_ld16(lane_taddr + 16 * g, v);
+                            uint32_t v[16], o[8];
+                            tmem_ld16(taddr + 16 * g, v);
                             float4 b[4];
 #pragma unroll
                             for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
                             tmem_ld_wait();
 #pragma unroll
                             for (int i = 0; i < 4; ++i) {
-                                persist[8 * g + 2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
-                                                                    __uint_as_float(v[4 * i + 1]) + b[i].y);
-                                persist[8 * g + 2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
-                                                                        __uint_as_float(v[4 * i + 3]) + b[i].w);
+                                o[2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
+                                                       __uint_as_float(v[4 * i + 1]) + b[i].y);
+                                o[2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
+                                                           __uint_as_float(v[4 * i + 3]) + b[i].w);
+                            }
+#pragma unroll
+                            for (int h2 = 0; h2 < 2; ++h2) {
+                                const int u = 2 * g + h2;
+                                if (8 * u < S) {
+                                    st_shared_v4(a_unit_addr(a_slot, row, u), o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2],
+                                                 o[4 * h2 + 3]);
+                                    if (valid)
+                                        *(reinterpret_cast<uint4 *>(p.bu_proposals + (size_t)i_idx * S) + u) =
+                                            make_uint4(o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2], o[4 * h2 + 3]);
+                                }
                             }
                         }
                     }
-                    // the stored particle is what the filter carries forward: bf16(s')
-#pragma unroll
-                    for (int u = 0; u < 8; ++u)
-                        if (8 * u < S) {
-                            st_shared_v4(a_unit_addr(a_u32, row, u), persist[4 * u], persist[4 * u + 1],
-                                         persist[4 * u + 2], persist[4 * u + 3]);
-                            if (valid)
-                                *(reinterpret_cast<uint4 *>(p.bu_proposals + (size_t)i_idx * S) + u) =
-                                    make_uint4(persist[4 * u], persist[4 * u + 1], persist[4 * u + 2], persist[4 * u + 3]);
-                        }
                 } else {
-                    for (int u = S >> 3; u < g_units; ++u) st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
+                    for (int u = S >> 3; u < g_units; ++u) st_shared_v4(a_unit_addr(a_slot, row, u), 0u, 0u, 0u, 0u);
                 }
                 fence_proxy_async_smem();
                 tc_fence_before();
                 es.arrive_event();
-            } else {  // T2_EPI_SCORE: last layer of the unit
+            } else {  // T2_EPI_SCORE: last layer of the slot's unit
+                const int i_idx = row_index(step, slot);
+                const bool valid = i_idx < p.P;
                 float w = 1.0f, lw = 0.0f;
                 if (half == 0 && p.weights) {
                     w = valid ? __ldg(p.weights + i_idx) : 0.0f;
@@ -647,7 +660,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                     for (int g = 0; g < 8; ++g) {
                         if (16 * g < (int)l.n_pad) {
                             uint32_t v[16];
-                            tmem_ld16(lane_taddr + 16 * g, v);
+                            tmem_ld16(taddr + 16 * g, v);
                             float4 b[4], e4[4];
 #pragma unroll
                             for (int i = 0; i < 4; ++i) {
@@ -678,11 +691,8 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                         p.bu_part_wsum[i0 >> 5] = ws;
                     }
                 }
-                ++unit_i;
-                if (unit_i < n_my_units) {
-                    load_unit();
-                    write_ft_input();
-                }
+                // this slot's next unit: its input goes into the slot's operand chunks with this event
+                if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot);
                 named_bar_sync(1, 256);
                 fence_proxy_async_smem();
                 tc_fence_before();
@@ -690,6 +700,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             }
         }
     }
+    (void)unit_i;
 }
 
 template <bool BELIEF>
@@ -792,7 +803,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         // warp-uniform); one elected lane issues the MMAs and commits. =====
         if (rank == 0) {
             uint32_t stage = 0, phase = 0;
-            int waited = -1, base = 1, blk_base = 0;
+            int waited = -1, base = p.hdr.init_events, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
             long long tr_evt = 0, tr_full = 0, tr_mma = 0, tr_commit = 0;
@@ -946,6 +957,8 @@ struct Builder2 {
     int col_free[512];
     int a_ready[8];
     int a_chunks = 1;
+    // current slot (two-slot programs): operand chunk / TMEM column offsets of the layers added next
+    int slot = 0, chunk_off = 0, col_off = 0, slot_chunks = 8;
     int n_blocks = 0;  // accumulator blocks of the step so far (each is handed to the epilogues on its own)
     int policy = 0;
 
@@ -954,8 +967,33 @@ struct Builder2 {
         for (int &a : a_ready) a = -1;
     }
 
+    // Two-slot mode: every layer is added once per slot (slot 1 shares slot 0's biases and weight
+    // tiles; its operand chunks / TMEM columns are disjoint, so its dependencies are tracked apart).
+    bool dual = false;
+    std::map<uint32_t, uint32_t> tile_src;  // layer << 16 | block << 8 | first K chunk  ->  src_row of the packed tile
+    void set_dual(int chunks_per_slot, int cols_per_slot) {
+        dual = true;
+        slot_chunks = chunks_per_slot;
+        dual_cols = cols_per_slot;
+        // slot 0's input / accumulator were last touched by the event BEFORE the previous step's last
+        for (int j = 0; j < chunks_per_slot; ++j) a_ready[j] = -2;
+        for (int c = 0; c < cols_per_slot; ++c) col_free[c] = -2;
+    }
+    int dual_cols = 256;
+
     // W: [n0][k0] row-major fp32 ("algorithmic" column order); bias_rows x n0 biases.
     void add_layer(const float *W, int n0, int k0, const float *b, int bias_rows, int epi, int act) {
+        if (!dual) {
+            add_one(W, n0, k0, b, bias_rows, epi, act, -1);
+            return;
+        }
+        slot = 0; chunk_off = 0; col_off = 0;
+        const int li = add_one(W, n0, k0, b, bias_rows, epi, act, -1);
+        slot = 1; chunk_off = slot_chunks; col_off = dual_cols;
+        add_one(W, n0, k0, b, bias_rows, epi, act, li);
+    }
+
+    int add_one(const float *W, int n0, int k0, const float *b, int bias_rows, int epi, int act, int same_as) {
         T2Layer l{};
         const bool hidden = epi == T2_EPI_HIDDEN;
         const int n_pad = hidden ? n0 : rup(n0, 16);
@@ -966,13 +1004,20 @@ struct Builder2 {
         l.act = (uint8_t)act;
         l.bias_per_action = bias_rows > 1;
         const float bscale = (hidden && act == VOILA_ACT_SILU) ? 0.5f : 1.0f;  // see act_biased()
-        for (int r = 0; r < bias_rows; ++r)
-            for (int j = 0; j < n_pad; ++j)
-                bias.push_back((b && j < n0) ? bscale * b[(size_t)r * n0 + j] : 0.0f);
-        a_chunks = std::max(a_chunks, std::max(kc_n, hidden ? n_pad / 64 : 1));
+        if (same_as < 0)
+            for (int r = 0; r < bias_rows; ++r)
+                for (int j = 0; j < n_pad; ++j)
+                    bias.push_back((b && j < n0) ? bscale * b[(size_t)r * n0 + j] : 0.0f);
+        a_chunks = std::max(a_chunks, chunk_off + std::max(kc_n, hidden ? n_pad / 64 : 1));
+        l.slot = (uint8_t)slot;
+        l.chunk_off = (uint8_t)chunk_off;
+        l.col_off = (uint16_t)col_off;
         const int li = (int)layers.size();
         l.sbias_off = (uint32_t)sbias_init.size();
-        if (bias_rows > 1) {
+        if (same_as >= 0) {
+            l.bias_off = layers[same_as].bias_off;
+            l.sbias_off = layers[same_as].sbias_off;
+        } else if (bias_rows > 1) {
             sbias_init.resize(sbias_init.size() + 2 * (size_t)n_pad, 0.0f);
             if (pa_layer[0] < 0) pa_layer[0] = li;
             else if (pa_layer[1] < 0) pa_layer[1] = li;
@@ -986,22 +1031,29 @@ struct Builder2 {
         for (size_t bi = 0; bi < blocks.size(); ++bi) {
             const int bn = blocks[bi], half = bn / 2;
             const int nk_max = std::max(1, std::min(4, 128 / half));
-            int blk_need = -1;
-            for (int c = n_start; c < n_start + bn; ++c) blk_need = std::max(blk_need, col_free[c]);
+            int blk_need = -1000;
+            for (int c = n_start; c < n_start + bn; ++c) blk_need = std::max(blk_need, col_free[col_off + c]);
             for (int kc0 = 0; kc0 < kc_n; kc0 += nk_max) {
                 const int nk = std::min(nk_max, kc_n - kc0);
                 T2Tile t{};
                 t.src_row = (uint32_t)(wstream.size() / 128);
                 t.idesc = umma_idesc_bf16_m256((uint32_t)bn);
-                t.d_col16 = (uint8_t)(n_start / 16);
+                t.d_col16 = (uint8_t)((col_off + n_start) / 16);
                 t.blk = (uint8_t)(n_blocks + (int)bi);
-                t.kc0 = (uint8_t)kc0;
+                t.kc0 = (uint8_t)(chunk_off + kc0);
                 t.nk = (uint8_t)nk;
                 t.rows8 = (uint8_t)(half / 8);
                 int need = blk_need;
-                for (int c = 0; c < nk; ++c) need = std::max(need, a_ready[kc0 + c]);
+                for (int c = 0; c < nk; ++c) need = std::max(need, a_ready[chunk_off + kc0 + c]);
                 t.need = (int16_t)need;
                 t.flags = (uint8_t)(bi << 4);  // scratch: block index, cleared below
+                const uint32_t key_bk = ((uint32_t)bi << 8) | (uint32_t)kc0;
+                if (same_as >= 0) {  // slot 1 streams the very tile slot 0 packed
+                    t.src_row = tile_src.at(((uint32_t)same_as << 16) | key_bk);
+                    lt.push_back(t);
+                    continue;
+                }
+                tile_src[((uint32_t)li << 16) | key_bk] = t.src_row;
                 // pack: CTA 0's rows then CTA 1's; per CTA chunk by chunk; 16-byte units XOR (row & 7)
                 const size_t base = wstream.size();
                 wstream.resize(base + (size_t)2 * nk * half * 128, 0);
@@ -1052,7 +1104,7 @@ struct Builder2 {
                 if ((int)t.blk != n_blocks - 1) continue;
                 if ((int)t.kc0 <= prev_kc0) bad_order = true;  // signals must arrive in chunk order
                 prev_kc0 = t.kc0;
-                if ((int)t.kc0 < (int)l.wait_chunks) {
+                if ((int)t.kc0 - chunk_off < (int)l.wait_chunks) {
                     t.flags |= 4;
                     ++n_sig;
                 }
@@ -1063,16 +1115,17 @@ struct Builder2 {
         layers.push_back(l);
         if (hidden) {
             for (int j = 0; j < n_pad / 64; ++j) {
-                for (int c = 64 * j; c < 64 * j + 64; ++c) col_free[c] = evt;
-                a_ready[j] = evt;
+                for (int c = 64 * j; c < 64 * j + 64; ++c) col_free[col_off + c] = evt;
+                a_ready[chunk_off + j] = evt;
                 ++evt;
             }
         } else {
-            for (int c = 0; c < n_pad; ++c) col_free[c] = evt;
-            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE)
-                for (int &a : a_ready) a = evt;  // the next layer-1 input is written with this event
+            for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
+            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE)  // the next layer-1 input is written with this event
+                for (int j = chunk_off; j < std::min(8, chunk_off + slot_chunks); ++j) a_ready[j] = evt;
             ++evt;
         }
+        return li;
     }
 };
 
@@ -1088,8 +1141,9 @@ struct T2Program {
 
 struct T2Handle {
     T2Program roll;    // rollout: [reward] + f_T + f_Z per step
-    T2Program belief;  // belief update: f_T + g per 256-particle unit
-    bool has_belief = false;
+    T2Program belief;       // belief update: f_T + g per 256-particle unit
+    T2Program belief_dual;  // the same with two units in flight per CTA pair (narrow models)
+    bool has_belief = false, has_belief_dual = false;
 };
 
 // Layer 1 of a generator sees the "algorithmic" input [s ; w] (K = S + Nz): the one-hot block is
@@ -1138,7 +1192,10 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     g.hdr.pa_layer[0] = pb.pa_layer[0];
     g.hdr.pa_layer[1] = pb.pa_layer[1];
     int max_n = 32;
-    for (const T2Layer &l : pb.layers) max_n = std::max(max_n, (int)l.n_pad);
+    for (const T2Layer &l : pb.layers) max_n = std::max(max_n, (int)l.col_off + (int)l.n_pad);
+    g.hdr.init_events = pb.dual ? 2 : 1;
+    g.hdr.n_slots = pb.dual ? 2 : 1;
+    g.hdr.slot_chunks = pb.dual ? pb.slot_chunks : 0;
     int cols = 32;
     while (cols < max_n) cols *= 2;
     g.hdr.tmem_cols = cols;
@@ -1226,25 +1283,39 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         }
     }
     if (tower_fits_tc2(d)) {
-        // belief-update program: proposal s' = f_T(s, a, w), then the state tower g(s') and the score
-        Builder2 pb;
-        pb.policy = policy;
-        add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
-        const voila_mlp &g = d->lik_state;
-        if (d->lik_action_cond) {
-            add_generator2(pb, g, S, A, 0, T2_EPI_SCORE);
-        } else {
-            for (int l = 0; l < g.n_layers; ++l)
-                pb.add_layer(g.W[l], g.dims[l + 1], g.dims[l], g.b[l], 1,
-                             l == g.n_layers - 1 ? T2_EPI_SCORE : T2_EPI_HIDDEN, g.act);
+        // belief-update program: proposal s' = f_T(s, a, w), then the state tower g(s') and the score.
+        // Narrow models (every layer <= 256 wide, every K <= 256) get a second, TWO-SLOT build: two
+        // units in flight per CTA pair (4 operand chunks and 256 TMEM columns each), so that the
+        // epilogue of one unit overlaps the MMAs of the other; used when there is more than one
+        // unit per CTA pair (large N), while small N keeps the one-slot program (lower latency).
+        int widest = S + Nz;
+        for (int l = 1; l <= d->f_T.n_layers; ++l) widest = std::max(widest, d->f_T.dims[l]);
+        for (int l = 0; l <= d->lik_state.n_layers; ++l) widest = std::max(widest, l == 0 ? S : d->lik_state.dims[l]);
+        const bool want_dual = widest <= 256 && !getenv("VOILA_T2_BELIEF_1SLOT");
+        for (int dual = 0; dual <= (want_dual ? 1 : 0); ++dual) {
+            Builder2 pb;
+            pb.policy = policy;
+            if (dual) pb.set_dual(4, 256);
+            add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
+            const voila_mlp &g = d->lik_state;
+            if (d->lik_action_cond) {
+                add_generator2(pb, g, S, A, 0, T2_EPI_SCORE);
+            } else {
+                for (int l = 0; l < g.n_layers; ++l)
+                    pb.add_layer(g.W[l], g.dims[l + 1], g.dims[l], g.b[l], 1,
+                                 l == g.n_layers - 1 ? T2_EPI_SCORE : T2_EPI_HIDDEN, g.act);
+            }
+            T2Program &prog = dual ? h->belief_dual : h->belief;
+            const int dd = g.dims[g.n_layers];
+            prog.hdr.g_in_chunks = rup(S, 64) / 64;
+            prog.hdr.e_pad = rup(dd, 16);
+            prog.hdr.e_off = (int)pb.sbias_init.size();
+            pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
+            const std::string m = finish_program(pb, prog, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+            // without a one-slot program the CUDA-core propose+score kernel serves the belief update
+            if (dual) h->has_belief_dual = m.empty();
+            else h->has_belief = m.empty();
         }
-        const int dd = g.dims[g.n_layers];
-        h->belief.hdr.g_in_chunks = rup(S, 64) / 64;
-        h->belief.hdr.e_pad = rup(dd, 16);
-        h->belief.hdr.e_off = (int)pb.sbias_init.size();
-        pb.sbias_init.resize(pb.sbias_init.size() + (size_t)h->belief.hdr.e_pad, 0.0f);
-        const std::string m = finish_program(pb, h->belief, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
-        h->has_belief = m.empty();  // otherwise the CUDA-core propose+score kernel serves the belief update
     }
     return h;
 }
@@ -1297,13 +1368,17 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
 // part_wsum gets one entry per 32 particles.
 cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const BeliefArgs &a, cudaStream_t st,
                                         int *n_launches) {
-    const T2Program &g = reinterpret_cast<const T2Handle *>(tc)->belief;
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    // two units in flight per CTA pair pay off once a pair has more than one unit to process
+    const bool dual = h->has_belief_dual && a.N > 2 * kT2Rows * h->belief.max_clusters;
+    const T2Program &g = dual ? h->belief_dual : h->belief;
     T2Params p = base_params(g, m);
     p.particles = reinterpret_cast<const uint16_t *>(a.particles);
     p.weights = a.weights;
     p.P = a.N; p.Q = 1; p.H = 1;
     p.seed = a.seed;
-    p.n_units = (a.N + 2 * kT2Rows - 1) / (2 * kT2Rows);
+    const int unit_rows = 2 * kT2Rows * g.hdr.n_slots;  // particles per work unit of a CTA pair
+    p.n_units = (a.N + unit_rows - 1) / unit_rows;
     p.bu_action = a.action;
     p.bu_e = a.e;
     p.bu_proposals = reinterpret_cast<uint16_t *>(a.proposals);

@@ -52,7 +52,14 @@ struct T2Layer {  // what the epilogue needs to know about a layer
     uint8_t act;        // voila_act of a hidden layer
     uint8_t bias_per_action;
     uint8_t blk_mask;   // hidden layers: bit c set = 64-column chunk c is the first of an accumulator block
+    // Two-slot programs (belief update of narrow models): two independent 256-row units are in
+    // flight per CTA pair, each with its own operand chunks and TMEM columns, so the epilogue of
+    // one unit overlaps the MMAs of the other.  A layer record belongs to one slot.
+    uint8_t slot;        // 0 | 1
+    uint8_t chunk_off;   // first operand chunk of the slot
+    uint16_t col_off;    // first TMEM column of the slot
 };
+static_assert(sizeof(T2Layer) == 20, "T2Layer is copied to shared memory as 32-bit words");
 
 struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (16 bytes)
     uint32_t src_row;  // first 128-byte row of the tile in the weight stream (CTA r: + r * rows)
@@ -72,6 +79,9 @@ struct T2Header {
     int tmem_cols, n_stages, in_chunks, blocks_per_step;  // accumulator blocks (hand-offs) per step
     int sbias_floats;     // size of the shared-memory bias table
     int pa_layer[2];      // layers whose bias row depends on the action (-1: none)
+    int init_events;      // events published before the first step (one per slot)
+    int n_slots;          // 1 | 2 units in flight per CTA pair (see T2Layer::slot)
+    int slot_chunks;      // operand chunks per slot
     int g_in_chunks;      // belief program: operand chunks of the state tower's input
     int e_off, e_pad;     // belief program: f(o) in the shared-memory table (float offset, padded length)
 };

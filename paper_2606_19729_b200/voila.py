@@ -264,12 +264,11 @@ class Voila:
             out["final_states"] = finals
         return out
 
-    def voila_belief_update(self, particles, action, observation, weights, seed, want_debug=True):
+    def belief_update_buffers(self, particles, want_debug=True):
+        """Output buffers of voila_belief_update for particle sets shaped like `particles` (the caller
+        may keep and reuse them: pass as `out=`; `out["particles"]` must not alias the input)."""
         torch = self._torch
-        N, S = particles.shape
-        assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
-        assert observation.dtype == torch.float32 and observation.numel() == self.O
-        self._ensure(N=N)
+        N = particles.shape[0]
         dev = particles.device
         out = {
             "particles": torch.empty_like(particles),
@@ -281,6 +280,16 @@ class Voila:
         if want_debug:
             out["post_weights"] = torch.empty(N, dtype=torch.float32, device=dev)
             out["proposals"] = torch.empty_like(particles)
+        return out
+
+    def voila_belief_update(self, particles, action, observation, weights, seed, want_debug=True, out=None):
+        torch = self._torch
+        N, S = particles.shape
+        assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
+        assert observation.dtype == torch.float32 and observation.numel() == self.O
+        self._ensure(N=N)
+        if out is None:
+            out = self.belief_update_buffers(particles, want_debug)
         self._check(self.lib.voila_belief_update(
             self._h, _dptr(particles), N, int(action), _dptr(observation), _dptr(weights),
             C.c_uint64(int(seed)), _dptr(out["particles"]), _dptr(out["weights"]),

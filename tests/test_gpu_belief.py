@@ -88,7 +88,9 @@ def test_belief_update_action_conditioned_tower(torch_cuda, oracle):
 
 @pytest.mark.parametrize("kernel_name", ["ffma", "tcgen05", "pair"])
 @pytest.mark.parametrize("cfg_idx,N", [(2, 1024), (3, 2048), (4, 5000), (5, 700), (3, 1), (4, 255), (4, 257),
-                                       (5, 40_001)])
+                                       (5, 40_001),
+                                       # above 256 x 74 particles narrow models run the TWO-SLOT program
+                                       (4, 40_001), (3, 19_000), (2, 65_536 + 300)])
 def test_belief_update_bf16(torch_cuda, oracle, kernel_name, cfg_idx, N):
     import paper_2606_19729_b200 as vl
     kernel = {"ffma": vl.KERNEL_FFMA, "tcgen05": vl.KERNEL_TCGEN05, "pair": vl.KERNEL_TCGEN05_PAIR}[kernel_name]
@@ -106,12 +108,13 @@ def test_belief_update_bf16_pair_variants(torch_cuda, oracle):
     bias of g's first layer), uniform prior (weights = NULL), another action and seed."""
     import paper_2606_19729_b200 as vl
     cfg = synth.CONFIGS[3]
-    for cond, use_w, action, seed in [(1, False, 5, 99), (0, False, 0, 3), (1, True, 15, 1 << 40)]:
+    for cond, use_w, action, seed, N in [(1, False, 5, 99, 1500), (0, False, 0, 3, 1500), (1, True, 15, 1 << 40, 1500),
+                                         (1, True, 7, 12345, 30_011)]:  # the last one: two-slot program
         model = synth.make_model(cfg, prec=synth.PREC_BF16, lik_action_cond=cond)
-        inp = synth.make_inputs(cfg, N=1500, P=8, Q=1, H=1)
+        inp = synth.make_inputs(cfg, N=N, P=8, Q=1, H=1)
         w = None
         if use_w:
-            w = np.exp(2.0 * np.random.default_rng(4).standard_normal(1500)).astype(np.float32)
+            w = np.exp(2.0 * np.random.default_rng(4).standard_normal(N)).astype(np.float32)
             w[::7] = 0.0
         g = _gpu_bu(torch_cuda, model, inp.bu_particles, action, inp.observation, w, seed, synth.PREC_BF16,
                     vl.KERNEL_TCGEN05_PAIR)
