@@ -524,9 +524,14 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
 // overlaps the MMAs of the other.
 __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                                uint64_t *evt, uint64_t *layer_done, float *sbias, int warp, int lane,
-                                               uint32_t rank, int cluster_id, int n_clusters, int n_my_units) {
+                                               uint32_t rank, int cluster_id, int n_clusters, int n_my_units,
+                                               int my_slot) {
+    // my_slot < 0: this set of eight epilogue warps serves every slot in program order;
+    // my_slot = 0 | 1 (16 epilogue warps): it serves one slot and only keeps the books (event,
+    // accumulator-block and chunk-free sequence numbers) for the other slot's layer records.
     const int n_layers = p.hdr.n_layers, n_slots = p.hdr.n_slots;
-    const int ew = warp - 4, qd = warp & 3, half = ew >> 2;
+    const int ew = (warp - 4) & 7, qd = warp & 3, half = ew >> 2;
+    const uint32_t bar_id = 1u + (uint32_t)(my_slot > 0 ? my_slot : 0);
     const int row = qd * 32 + lane;
     const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
     const int S = p.S, Nz = p.Nz;
@@ -543,7 +548,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 
     // one-time: action rows of the bias table (slot 0), e = f(o)
     {
-        const int tid_e = (int)threadIdx.x - 128;
+        const int tid_e = ((int)threadIdx.x - 128) & 255;  // each set of epilogue warps writes the (same) values
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int li = p.hdr.pa_layer[i];
@@ -585,8 +590,12 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 
     if (n_my_units > 0) {
         for (int s = 0; s < n_slots; ++s) {  // one initial event per slot (hdr.init_events)
+            if (my_slot >= 0 && s != my_slot) {
+                ++es.ev;
+                continue;
+            }
             load_input(0, s, a_u32 + (uint32_t)(s * p.hdr.slot_chunks) * kT2ChunkBytes);
-            named_bar_sync(1, 256);  // also orders the bias-table writes above before their first use
+            named_bar_sync(bar_id, 256);  // also orders the bias-table writes above before their first use
             fence_proxy_async_smem();
             es.arrive_event();
         }
@@ -598,6 +607,13 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             const float *bias = sbias + l.sbias_off;
             const uint32_t a_slot = a_u32 + (uint32_t)l.chunk_off * kT2ChunkBytes;
             const uint32_t taddr = lane_taddr + (uint32_t)l.col_off;
+            if (my_slot >= 0 && slot != my_slot) {  // the other set's record: sequence numbers only
+                const bool hid = l.epi == T2_EPI_HIDDEN;
+                es.ev += hid ? (int)(l.n_pad >> 6) : 1;
+                es.ld_seq += hid ? (uint32_t)__popc((unsigned)l.blk_mask) : 1u;
+                if (hid && l.wait_chunks > 0) es.free_seq += ((uint32_t)l.wait_chunks + l.free_nk - 1u) / l.free_nk;
+                continue;
+            }
             if (l.epi == T2_EPI_HIDDEN) {
                 EpiConst ecs = ec;
                 ecs.st_base += (uint32_t)l.chunk_off * kT2ChunkBytes;
@@ -693,7 +709,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 }
                 // this slot's next unit: its input goes into the slot's operand chunks with this event
                 if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot);
-                named_bar_sync(1, 256);
+                named_bar_sync(bar_id, 256);
                 fence_proxy_async_smem();
                 tc_fence_before();
                 es.arrive_event();
@@ -703,7 +719,10 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
     (void)unit_i;
 }
 
-template <bool BELIEF>
+// NTHREADS: 384 (8 epilogue warps) or 640 (16: one set of 8 per slot of a two-slot program).
+// R_LOW / R_HIGH: registers per thread of the producer/issuer warpgroup and of the epilogue
+// warpgroups after `setmaxnreg` (their total must fit the launch allocation).
+template <bool BELIEF, int NTHREADS, int R_LOW, int R_HIGH>
 __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &wmap) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw_u32 = smem_u32(smem_raw);
@@ -729,13 +748,13 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     {
         const uint32_t *src = reinterpret_cast<const uint32_t *>(p.layers);
         uint32_t *dst = reinterpret_cast<uint32_t *>(L);
-        for (int i = threadIdx.x; i < n_layers * (int)(sizeof(T2Layer) / 4); i += kT2Threads) dst[i] = src[i];
+        for (int i = threadIdx.x; i < n_layers * (int)(sizeof(T2Layer) / 4); i += NTHREADS) dst[i] = src[i];
         src = reinterpret_cast<const uint32_t *>(p.tiles);
         dst = reinterpret_cast<uint32_t *>(T);
-        for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2Tile) / 4); i += kT2Threads) dst[i] = src[i];
-        for (int i = threadIdx.x; i < p.hdr.sbias_floats; i += kT2Threads) sbias[i] = p.sbias_init[i];
+        for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2Tile) / 4); i += NTHREADS) dst[i] = src[i];
+        for (int i = threadIdx.x; i < p.hdr.sbias_floats; i += NTHREADS) sbias[i] = p.sbias_init[i];
         uint4 *az = reinterpret_cast<uint4 *>(smem + map.a);
-        for (int i = threadIdx.x; i < p.hdr.a_chunks * kT2ChunkBytes / 16; i += kT2Threads)
+        for (int i = threadIdx.x; i < p.hdr.a_chunks * kT2ChunkBytes / 16; i += NTHREADS)
             az[i] = make_uint4(0u, 0u, 0u, 0u);
         fence_proxy_async_smem();
     }
@@ -765,7 +784,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
 
     // the epilogue warpgroups take the registers the producer / issuer warpgroup does not need
     if (warp < 4) {
-    setmaxnreg_dec<56>();
+    setmaxnreg_dec<R_LOW>();
     if (warp == 0) {
         // ===== producer: this CTA's half of every weight tile, in issue order, once per step =====
         if (lane == 0) {
@@ -876,10 +895,10 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         }
     }
     } else {
-        setmaxnreg_inc<224>();
+        setmaxnreg_inc<R_HIGH>();
         if (BELIEF)
             t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
-                           n_my_units);
+                           n_my_units, NTHREADS == kT2Threads ? -1 : (warp - 4) >> 3);
         else
             t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
                         n_clusters, n_my_units, total_steps);
@@ -893,11 +912,18 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     rollout_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<false>(p, wmap);
+    tc2_body<false, kT2Threads, 56, 224>(p, wmap);
 }
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     belief_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<true>(p, wmap);
+    tc2_body<true, kT2Threads, 56, 224>(p, wmap);
+}
+// Two-slot belief program with one set of eight epilogue warps PER SLOT (20 warps): the two units'
+// epilogues run concurrently, four epilogue warps per scheduler hide each other's latencies.
+constexpr int kT2ThreadsDual = 640;
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
+    belief_tc2_dual_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    tc2_body<true, kT2ThreadsDual, 40, 104>(p, wmap);
 }
 
 }  // namespace
@@ -1177,7 +1203,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 // many CTA pairs of `kernel` can be resident.  Returns an empty string on success.
 template <typename Kernel>
 std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chunks, int sm_count,
-                           std::vector<void *> *allocs) {
+                           std::vector<void *> *allocs, int n_threads = kT2Threads) {
     if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa || pb.bad_order)
         return "model too deep for the tcgen05 program tables";
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
@@ -1235,7 +1261,7 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     // how many CTA pairs can be resident at once (one CTA per SM; normally sm_count / 2)
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(sm_count & ~1));
-    cfg.blockDim = dim3(kT2Threads);
+    cfg.blockDim = dim3((unsigned)n_threads);
     cfg.dynamicSmemBytes = g.smem_bytes;
     int nc = 0;
     if (cudaOccupancyMaxActiveClusters(&nc, kernel, &cfg) != cudaSuccess || nc < 1) {
@@ -1311,7 +1337,10 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             prog.hdr.e_pad = rup(dd, 16);
             prog.hdr.e_off = (int)pb.sbias_init.size();
             pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
-            const std::string m = finish_program(pb, prog, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+            const std::string m =
+                dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(S + Nz, 64) / 64, sm_count, allocs,
+                                      kT2ThreadsDual)
+                     : finish_program(pb, prog, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
             // without a one-slot program the CUDA-core propose+score kernel serves the belief update
             if (dual) h->has_belief_dual = m.empty();
             else h->has_belief = m.empty();
@@ -1388,7 +1417,8 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
     p.inv_lambda = 1.0f / m.lambda;
     p.d = m.mlp[3].dims[m.mlp[3].n_layers];
     const int clusters = std::min(g.max_clusters, p.n_units);
-    belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (n_launches) *n_launches = 1;
     return cudaGetLastError();
 }
