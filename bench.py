@@ -337,7 +337,7 @@ def run_voila(args):
               "propose_score_us": 1e3 * float(np.mean(kt[1])) if kt[1] else None,
               "scan_us": 1e3 * float(np.mean(kt[2])) if kt[2] else None,
               "resample_gather_us": 1e3 * float(np.mean(kt[3])) if kt[3] else None}
-    if kt[1] and ctx.prec == vl.PREC_BF16 and "tc2" in ctx.voila_last_belief_kernel():
+    if kt[1] and ctx.prec == vl.PREC_BF16 and "belief_tc2_" in ctx.voila_last_belief_kernel():
         tf = N * synth.flops_per_belief_particle(model) / (np.mean(kt[1]) * 1e-3) / 1e12
         belief["propose_score_roofline"] = {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"],
                                             "unit": "TFLOP/s", "frac": tf / peaks["bf16_burst"],

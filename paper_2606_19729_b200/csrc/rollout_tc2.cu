@@ -1396,7 +1396,7 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
 // Belief update, propose + score on the CTA-pair tcgen05 program.
 // part_wsum gets one entry per 32 particles.
 cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const BeliefArgs &a, cudaStream_t st,
-                                        int *n_launches) {
+                                        int *n_launches, std::string *kernel_name) {
     const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
     // two units in flight per CTA pair pay off once a pair has more than one unit to process
     const bool dual = h->has_belief_dual && a.N > 2 * kT2Rows * h->belief.max_clusters;
@@ -1419,6 +1419,9 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
     const int clusters = std::min(g.max_clusters, p.n_units);
     if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
     else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (kernel_name)
+        *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight>"
+                            : "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
     if (n_launches) *n_launches = 1;
     return cudaGetLastError();
 }

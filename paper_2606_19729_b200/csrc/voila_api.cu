@@ -501,11 +501,10 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
     if (use_tc2(ctx) && tc2_has_belief(ctx->tc2)) {
         int n = 0;
         ProfScope prof(ctx, VOILA_K_PROPOSE, st);
-        e = launch_bu_propose_score_tc2(ctx->tc2, ctx->model, a, st, &n);
+        e = launch_bu_propose_score_tc2(ctx->tc2, ctx->model, a, st, &n, &ctx->last_belief_kernel);
         if (e != cudaSuccess) return cuda_fail(ctx, e);
         ctx->launches += n;
         n_parts = (N + 31) / 32;
-        ctx->last_belief_kernel = "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
     } else if (use_tc(ctx) && tc_has_belief(ctx->tc)) {
         int n = 0;
         ProfScope prof(ctx, VOILA_K_PROPOSE, st);

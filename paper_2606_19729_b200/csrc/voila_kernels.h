@@ -66,6 +66,6 @@ cudaError_t launch_rollout_tc2(void *tc2, const ModelDev &m, const RolloutArgs &
                                std::string *kernel_name, int *n_launches);
 // writes one prior-weight partial sum per 32 particles into a.part_wsum
 cudaError_t launch_bu_propose_score_tc2(void *tc2, const ModelDev &m, const BeliefArgs &a,
-                                        cudaStream_t st, int *n_launches);
+                                        cudaStream_t st, int *n_launches, std::string *kernel_name);
 
 }  // namespace voila

@@ -31,7 +31,7 @@ def _gpu_bu(torch, model, particles, action, obs, weights, seed, prec, kernel=0)
     out = ctx.voila_belief_update(parts, action, o, w, seed)
     torch.cuda.synchronize()
     if kernel == vl.KERNEL_TCGEN05_PAIR:  # the tensor-core program really ran (no silent CUDA-core fallback)
-        assert ctx.voila_last_belief_kernel().startswith("belief_tc2_kernel")
+        assert ctx.voila_last_belief_kernel().startswith("belief_tc2_")
     res = {k: t2n(v) if v.dtype != torch.int32 else v.cpu().numpy() for k, v in out.items()}
     ctx.close()
     return res

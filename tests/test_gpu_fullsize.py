@@ -88,7 +88,7 @@ def test_belief_update_full_size_cfg4(torch_cuda, oracle):
     out = ctx.voila_belief_update(parts, 1, torch.from_numpy(inp.observation).cuda(),
                                   torch.from_numpy(inp.bu_weights).cuda(), 4242)
     torch.cuda.synchronize()
-    assert ctx.voila_last_belief_kernel().startswith("belief_tc2_kernel")
+    assert ctx.voila_last_belief_kernel().startswith("belief_tc2_")
     g = {k: t2n(v) if v.dtype != torch.int32 else v.cpu().numpy() for k, v in out.items()}
     ctx.close()
     mism = _check_bu(oracle, model, inp.bu_particles, 1, inp.observation, inp.bu_weights, 4242, g,
