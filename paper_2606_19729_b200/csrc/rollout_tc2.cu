@@ -538,7 +538,6 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
     const int in_units = p.hdr.in_chunks * 8;   // f_T input operand, 8-column units
     const int g_units = p.hdr.g_in_chunks * 8;  // g input operand
     const float *e_s = sbias + p.hdr.e_off;
-    int unit_i = 0;
     EpiSync es;
     es.evt_cl = mapa_u32(smem_u32(evt), 0u);
     es.layer_done = layer_done;
@@ -716,7 +715,6 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             }
         }
     }
-    (void)unit_i;
 }
 
 // NTHREADS: 384 (8 epilogue warps) or 640 (16: one set of 8 per slot of a two-slot program).
