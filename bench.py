@@ -210,7 +210,7 @@ def run_voila(args):
         """CFG5 protocol: the executed action is the first action of argmax_q V_q, taken
         on the device (`voila_best_action`); the 4-byte read-back is the planner's output.  CFG1-4
         update with the fixed action of the config."""
-        if not chain:
+        if cfg.index != 5:
             return inp.bu_action
         _, ba = ctx.voila_best_action(values, seqs)
         return int(ba.item())
@@ -243,8 +243,9 @@ def run_voila(args):
         flush.fill_(k & 0xFF)  # evict L2 between timed iterations (outside the event pairs)
         ev[k][0].record(stream)
         out = ctx.voila_rollout_values(state["parts"], seqs, None, seed0 + 2 * (k + args.warmup))
+        a_exec = pick_action(out["values"])  # planning ends with the executed action (CFG5: 4-byte read-back)
         ev[k][1].record(stream)
-        bu = ctx.voila_belief_update(state["bu_parts"], pick_action(out["values"]), obs_all[k + args.warmup], bu_w,
+        bu = ctx.voila_belief_update(state["bu_parts"], a_exec, obs_all[k + args.warmup], bu_w,
                                      seed0 + 2 * (k + args.warmup) + 1, want_debug=False,
                                      out=bu_bufs[(k + args.warmup) & 1])
         ev[k][2].record(stream)
@@ -281,7 +282,7 @@ def run_voila(args):
 
     def e2e_step(k):
         ctx.voila_rollout_values_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals)
-        a_exec = int(h_seqs[int(np.argmax(h_vals.numpy())), 0]) if chain else inp.bu_action  # ties -> lowest q
+        a_exec = int(h_seqs[int(np.argmax(h_vals.numpy())), 0]) if cfg.index == 5 else inp.bu_action  # ties -> lowest q
         ctx.voila_belief_update_host(h_bu, a_exec, h_obs[k % h_obs.shape[0], :cfg.O], h_w,
                                      seed0 + 2 * k + 1, h_pout, None, h_anc, h_le, h_st)
 
