@@ -229,13 +229,99 @@ __device__ __forceinline__ void epi_hidden_layer(EpiSync &es, const T2Layer &l, 
     else epi_hidden_loop<VOILA_ACT_NONE>(es, l, bias_u32, ec);
 }
 
+// The same layer shared by TWO sets of epilogue warps (640-thread rollout kernel): a set handles the
+// chunks j with (j & 1) == parity and keeps the books for the others (event numbers advance without
+// an arrive; accumulator-block and chunk-free sequence numbers are brought up to date at the end).
+// Every chunk's event still collects 16 arrivals: 8 warps of ONE set in each CTA.
+template <int ACT>
+__device__ __forceinline__ void epi_hidden_loop_par(EpiSync &es, const T2Layer &l, uint32_t bias_u32, const EpiConst &ec,
+                                                    int parity) {
+    uint32_t va[16], vb[16];
+    const int chunks = l.n_pad >> 6;
+    const int wait_chunks = l.wait_chunks, free_nk = l.free_nk;
+    const uint32_t blk_mask = l.blk_mask;
+    const int n_blocks = __popc(blk_mask);
+    const int n_sig = wait_chunks > 0 ? (wait_chunks + free_nk - 1) / free_nk : 0;
+    int free_have = 0, blocks_waited = 0;
+    for (int j = 0; j < chunks; ++j) {
+        if ((j & 1) != parity) {
+            ++es.ev;
+            continue;
+        }
+        // blocks that start at a chunk <= j must have been handed over
+        const int need_blocks = __popc(blk_mask & ((2u << j) - 1u));
+        while (blocks_waited < need_blocks) {
+            es.wait_layer();
+            ++blocks_waited;
+        }
+        const uint32_t row_addr = ec.st_base + (uint32_t)j * kT2ChunkBytes;
+        const uint32_t bj = bias_u32 + 256u * (uint32_t)j;
+        tmem_ld16(ec.taddr0 + (uint32_t)(64 * j), va);
+        tmem_ld_wait();
+        tmem_ld16(ec.taddr0 + (uint32_t)(64 * j + 16), vb);
+        if (j < wait_chunks) {  // in-place store: the last block must have read chunk j
+            const int need_free = j / free_nk + 1;
+            while (free_have < need_free) {
+                es.wait_chunk_free();
+                ++free_have;
+            }
+            tc_fence_after();
+        }
+        hidden_store16<ACT>(va, bj, row_addr, ec.sw[0], ec.sw[1]);
+        tmem_ld_wait();
+        hidden_store16<ACT>(vb, bj + 64u, row_addr, ec.sw[2], ec.sw[3]);
+        fence_proxy_async_smem();
+        tc_fence_before();
+        es.arrive_event();
+    }
+    es.ld_seq += (uint32_t)(n_blocks - blocks_waited);
+    es.free_seq += (uint32_t)(n_sig - free_have);
+}
+__device__ __forceinline__ void epi_hidden_layer_par(EpiSync &es, const T2Layer &l, int bias_float_off,
+                                                     const EpiConst &ec, int parity) {
+    const uint32_t bias_u32 = ec.sbias_u32 + 4u * (uint32_t)bias_float_off;
+    if (l.act == VOILA_ACT_SILU) epi_hidden_loop_par<VOILA_ACT_SILU>(es, l, bias_u32, ec, parity);
+    else if (l.act == VOILA_ACT_RELU) epi_hidden_loop_par<VOILA_ACT_RELU>(es, l, bias_u32, ec, parity);
+    else epi_hidden_loop_par<VOILA_ACT_NONE>(es, l, bias_u32, ec, parity);
+}
+
+// Second set of epilogue warps of the 640-thread rollout kernel (warps 12-19): the odd chunks of
+// every hidden layer, nothing else (no per-row state: 72 registers).
+__device__ __forceinline__ void t2_helper_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
+                                                   uint64_t *evt, uint64_t *layer_done, float *sbias, int warp, int lane,
+                                                   int total_steps) {
+    const int n_layers = p.hdr.n_layers;
+    const int ew = (warp - 4) & 7, qd = warp & 3, half = ew >> 2;
+    const int row = qd * 32 + lane;
+    const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
+    EpiSync es;
+    es.evt_cl = mapa_u32(smem_u32(evt), 0u);
+    es.layer_done = layer_done;
+    es.cfree = layer_done + kT2AccRing;
+    es.lane = lane;
+    const EpiConst ec = make_epi_const(a_u32, lane_taddr, sbias, row, half);
+    es.ev = 1;  // the first set publishes the initial-input event
+    for (int step = 0; step < total_steps; ++step) {
+        for (int li = 0; li < n_layers; ++li) {
+            const T2Layer l = L[li];
+            if (l.epi == T2_EPI_HIDDEN) {
+                epi_hidden_layer_par(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ec, 1);
+            } else {
+                ++es.ev;
+                ++es.ld_seq;
+            }
+        }
+    }
+}
+
 // Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
 // in hidden layers, one 32-column half of every 64-column chunk.  Events are published on the
 // LEADER's mbarriers (remote arrive from the peer CTA).
 __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                             uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
                                             float *sbias, int warp, int lane, uint32_t rank, int cluster_id, int n_clusters,
-                                            int n_my_units, int total_steps) {
+                                            int n_my_units, int total_steps, bool shared_hidden) {
+    // shared_hidden: a second set of epilogue warps takes the odd chunks of the hidden layers
     const int n_layers = p.hdr.n_layers;
     const uint32_t evt_cl = mapa_u32(smem_u32(evt), 0u);
     {
@@ -354,7 +440,9 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 const T2Layer l = L[li];
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
-                    epi_hidden_layer(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ec);
+                    const int boff = (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
+                    if (shared_hidden) epi_hidden_layer_par(es, l, boff, ec, 0);
+                    else epi_hidden_layer(es, l, boff, ec);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
                     if (half == 0) {
@@ -720,7 +808,9 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 // NTHREADS: 384 (8 epilogue warps) or 640 (16: one set of 8 per slot of a two-slot program).
 // R_LOW / R_HIGH: registers per thread of the producer/issuer warpgroup and of the epilogue
 // warpgroups after `setmaxnreg` (their total must fit the launch allocation).
-template <bool BELIEF, int NTHREADS, int R_LOW, int R_HIGH>
+// R_HELP: registers of the second set of epilogue warps (warps 12-19 of a 640-thread kernel);
+// > 0: raised to R_HELP, < 0: lowered to -R_HELP.
+template <bool BELIEF, int NTHREADS, int R_LOW, int R_HIGH, int R_HELP = 0>
 __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &wmap) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw_u32 = smem_u32(smem_raw);
@@ -820,21 +910,29 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         // warp-uniform); one elected lane issues the MMAs and commits. =====
         if (rank == 0) {
             uint32_t stage = 0, phase = 0;
-            int waited = -1, base = p.hdr.init_events, blk_base = 0;
+            int waited0 = -1, waited1 = -1;  // latest event waited for, per publishing set (T2Tile::need2)
+            int base = p.hdr.init_events, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
             long long tr_evt = 0, tr_full = 0, tr_mma = 0, tr_commit = 0;
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
-                T2Tile t = T[0];
                 for (int i = 0; i < n_tiles; ++i) {
-                    const T2Tile nxt = T[i + 1 < n_tiles ? i + 1 : 0];  // prefetch the next record
-                    const int need = base + (int)t.need;
-                    if (need > waited) {
+                    const T2Tile t = T[i];
+                    const int need = base + (int)t.need, need2 = base + (int)t.need2;
+                    // events needed from set 0 and from set 1 (equal entries: one set only)
+                    const int n0 = t.need_set ? need2 : need, n1 = t.need_set ? need : need2;
+                    if (n0 > waited0) {
                         T2_TRACE_T0();
-                        mbar_wait(&evt[need & (kT2EvtRing - 1)], (uint32_t)(need / kT2EvtRing) & 1u);
+                        mbar_wait(&evt[n0 & (kT2EvtRing - 1)], (uint32_t)(n0 / kT2EvtRing) & 1u);
                         T2_TRACE_ADD(tr_evt);
-                        waited = need;
+                        waited0 = n0;
+                    }
+                    if (need2 != need && n1 > waited1) {
+                        T2_TRACE_T0();
+                        mbar_wait(&evt[n1 & (kT2EvtRing - 1)], (uint32_t)(n1 / kT2EvtRing) & 1u);
+                        T2_TRACE_ADD(tr_evt);
+                        waited1 = n1;
                     }
                     {
                         T2_TRACE_T0();
@@ -875,7 +973,6 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                         stage = 0;
                         phase ^= 1u;
                     }
-                    t = nxt;
                 }
                 base += p.hdr.evt_per_step;
                 blk_base += p.hdr.blocks_per_step;
@@ -892,14 +989,23 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             (void)tr_evt; (void)tr_full; (void)tr_start; (void)tr_mma; (void)tr_commit;
         }
     }
-    } else {
+    } else if (NTHREADS == kT2Threads || warp < 12) {
         setmaxnreg_inc<R_HIGH>();
         if (BELIEF)
             t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
-                           n_my_units, NTHREADS == kT2Threads ? -1 : (warp - 4) >> 3);
+                           n_my_units, NTHREADS == kT2Threads ? -1 : 0);
         else
             t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
-                        n_clusters, n_my_units, total_steps);
+                        n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads);
+    } else {
+        // second set of epilogue warps (640-thread kernels)
+        if (R_HELP > 0) setmaxnreg_inc<(R_HELP > 0 ? R_HELP : 24)>();
+        else setmaxnreg_dec<(R_HELP < 0 ? -R_HELP : 24)>();
+        if (BELIEF)
+            t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
+                           n_my_units, 1);
+        else
+            t2_helper_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, total_steps);
     }
 
     tc_fence_before();
@@ -921,7 +1027,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
 constexpr int kT2ThreadsDual = 640;
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
     belief_tc2_dual_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<true, kT2ThreadsDual, 40, 104>(p, wmap);
+    tc2_body<true, kT2ThreadsDual, 40, 104, 104>(p, wmap);
+}
+// Rollout with a second set of epilogue warps that takes the odd chunks of every hidden layer: the
+// layer's epilogue (TMEM read, activation, pack, store) runs on 16 warps, four per scheduler.
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
+    rollout_tc2x_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    tc2_body<false, kT2ThreadsDual, 32, 168, -56>(p, wmap);
 }
 
 }  // namespace
@@ -993,6 +1105,8 @@ struct Builder2 {
 
     // Two-slot mode: every layer is added once per slot (slot 1 shares slot 0's biases and weight
     // tiles; its operand chunks / TMEM columns are disjoint, so its dependencies are tracked apart).
+    bool par_split = false;        // two sets of epilogue warps share every hidden layer (even / odd chunks)
+    std::vector<uint8_t> evt_set;  // set that publishes event e of the step
     bool dual = false;
     std::map<uint32_t, uint32_t> tile_src;  // layer << 16 | block << 8 | first K chunk  ->  src_row of the packed tile
     void set_dual(int chunks_per_slot, int cols_per_slot) {
@@ -1141,15 +1255,37 @@ struct Builder2 {
             for (int j = 0; j < n_pad / 64; ++j) {
                 for (int c = 64 * j; c < 64 * j + 64; ++c) col_free[col_off + c] = evt;
                 a_ready[chunk_off + j] = evt;
+                evt_set.push_back((uint8_t)(par_split ? (j & 1) : 0));
                 ++evt;
             }
         } else {
             for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
             if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE)  // the next layer-1 input is written with this event
                 for (int j = chunk_off; j < std::min(8, chunk_off + slot_chunks); ++j) a_ready[j] = evt;
+            evt_set.push_back(0);
             ++evt;
         }
         return li;
+    }
+
+    // After the last layer: the second wait of every tile (see T2Tile::need2).
+    void finish_needs() {
+        int last_of_set[2] = {-100000, -100000};  // latest event of each set in a step
+        for (int e = 0; e < evt; ++e) last_of_set[evt_set[e]] = e;
+        for (T2Tile &t : tiles) {
+            const int need = t.need;
+            // negative needs name events of the previous step; -1 is its last event (set 0), and
+            // the dual-slot programs' -2 / -1 are handled by their own in-order slots
+            const int set = need >= 0 ? evt_set[need] : 0;
+            t.need_set = (uint8_t)set;
+            int other = -100000;
+            if (par_split) {
+                for (int e = std::min(need, evt) - 1; e >= 0 && other < -1000; --e)
+                    if (evt_set[e] != set) other = e;
+                if (other < -1000 && last_of_set[1 - set] > -1000) other = last_of_set[1 - set] - evt;  // previous step
+            }
+            t.need2 = (int16_t)(other > -1000 ? other : need);
+        }
     }
 };
 
@@ -1168,6 +1304,7 @@ struct T2Handle {
     T2Program belief;       // belief update: f_T + g per 256-particle unit
     T2Program belief_dual;  // the same with two units in flight per CTA pair (narrow models)
     bool has_belief = false, has_belief_dual = false;
+    bool roll_x = false;    // rollout runs the 640-thread kernel (two sets of epilogue warps)
 };
 
 // Layer 1 of a generator sees the "algorithmic" input [s ; w] (K = S + Nz): the one-hot block is
@@ -1204,6 +1341,7 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
                            std::vector<void *> *allocs, int n_threads = kT2Threads) {
     if ((int)pb.layers.size() > kT2MaxLayers || (int)pb.tiles.size() > kT2MaxTiles || pb.too_many_pa || pb.bad_order)
         return "model too deep for the tcgen05 program tables";
+    pb.finish_needs();
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
     pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
     g.hdr.n_layers = (int)pb.layers.size();
@@ -1295,11 +1433,26 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     {
         Builder2 pb;
         pb.policy = policy;
+        // Narrow generators (every hidden layer <= 256 wide) are bound by the epilogue's latency chain:
+        // they run the 640-thread kernel whose two sets of epilogue warps share every hidden layer
+        // (measured: CFG3 +8 %, CFG2 +5 %; 512-wide CFG5 -1 %, so wide models keep eight warps).
+        {
+            int widest = 0;
+            for (int l = 1; l < d->f_T.n_layers; ++l) widest = std::max(widest, d->f_T.dims[l]);
+            for (int l = 1; l < d->f_Z.n_layers; ++l) widest = std::max(widest, d->f_Z.dims[l]);
+            const char *e = getenv("VOILA_T2_ROLLOUT_WARPS");  // "8" | "16": override for A/B runs
+            h->roll_x = e ? atoi(e) == 16 : widest <= 256;
+        }
+        pb.par_split = h->roll_x;
         if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
             pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
         add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
         add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
-        const std::string m = finish_program(pb, h->roll, rollout_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+        // 16 epilogue warps (two sets sharing every hidden layer) unless the 8-warp kernel is asked for
+        const std::string m =
+            h->roll_x ? finish_program(pb, h->roll, rollout_tc2x_kernel, rup(S + Nz, 64) / 64, sm_count, allocs,
+                                       kT2ThreadsDual)
+                      : finish_program(pb, h->roll, rollout_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
         if (!m.empty()) {
             if (err) *err = m;
             delete h;
@@ -1370,7 +1523,8 @@ T2Params base_params(const T2Program &g, const ModelDev &m) {
 
 cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
                                std::string *kernel_name, int *n_launches) {
-    const T2Program &g = reinterpret_cast<const T2Handle *>(tc)->roll;
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    const T2Program &g = h->roll;
     T2Params p = base_params(g, m);
     p.particles = reinterpret_cast<const uint16_t *>(a.particles);
     p.seqs = a.action_seqs;
@@ -1385,8 +1539,11 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     p.tiles_per_q = a.tiles;  // = 2 * blocks_per_q (see rollout_tile_count)
     p.n_units = p.blocks_per_q * a.Q;
     const int clusters = std::min(g.max_clusters, p.n_units);
-    rollout_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
-    if (kernel_name) *kernel_name = "rollout_tc2_kernel<tcgen05 cta_group::2 bf16>";
+    if (h->roll_x) rollout_tc2x_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else rollout_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (kernel_name)
+        *kernel_name = h->roll_x ? "rollout_tc2x_kernel<tcgen05 cta_group::2 bf16, 16 epilogue warps>"
+                                 : "rollout_tc2_kernel<tcgen05 cta_group::2 bf16>";
     if (n_launches) *n_launches = 1;
     return cudaGetLastError();
 }

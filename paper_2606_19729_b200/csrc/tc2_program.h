@@ -61,7 +61,7 @@ struct T2Layer {  // what the epilogue needs to know about a layer
 };
 static_assert(sizeof(T2Layer) == 20, "T2Layer is copied to shared memory as 32-bit words");
 
-struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (16 bytes)
+struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (20 bytes)
     uint32_t src_row;  // first 128-byte row of the tile in the weight stream (CTA r: + r * rows)
     uint32_t idesc;    // tcgen05 instruction descriptor (M = 256, N = bn)
     uint8_t d_col16;   // first accumulator column of the block / 16
@@ -72,7 +72,15 @@ struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block 
     uint8_t rows8;     // weight rows per CTA per chunk / 8 (= bn / 16)
     uint8_t flags;     // bit 0: first tile of its block (overwrite); bit 1: last tile of its block;
                        // bit 2: commit an "operand chunk free" signal after this tile
+    // Events are published in order by each SET of epilogue warps, not across sets (the 640-thread
+    // rollout kernel has two sets sharing every hidden layer: even chunks / odd chunks).  "Every
+    // event <= need has happened" therefore takes two waits: `need` (set `need_set`) and `need2`,
+    // the latest earlier event of the OTHER set (= need when there is one set only).
+    int16_t need2;
+    uint8_t need_set;  // 0 | 1: the set that publishes event `need`
+    uint8_t pad;
 };
+static_assert(sizeof(T2Tile) == 20, "T2Tile is copied to shared memory as 32-bit words");
 
 struct T2Header {
     int n_layers, n_tiles, evt_per_step, a_chunks;
