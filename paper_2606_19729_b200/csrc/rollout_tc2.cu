@@ -911,6 +911,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         if (rank == 0) {
             uint32_t stage = 0, phase = 0;
             int waited0 = -1, waited1 = -1;  // latest event waited for, per publishing set (T2Tile::need2)
+            const uint32_t a_desc_lo = (uint32_t)umma_desc_sw128(a_u32), ring_desc_lo = (uint32_t)umma_desc_sw128(ring_u32);
+            const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0u) >> 32);
             int base = p.hdr.init_events, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
@@ -947,14 +949,22 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
 #ifdef VOILA_T2_TRACE
                     const long long tm0 = clock64();
 #endif
-                    for (int c = 0; c < (int)t.nk; ++c) {
-                        const uint64_t ad = umma_desc_sw128(a_u32 + (uint32_t)(t.kc0 + c) * kT2ChunkBytes);
-                        const uint64_t bd = umma_desc_sw128(ring_u32 + stage * kT2StageBytes + c * chunk_b);
+                    // descriptors differ only in their 14-bit address field (units of 16 bytes): add
+                    // offsets to the low word instead of rebuilding them (the rebuilt form was ~100
+                    // uniform-datapath instructions per tile)
+                    uint32_t a_lo = a_desc_lo + (uint32_t)t.kc0 * (kT2ChunkBytes >> 4);
+                    uint32_t b_lo = ring_desc_lo + stage * (kT2StageBytes >> 4);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {  // a stage holds up to 4 K chunks
+                        if (c >= (int)t.nk) break;
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {  // 64-wide chunk = 4 x (K = 16); +32 bytes per K step
-                            umma_ss_2cta(d, ad + 2u * k, bd + 2u * k, t.idesc, acc);
+                            umma_ss_2cta(d, ((uint64_t)desc_hi << 32) | (a_lo + 2u * k),
+                                         ((uint64_t)desc_hi << 32) | (b_lo + 2u * k), t.idesc, acc);
                             acc = 1u;
                         }
+                        a_lo += kT2ChunkBytes >> 4;
+                        b_lo += chunk_b >> 4;
                     }
 #ifdef VOILA_T2_TRACE
                     const long long tm1 = clock64();
@@ -1433,15 +1443,11 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     {
         Builder2 pb;
         pb.policy = policy;
-        // Narrow generators (every hidden layer <= 256 wide) are bound by the epilogue's latency chain:
-        // they run the 640-thread kernel whose two sets of epilogue warps share every hidden layer
-        // (measured: CFG3 +8 %, CFG2 +5 %; 512-wide CFG5 -1 %, so wide models keep eight warps).
+        // The 640-thread kernel (two sets of epilogue warps sharing every hidden layer) is the default:
+        // measured +11 % on CFG3, +7 % on CFG2, +2 % on CFG5 over the eight-warp kernel.
         {
-            int widest = 0;
-            for (int l = 1; l < d->f_T.n_layers; ++l) widest = std::max(widest, d->f_T.dims[l]);
-            for (int l = 1; l < d->f_Z.n_layers; ++l) widest = std::max(widest, d->f_Z.dims[l]);
             const char *e = getenv("VOILA_T2_ROLLOUT_WARPS");  // "8" | "16": override for A/B runs
-            h->roll_x = e ? atoi(e) == 16 : widest <= 256;
+            h->roll_x = e ? atoi(e) == 16 : true;
         }
         pb.par_split = h->roll_x;
         if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
