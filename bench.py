@@ -323,10 +323,10 @@ def run_voila(args):
                 "frac": achieved / peak, "traffic": None,
                 "peak_kind": "fp32 FFMA: SMs x 128 lanes x 2 flop x max SM clock (CUDA-core kernel)"}
     # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (inputs are
-    # read once and stay in L2; the horizon loop never touches HBM): profiles/r01d_rollout_and_belief.md
+    # read once and stay in L2; the horizon loop never touches HBM): profiles/r01f_rollout_tc2x_cfg5.md
     if cfg.name.startswith("cfg5") and "rollout_tc2" in ctx.voila_last_rollout_kernel():
-        roof["traffic"] = 4343808
-        roof["traffic_from"] = "profiles/r01d_rollout_and_belief.md (ncu --set full, Q=37 launch of the same shapes)"
+        roof["traffic"] = 4435968
+        roof["traffic_from"] = "profiles/r01f_rollout_tc2x_cfg5.md (ncu --set full, Q=37 launch of the same shapes)"
     roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
                  "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
                  "share_of_step": k_ms / ms_per_step})
