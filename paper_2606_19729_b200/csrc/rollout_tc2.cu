@@ -7,7 +7,10 @@
 //             (M = 256, N = bn, K = 16, bf16 -> fp32 in both CTAs' TMEM), multicast commits
 //   warp 2    TMEM allocation
 //   warps 4-11 epilogue: tcgen05.ld accumulator block -> bias + activation -> bf16 -> operand
-//             buffer (in place), Philox noise, reward / return accumulation, observation witness.
+//             buffer (in place), Philox noise, reward / return accumulation, observation witness
+//   warps 12-19 (640-thread kernels: rollout_tc2x_kernel, belief_tc2_dual_kernel) a second set of
+//             epilogue warps: the odd chunks of every hidden layer / the second unit in flight.
+// The same machinery runs the belief update's propose+score program (belief_tc2*_kernel).
 // The horizon loop never leaves the SMs: HBM sees the particle rows once per work unit and the
 // per-unit partial sums; weights come from L2, half a tile per CTA.
 #include <cuda.h>

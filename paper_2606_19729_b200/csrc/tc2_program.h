@@ -16,6 +16,14 @@
 // block n+1.  Because the operand buffer is rewritten in place, the epilogue of an earlier block
 // may store output chunk c only after the LAST block's tile that reads operand chunk c has
 // retired: those tiles commit "operand chunk free" signals (`cfree` ring) in chunk order.
+//
+// Two refinements share this program format:
+//  * two SETS of epilogue warps (640-thread kernels): the second set takes the odd chunks of every
+//    hidden layer.  A set publishes its events in order, the sets are not ordered with respect to
+//    each other, so a tile names two events to wait for (T2Tile::need / need2);
+//  * two SLOTS (belief update of narrow models): two independent 256-row units in flight per CTA
+//    pair, each with its own operand chunks and TMEM columns (T2Layer::slot / chunk_off / col_off),
+//    the program alternating the slots layer by layer, one set of epilogue warps per slot.
 #pragma once
 #include <stdint.h>
 
