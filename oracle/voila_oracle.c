@@ -455,11 +455,27 @@ int vo_resample_systematic(const float *v, int N, uint64_t seed, int32_t *ancest
  *   Any output pointer may be NULL.  Returns 0, or -2 if all weights are zero / m is not finite
  *   (then particles_out := proposals, ancestors := identity).
  * ---------------------------------------------------------------------------------------- */
-int vo_belief_update(const vo_model *m, const float *particles, int N, int action,
-                     const float *observation, const float *weights, uint64_t seed,
-                     float *proposals_out, float *logits_out, float *post_weights_out,
-                     double *log_evidence_out, int32_t *ancestors_out, float *particles_out,
-                     float *weights_out) {
+/* Effective sample size of unnormalised weights (Kong, Liu & Wong 1994; the criterion of adaptive
+ * resampling in SIR filters): ESS = (sum v)^2 / sum v^2, in [1, N]; 0 if all v = 0. */
+double vo_effective_sample_size(const float *v, int N) {
+    double s1 = 0, s2 = 0;
+    for (int i = 0; i < N; ++i) {
+        s1 += (double)v[i];
+        s2 += (double)v[i] * (double)v[i];
+    }
+    return s2 > 0 ? s1 * s1 / s2 : 0.0;
+}
+
+/* Belief update with ADAPTIVE resampling: the filter resamples only when
+ * ESS(v) < ess_threshold * N (ess_threshold = +inf: always, the plain update below).  Otherwise the
+ * proposals are kept (ancestors = identity) and the normalised weights v_i / sum v are carried
+ * forward in weights_out.  ess_out / resampled_out may be NULL. */
+int vo_belief_update_ess(const vo_model *m, const float *particles, int N, int action,
+                         const float *observation, const float *weights, uint64_t seed,
+                         float ess_threshold, float *proposals_out, float *logits_out,
+                         float *post_weights_out, double *log_evidence_out, int32_t *ancestors_out,
+                         float *particles_out, float *weights_out, double *ess_out,
+                         int32_t *resampled_out) {
     int S = m->S, O = m->O, A = m->A;
     const vo_mlp *tf = &m->mlp[2], *tg = &m->mlp[3];
     int d = tf->dims[tf->n_layers];
@@ -506,13 +522,17 @@ int vo_belief_update(const vo_model *m, const float *particles, int N, int actio
         sv += (double)v[i];
         sw += weights ? (double)weights[i] : 1.0;
     }
-    if (status == 0) status = vo_resample_systematic(v, N, seed, anc);
-    if (status) for (int k = 0; k < N; ++k) anc[k] = k;
+    const double ess = status ? 0.0 : vo_effective_sample_size(v, N);
+    const int resample = status == 0 && (isinf(ess_threshold) || ess < (double)ess_threshold * (double)N);
+    if (resample) status = vo_resample_systematic(v, N, seed, anc);
+    if (status || !resample) for (int k = 0; k < N; ++k) anc[k] = k;
+    if (ess_out) *ess_out = ess;
+    if (resampled_out) *resampled_out = (resample && status == 0) ? 1 : 0;
     if (log_evidence_out) *log_evidence_out = status ? -INFINITY : (double)mx + log(sv) - log(sw);
     for (int k = 0; k < N; ++k) {
         if (particles_out)
             for (int j = 0; j < S; ++j) particles_out[(size_t)k * S + j] = prop[(size_t)anc[k] * S + j];
-        if (weights_out) weights_out[k] = 1.0f / (float)N;
+        if (weights_out) weights_out[k] = (resample || status) ? 1.0f / (float)N : (float)((double)v[k] / sv);
         if (ancestors_out) ancestors_out[k] = anc[k];
     }
     if (proposals_out) memcpy(proposals_out, prop, sizeof(float) * (size_t)N * S);
@@ -520,6 +540,17 @@ int vo_belief_update(const vo_model *m, const float *particles, int N, int actio
     if (post_weights_out) memcpy(post_weights_out, v, sizeof(float) * (size_t)N);
     free(prop); free(L); free(v); free(anc);
     return status;
+}
+
+/* The plain SIR update: always resample. */
+int vo_belief_update(const vo_model *m, const float *particles, int N, int action,
+                     const float *observation, const float *weights, uint64_t seed,
+                     float *proposals_out, float *logits_out, float *post_weights_out,
+                     double *log_evidence_out, int32_t *ancestors_out, float *particles_out,
+                     float *weights_out) {
+    return vo_belief_update_ess(m, particles, N, action, observation, weights, seed, INFINITY, proposals_out,
+                                logits_out, post_weights_out, log_evidence_out, ancestors_out, particles_out,
+                                weights_out, NULL, NULL);
 }
 
 /* Normalised weights as the resampler sees them (O6): wbar_i = q_i / W in double. */

@@ -60,6 +60,10 @@ def _lib(real: str = "f32"):
     lib.vo_resample_systematic.restype = i32
     lib.vo_belief_update.argtypes = [vp, vp, i32, i32, vp, vp, u64, vp, vp, vp, vp, vp, vp, vp]
     lib.vo_belief_update.restype = i32
+    lib.vo_belief_update_ess.argtypes = [vp, vp, i32, i32, vp, vp, u64, C.c_float, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vo_belief_update_ess.restype = i32
+    lib.vo_effective_sample_size.argtypes = [vp, i32]
+    lib.vo_effective_sample_size.restype = C.c_double
     lib.vo_normalised_weights.argtypes = [vp, i32, vp]
     lib.vo_normalised_weights.restype = i32
     lib.vo_num_threads.restype = i32
@@ -107,6 +111,11 @@ def resample_systematic(v, seed):
     anc = np.zeros(v.shape[0], dtype=np.int32)
     st = _lib().vo_resample_systematic(_p(v), v.shape[0], int(seed), _p(anc))
     return anc, st
+
+
+def effective_sample_size(v):
+    v = _f32(v)
+    return float(_lib().vo_effective_sample_size(_p(v), v.shape[0]))
 
 
 def normalised_weights(v):
@@ -194,7 +203,9 @@ class OracleModel:
             return values, witness, returns
         return values, witness
 
-    def belief_update(self, particles, action, observation, weights, seed):
+    def belief_update(self, particles, action, observation, weights, seed, ess_threshold=None):
+        """ess_threshold=None: the plain SIR update (always resample); a float: adaptive resampling
+        (resample iff ESS < ess_threshold * N), outputs "ess" and "resampled" added."""
         particles = _f32(particles)
         observation = _f32(observation)
         weights = _f32(weights)
@@ -208,11 +219,22 @@ class OracleModel:
             "weights": np.zeros(N, dtype=np.float32),
         }
         le = np.zeros(1, dtype=np.float64)
-        rc = self.lib.vo_belief_update(self.h, _p(particles), N, int(action), _p(observation),
-                                       _p(weights), int(seed), _p(out["proposals"]),
-                                       _p(out["logits"]), _p(out["post_weights"]), _p(le),
-                                       _p(out["ancestors"]), _p(out["particles"]),
-                                       _p(out["weights"]))
+        if ess_threshold is None:
+            rc = self.lib.vo_belief_update(self.h, _p(particles), N, int(action), _p(observation),
+                                           _p(weights), int(seed), _p(out["proposals"]),
+                                           _p(out["logits"]), _p(out["post_weights"]), _p(le),
+                                           _p(out["ancestors"]), _p(out["particles"]),
+                                           _p(out["weights"]))
+        else:
+            ess = np.zeros(1, dtype=np.float64)
+            res = np.zeros(1, dtype=np.int32)
+            rc = self.lib.vo_belief_update_ess(self.h, _p(particles), N, int(action), _p(observation),
+                                               _p(weights), int(seed), C.c_float(ess_threshold),
+                                               _p(out["proposals"]), _p(out["logits"]),
+                                               _p(out["post_weights"]), _p(le), _p(out["ancestors"]),
+                                               _p(out["particles"]), _p(out["weights"]), _p(ess), _p(res))
+            out["ess"] = float(ess[0])
+            out["resampled"] = int(res[0])
         out["log_evidence"] = float(le[0])
         out["status"] = rc
         return out
