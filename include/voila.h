@@ -190,6 +190,21 @@ voila_status voila_best_action(voila_ctx *ctx, const float *values, const int32_
                                int H, int32_t *best_q_out, int32_t *best_action_out,
                                void *cuda_stream);
 
+/* Belief update with ADAPTIVE resampling (the SIR filter of PAPER.md:77 with the
+ * usual effective-sample-size criterion): ESS = (sum_i v_i)^2 / sum_i v_i^2 of the posterior weights
+ * v_i = exp(L_i - max L).  The filter resamples iff ESS < ess_threshold * N; otherwise
+ * particles_out = proposals, ancestors_out[k] = k and weights_out[k] = v_k / sum v (the normalised
+ * weights are carried to the next update).  ess_threshold > 0; INFINITY = always resample, which is
+ * exactly voila_belief_update.  Every other argument as in voila_belief_update, plus
+ *   ess_out dev [1] fp32 or NULL, resampled_out dev [1] int32 (1 | 0) or NULL.
+ * Errors: VOILA_ERR_INVALID_ARG for ess_threshold <= 0 or NaN. */
+voila_status voila_belief_update_ess(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                     const float *observation, const float *weights, uint64_t seed,
+                                     float ess_threshold, void *particles_out, float *weights_out,
+                                     int32_t *ancestors_out, float *post_weights_out, void *proposals_out,
+                                     float *log_evidence_out, float *ess_out, int32_t *resampled_out,
+                                     int32_t *dev_status_out, void *cuda_stream);
+
 /* Host-buffer variants: every pointer is HOST memory (pinned for best speed); inputs are copied to
  * ctx-owned device staging buffers, the device entry point runs, outputs are copied back and the
  * stream is synchronised.  Optional outputs as above (NULL to skip). */

@@ -30,7 +30,7 @@ __global__ void bu_init_kernel(ScanBuffers sb, int tiles) {
     if (i == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.pad = 0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(kObsThreads) bu_init_obs_kernel(ScanBuffers sb
     if (tid == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.pad = 0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
     __shared__ u64 warp_tot[kWarpsS];
     __shared__ u64 look_tot[kWarpsS];
     __shared__ int look_first[kWarpsS];
-    __shared__ double dsum[kWarpsS];
+    __shared__ double dsum[kWarpsS], dsum2[kWarpsS];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // Tile = CTA index: a look-back only waits for lower-numbered CTAs, which the hardware
     // dispatches first (the same assumption CUB's single-pass scan makes).
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
     }
     u64 c[kItems];
     u64 run = 0;
-    double sv = 0.0;
+    double sv = 0.0, sv2 = 0.0;  // sum v, sum v^2 (effective sample size)
 #pragma unroll
     for (int i = 0; i < kItems; ++i) {
         float v = x[i];
@@ -175,6 +175,7 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
         if (base + i >= N) v = 0.0f;
         x[i] = v;
         sv += (double)v;
+        sv2 += (double)v * (double)v;
         run += quantise_weight(v);
         c[i] = run;
     }
@@ -186,9 +187,15 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
         if (lane >= o) incl += t;
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) sv += __shfl_xor_sync(0xffffffffu, sv, o);
+    for (int o = 16; o > 0; o >>= 1) {
+        sv += __shfl_xor_sync(0xffffffffu, sv, o);
+        sv2 += __shfl_xor_sync(0xffffffffu, sv2, o);
+    }
     if (lane == 31) warp_tot[warp] = incl;
-    if (lane == 0) dsum[warp] = sv;
+    if (lane == 0) {
+        dsum[warp] = sv;
+        dsum2[warp] = sv2;
+    }
     __syncthreads();
     u64 warp_prefix = 0, agg = 0;
 #pragma unroll
@@ -207,10 +214,14 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
             sb.tile_agg[tile] = agg;
             st_flag(sb.tile_flag + tile, kFlagAggregate);
         }
-        double t = 0.0;
+        double t = 0.0, t2 = 0.0;
 #pragma unroll
-        for (int w = 0; w < kWarpsS; ++w) t += dsum[w];
+        for (int w = 0; w < kWarpsS; ++w) {
+            t += dsum[w];
+            t2 += dsum2[w];
+        }
         sb.tile_sumv[tile] = t;
+        sb.tile_sumv[gridDim.x + tile] = t2;
     }
     // Decoupled look-back, one predecessor per THREAD and round (kScanThreads per round): when all
     // tiles of a launch are co-resident nobody owns an inclusive prefix early, and a 32-wide
@@ -297,10 +308,13 @@ __device__ __forceinline__ double fin_block_sum(const double *__restrict__ v, in
 
 __global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb, int N, int tiles, int n_wsum_parts,
                                                                   int has_prior, int from_logits, uint64_t seed,
-                                                                  float *log_evidence_out, int32_t *dev_status_out) {
+                                                                  float ess_threshold, float *log_evidence_out,
+                                                                  int32_t *dev_status_out, float *ess_out,
+                                                                  int32_t *resampled_out) {
     __shared__ double sh[kFinThreads];
     const int tid = threadIdx.x;
     const double sum_v = fin_block_sum(sb.tile_sumv, tiles, sh);
+    const double sum_v2 = fin_block_sum(sb.tile_sumv + tiles, tiles, sh);
     const double sum_wp = has_prior ? fin_block_sum(sb.part_wsum, n_wsum_parts, sh) : 0.0;
     if (tid == 0) {
         const double sum_w = has_prior ? sum_wp : (double)N;
@@ -321,6 +335,13 @@ __global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb
         sb.state->sum_w = sum_w;
         sb.state->max_logit = m;
         sb.state->status = status;
+        // adaptive resampling: resample iff ESS < ess_threshold * N (+inf: always)
+        const double ess = (status == 0 && sum_v2 > 0.0) ? sum_v * sum_v / sum_v2 : 0.0;
+        const int resample = status == 0 && (isinf(ess_threshold) || ess < (double)ess_threshold * (double)N);
+        sb.state->ess = ess;
+        sb.state->resample = resample;
+        if (ess_out) *ess_out = (float)ess;
+        if (resampled_out) *resampled_out = resample;
         if (dev_status_out) *dev_status_out = status;
         if (log_evidence_out)
             *log_evidence_out = status ? -INFINITY : (float)((double)m + log(sum_v) - log(sum_w));
@@ -377,7 +398,8 @@ template <int VEC>
 __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, int N,
                                                               const uint8_t *__restrict__ proposals,
                                                               int row_bytes, uint8_t *particles_out,
-                                                              float *weights_out, int32_t *ancestors_out) {
+                                                              float *weights_out, int32_t *ancestors_out,
+                                                              const float *__restrict__ w_in, int from_logits) {
     __shared__ int anc_s[256];
     __shared__ int range_s[2];
     __shared__ u64 seg[kSegMax];
@@ -389,7 +411,7 @@ __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, in
     u64 rhs_lo = (u64)k * W, rhs_hi = __umul64hi((u64)k, W);
     rhs_lo += U;
     rhs_hi += (rhs_lo < U) ? 1ull : 0ull;
-    if (st.status == 0) {
+    if (st.status == 0 && st.resample) {
         // Ancestors are non-decreasing in k: bracket the CTA's outputs with the ancestors of its
         // first and last output (warps 0 and 1, one cooperative search each).
         if (warp < 2) {
@@ -431,11 +453,19 @@ __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, in
         }
         anc_s[tid] = a;
     } else {
-        anc_s[tid] = k;  // degenerate weights: identity
+        anc_s[tid] = k;  // degenerate weights, or ESS above the threshold: identity
     }
     if (k < N) {
         if (ancestors_out) ancestors_out[k] = anc_s[tid];
-        if (weights_out) weights_out[k] = 1.0f / (float)N;
+        if (weights_out) {
+            float w = 1.0f / (float)N;
+            if (st.status == 0 && !st.resample) {  // no resampling: carry the normalised weights v_k / sum v
+                const float x = w_in[k];
+                const float v = from_logits ? expf(x - st.max_logit) : x;
+                w = (float)((double)v / st.sum_v);
+            }
+            weights_out[k] = w;
+        }
     }
     __syncthreads();
     if (particles_out) {
@@ -482,29 +512,29 @@ cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bo
 
 cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, bool has_prior,
                                uint64_t seed, float *log_evidence_out, int32_t *dev_status_out,
-                               cudaStream_t st) {
+                               cudaStream_t st, float ess_threshold, float *ess_out, int32_t *resampled_out) {
     // n_wsum_parts < 0 marks the stage-level resampler (weights given directly, no logits)
     const int from_logits = n_wsum_parts >= 0;
     bu_finalize_kernel<<<1, kFinThreads, 0, st>>>(sb, N, scan_tiles(N), n_wsum_parts < 0 ? 0 : n_wsum_parts,
-                                          has_prior ? 1 : 0, from_logits, seed, log_evidence_out,
-                                          dev_status_out);
+                                          has_prior ? 1 : 0, from_logits, seed, ess_threshold, log_evidence_out,
+                                          dev_status_out, ess_out, resampled_out);
     return cudaGetLastError();
 }
 
 cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *proposals, int row_bytes,
                                    void *particles_out, float *weights_out, int32_t *ancestors_out,
-                                   cudaStream_t st) {
+                                   cudaStream_t st, const float *w_in, bool from_logits) {
     const int grid = (N + 255) / 256;
     const uint8_t *src = reinterpret_cast<const uint8_t *>(proposals);
     uint8_t *dst = reinterpret_cast<uint8_t *>(particles_out);
     if (row_bytes % 16 == 0)
-        resample_gather_kernel<16><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out);
+        resample_gather_kernel<16><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out, w_in, from_logits ? 1 : 0);
     else if (row_bytes % 8 == 0)
-        resample_gather_kernel<8><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out);
+        resample_gather_kernel<8><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out, w_in, from_logits ? 1 : 0);
     else if (row_bytes % 4 == 0)
-        resample_gather_kernel<4><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out);
+        resample_gather_kernel<4><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out, w_in, from_logits ? 1 : 0);
     else
-        resample_gather_kernel<2><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out);
+        resample_gather_kernel<2><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out, w_in, from_logits ? 1 : 0);
     return cudaGetLastError();
 }
 

@@ -83,7 +83,7 @@ Layout make_layout(const voila_ctx *ctx, int P, int Q, int N) {
     L.tile_flag = take(stiles * sizeof(unsigned));
     L.tile_agg = take(stiles * sizeof(unsigned long long));
     L.tile_incl = take(stiles * sizeof(unsigned long long));
-    L.tile_sumv = take(stiles * sizeof(double));
+    L.tile_sumv = take(2 * stiles * sizeof(double));  // per tile: sum v, then (at + tiles) sum v^2
     L.cdf = take((size_t)N * sizeof(unsigned long long));
     L.part_wsum = take(((size_t)(N + kTileRows - 1) / kTileRows) * sizeof(double));
     L.total = off;
@@ -441,11 +441,11 @@ voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
 
 static voila_status run_resample(voila_ctx *ctx, const ScanBuffers &sb, int N, const void *proposals,
                                  void *particles_out, float *weights_out, int32_t *ancestors_out,
-                                 cudaStream_t st) {
+                                 cudaStream_t st, const float *w_in, bool from_logits) {
     const int esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
     ProfScope prof(ctx, VOILA_K_RESAMPLE, st);
     cudaError_t e = launch_resample_gather(sb, N, proposals, ctx->S * esize, particles_out,
-                                           weights_out, ancestors_out, st);
+                                           weights_out, ancestors_out, st, w_in, from_logits);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 1;
     return VOILA_OK;
@@ -456,7 +456,20 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
                                  void *particles_out, float *weights_out, int32_t *ancestors_out,
                                  float *post_weights_out, void *proposals_out,
                                  float *log_evidence_out, int32_t *dev_status_out, void *cuda_stream) {
+    return voila_belief_update_ess(ctx, particles, N, action, observation, weights, seed, INFINITY, particles_out,
+                                   weights_out, ancestors_out, post_weights_out, proposals_out, log_evidence_out,
+                                   nullptr, nullptr, dev_status_out, cuda_stream);
+}
+
+voila_status voila_belief_update_ess(voila_ctx *ctx, const void *particles, int N, int32_t action,
+                                     const float *observation, const float *weights, uint64_t seed,
+                                     float ess_threshold, void *particles_out, float *weights_out,
+                                     int32_t *ancestors_out, float *post_weights_out, void *proposals_out,
+                                     float *log_evidence_out, float *ess_out, int32_t *resampled_out,
+                                     int32_t *dev_status_out, void *cuda_stream) {
     if (!ctx || !particles || !observation || !particles_out || N < 1) return VOILA_ERR_INVALID_ARG;
+    if (!(ess_threshold > 0.0f)) return VOILA_ERR_INVALID_ARG;  // also rejects NaN
+    if (misaligned(ess_out) || misaligned(resampled_out)) return VOILA_ERR_INVALID_ARG;
     if (action < 0 || action >= ctx->A) return VOILA_ERR_INVALID_ARG;
     if (particles_out == particles || proposals_out == particles) return VOILA_ERR_INVALID_ARG;
     if (misaligned(particles) || misaligned(observation) || misaligned(weights) ||
@@ -524,10 +537,11 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
         e = launch_weight_scan(sb, a.logits, N, true, post_weights_out, st);
     }
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    e = launch_bu_finalize(sb, N, n_parts, weights != nullptr, seed, log_evidence_out, dev_status_out, st);
+    e = launch_bu_finalize(sb, N, n_parts, weights != nullptr, seed, log_evidence_out, dev_status_out, st,
+                           ess_threshold, ess_out, resampled_out);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 2;
-    return run_resample(ctx, sb, N, a.proposals, particles_out, weights_out, ancestors_out, st);
+    return run_resample(ctx, sb, N, a.proposals, particles_out, weights_out, ancestors_out, st, a.logits, true);
 }
 
 voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, uint64_t seed,
@@ -542,10 +556,11 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
     const ScanBuffers sb = scan_buffers(ctx, L);
     cudaError_t e = launch_bu_init(sb, N, st);
     if (e == cudaSuccess) e = launch_weight_scan(sb, v, N, false, nullptr, st);
-    if (e == cudaSuccess) e = launch_bu_finalize(sb, N, -1, false, seed, nullptr, dev_status_out, st);
+    if (e == cudaSuccess)
+        e = launch_bu_finalize(sb, N, -1, false, seed, nullptr, dev_status_out, st, INFINITY, nullptr, nullptr);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 3;
-    return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st);
+    return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st, v, false);
 }
 
 voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,

@@ -73,7 +73,8 @@ struct ScanState {
     float max_logit;
     int status;
     unsigned int tile_counter;
-    unsigned int pad;
+    int resample;        // 1: resample (always, unless adaptive resampling found ESS >= threshold * N)
+    double ess;          // effective sample size (sum v)^2 / sum v^2 of the posterior weights
 };
 
 }  // namespace voila

@@ -38,12 +38,15 @@ cudaError_t launch_bu_init_obs(const ScanBuffers &sb, int N, const MlpDev &f, co
 // from_logits: v_i = exp(L_i - max) (belief update) ; else v_i = in[i] (stage-level resampler)
 cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bool from_logits,
                                float *post_weights_out, cudaStream_t st);
+// ess_threshold: resample iff ESS < ess_threshold * N (INFINITY: always); ess_out / resampled_out may be null
 cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, bool has_prior,
                                uint64_t seed, float *log_evidence_out, int32_t *dev_status_out,
-                               cudaStream_t st);
+                               cudaStream_t st, float ess_threshold, float *ess_out, int32_t *resampled_out);
+// w_in: the array the scan read (logits or weights): without resampling weights_out = v_k / sum v
 cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *proposals,
                                    int row_bytes, void *particles_out, float *weights_out,
-                                   int32_t *ancestors_out, cudaStream_t st);
+                                   int32_t *ancestors_out, cudaStream_t st, const float *w_in,
+                                   bool from_logits);
 
 // ---- rollout_tc.cu : tcgen05 / TMEM / bulk-copy path (bf16 mode) ----
 bool tc_supported(const voila_model_desc *desc, std::string *why);

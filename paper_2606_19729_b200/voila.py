@@ -21,7 +21,7 @@ PREC_FP32, PREC_BF16 = 0, 1
 # every symbol include/voila.h declares (tests check that the library exports all of them)
 EXPORTS = [
     "voila_create", "voila_destroy", "voila_workspace_bytes", "voila_reserve", "voila_set_kernel",
-    "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update",
+    "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update", "voila_belief_update_ess",
     "voila_resample_systematic", "voila_mlp_forward", "voila_best_action",
     "voila_rollout_values_host",
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
@@ -82,6 +82,9 @@ def load_library():
     lib.voila_belief_update.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp, vp,
                                         vp, vp]
     lib.voila_belief_update.restype = i32
+    lib.voila_belief_update_ess.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, C.c_float, vp, vp, vp, vp, vp,
+                                            vp, vp, vp, vp, vp]
+    lib.voila_belief_update_ess.restype = i32
     lib.voila_resample_systematic.argtypes = [vp, vp, i32, u64, vp, vp, vp]
     lib.voila_resample_systematic.restype = i32
     lib.voila_mlp_forward.argtypes = [vp, i32, vp, i32, vp, vp]
@@ -282,7 +285,10 @@ class Voila:
             out["proposals"] = torch.empty_like(particles)
         return out
 
-    def voila_belief_update(self, particles, action, observation, weights, seed, want_debug=True, out=None):
+    def voila_belief_update(self, particles, action, observation, weights, seed, want_debug=True, out=None,
+                            ess_threshold=None):
+        """ess_threshold=None: always resample (voila_belief_update); a float: adaptive resampling
+        (voila_belief_update_ess), outputs "ess" and "resampled" added."""
         torch = self._torch
         N, S = particles.shape
         assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
@@ -290,11 +296,22 @@ class Voila:
         self._ensure(N=N)
         if out is None:
             out = self.belief_update_buffers(particles, want_debug)
-        self._check(self.lib.voila_belief_update(
+        if ess_threshold is None:
+            self._check(self.lib.voila_belief_update(
+                self._h, _dptr(particles), N, int(action), _dptr(observation), _dptr(weights),
+                C.c_uint64(int(seed)), _dptr(out["particles"]), _dptr(out["weights"]),
+                _dptr(out["ancestors"]), _dptr(out.get("post_weights")), _dptr(out.get("proposals")),
+                _dptr(out["log_evidence"]), _dptr(out["status"]), self._stream()), "voila_belief_update")
+            return out
+        if "ess" not in out:
+            out["ess"] = torch.empty(1, dtype=torch.float32, device=particles.device)
+            out["resampled"] = torch.empty(1, dtype=torch.int32, device=particles.device)
+        self._check(self.lib.voila_belief_update_ess(
             self._h, _dptr(particles), N, int(action), _dptr(observation), _dptr(weights),
-            C.c_uint64(int(seed)), _dptr(out["particles"]), _dptr(out["weights"]),
+            C.c_uint64(int(seed)), C.c_float(float(ess_threshold)), _dptr(out["particles"]), _dptr(out["weights"]),
             _dptr(out["ancestors"]), _dptr(out.get("post_weights")), _dptr(out.get("proposals")),
-            _dptr(out["log_evidence"]), _dptr(out["status"]), self._stream()), "voila_belief_update")
+            _dptr(out["log_evidence"]), _dptr(out["ess"]), _dptr(out["resampled"]), _dptr(out["status"]),
+            self._stream()), "voila_belief_update_ess")
         return out
 
     def voila_resample_systematic(self, v, seed):

@@ -226,3 +226,60 @@ def test_belief_update_host_entry(torch_cuda, oracle):
     assert np.array_equal(anc.numpy(), dev["ancestors"])
     assert np.array_equal(pout.numpy(), dev["particles"])
     ctx.close()
+
+
+@pytest.mark.parametrize("prec_name,cfg_idx,N", [("fp32", 2, 3000), ("bf16", 3, 5000), ("bf16", 4, 40_001)])
+def test_belief_update_adaptive_resampling(torch_cuda, oracle, prec_name, cfg_idx, N):
+    """voila_belief_update_ess: ESS against the oracle, both branches of the decision."""
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    bf16 = prec_name == "bf16"
+    prec = synth.PREC_BF16 if bf16 else synth.PREC_FP32
+    cfg = synth.CONFIGS[cfg_idx]
+    model = synth.make_model(cfg, prec=prec, lam=1.25)
+    inp = synth.make_inputs(cfg, N=N, P=8, Q=1, H=1)
+    om = oracle.OracleModel(model)
+    src = synth.bf16_round_np(inp.bu_particles) if bf16 else inp.bu_particles
+    ref_plain = om.belief_update(src, 1, inp.observation, inp.bu_weights, 77)
+    ess_ref = oracle.effective_sample_size(ref_plain["post_weights"])
+    ctx = vl.Voila(model, device=0, prec=prec)
+    parts = ctx.to_particles(inp.bu_particles)
+    obs = torch.from_numpy(inp.observation).cuda()
+    w = None if inp.bu_weights is None else torch.from_numpy(inp.bu_weights).cuda()
+    frac = ess_ref / N
+    for thr, expect in [(2.0 * frac + 0.01, 1), (0.4 * frac, 0)]:  # well away from the boundary (thr may exceed 1)
+        out = ctx.voila_belief_update(parts, 1, obs, w, 77, ess_threshold=thr)
+        torch.cuda.synchronize()
+        g = {k: t2n(v) if v.dtype != torch.int32 else v.cpu().numpy() for k, v in out.items()}
+        o = om.belief_update(src, 1, inp.observation, inp.bu_weights, 77, ess_threshold=thr)
+        assert int(g["status"][0]) == 0 and o["status"] == 0
+        assert int(g["resampled"][0]) == expect == o["resampled"]
+        # ESS is a ratio of sums of v_i: a few % in bf16 mode (v_i themselves are within 5e-2)
+        assert abs(float(g["ess"][0]) - o["ess"]) <= (0.15 if bf16 else 1e-3) * o["ess"]
+        own_ess = oracle.effective_sample_size(g["post_weights"])
+        assert abs(float(g["ess"][0]) - own_ess) <= 1e-4 * own_ess     # consistent with its own weights
+        if expect:
+            anc_ref, st = oracle.resample_systematic(g["post_weights"], 77)
+            assert st == 0 and np.array_equal(g["ancestors"], anc_ref)
+            assert np.all(g["weights"] == np.float32(1.0) / np.float32(N))
+        else:
+            assert np.array_equal(g["ancestors"], np.arange(N))
+            assert np.array_equal(g["particles"], g["proposals"])
+            v = g["post_weights"].astype(np.float64)
+            assert np.allclose(g["weights"], v / v.sum(), rtol=2e-6, atol=0)
+            assert rel_inf(g["weights"], o["weights"]) <= (5e-2 if bf16 else 2e-4)
+    ctx.close()
+
+
+def test_belief_update_ess_argument_errors(torch_cuda):
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    cfg = synth.CONFIGS[1]
+    ctx = vl.Voila(synth.make_model(cfg))
+    inp = synth.make_inputs(cfg, N=64, P=8, Q=1, H=1)
+    parts = ctx.to_particles(inp.bu_particles)
+    obs = torch.from_numpy(inp.observation).cuda()
+    for bad in (0.0, -1.0, float("nan")):
+        with pytest.raises(vl.VoilaError):
+            ctx.voila_belief_update(parts, 1, obs, None, 1, ess_threshold=bad)
+    ctx.close()
