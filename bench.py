@@ -355,6 +355,11 @@ def run_voila(args):
                                    "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
                                    "bytes_per_particle": bytes_scan / N}
 
+    if N < (1 << 17):  # belief updates of a few thousand particles are launch-latency-bound
+        for k in ("resample_roofline", "scan_roofline", "propose_score_roofline"):
+            if k in belief:
+                belief[k]["note"] = "latency-bound at this N: report the microseconds, not the fraction"
+
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
