@@ -129,6 +129,29 @@ def _oracle_sample(cfg, model, inp, target_s=12.0):
     return Ps * Qs * H / dt, cores, desc, dt
 
 
+def _oracle_one_thread(cfg, model, inp, target_s=2.0):
+    """The oracle on ONE host thread (SURVEY 8d asks for both figures): a small rollout slice."""
+    from oracle import voila_oracle as oracle
+    from paper_2606_19729_b200 import synth
+    parts = synth.bf16_round_np(inp.particles) if model.prec == synth.PREC_BF16 else inp.particles
+    om = oracle.OracleModel(model)
+    n = oracle.num_threads()
+    oracle.set_num_threads(1)
+    try:
+        H = inp.action_seqs.shape[1]
+        Pp = min(parts.shape[0], 16)
+        t0 = time.perf_counter()
+        om.rollout_values(parts[:Pp], inp.action_seqs[:1], None, 1)
+        dt = max(time.perf_counter() - t0, 1e-4)
+        Ps = int(min(parts.shape[0], max(Pp, Pp * target_s / dt)))
+        t0 = time.perf_counter()
+        om.rollout_values(parts[:Ps], inp.action_seqs[:1], None, 1)
+        dt = time.perf_counter() - t0
+        return Ps * H / dt
+    finally:
+        oracle.set_num_threads(n)
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     from paper_2606_19729_b200 import synth
@@ -361,6 +384,7 @@ def run_voila(args):
                 belief[k]["note"] = "latency-bound at this N: report the microseconds, not the fraction"
 
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
+    cpu_1t = _oracle_one_thread(cfg, model, inp)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -372,7 +396,8 @@ def run_voila(args):
                    "chained_belief": chain, "reduced": reduced},
         "rollout_ms": float(np.mean(roll_ms)), "belief_update": belief,
         "roofline": roof,
-        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "value_one_thread": cpu_1t},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
     }
     print(json.dumps(line))
