@@ -383,6 +383,13 @@ def run_voila(args):
             if k in belief:
                 belief[k]["note"] = "latency-bound at this N: report the microseconds, not the fraction"
 
+    # SURVEY 8d / north_star also quote the nominal figures: 2250 TFLOP/s dense bf16, ~8 TB/s HBM3e
+    for r in [roof] + [belief[k] for k in ("propose_score_roofline", "resample_roofline", "scan_roofline") if k in belief]:
+        nominal = 2250.0 if r["bound"] == "tensor" else 8000.0 if r["bound"] == "hbm" else None
+        if nominal:
+            r["nominal_peak"] = nominal
+            r["frac_of_nominal"] = r["achieved"] / nominal
+
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     cpu_1t = _oracle_one_thread(cfg, model, inp)
     line = {
