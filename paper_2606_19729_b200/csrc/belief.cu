@@ -30,7 +30,7 @@ __global__ void bu_init_kernel(ScanBuffers sb, int tiles) {
     if (i == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(kObsThreads) bu_init_obs_kernel(ScanBuffers sb
     if (tid == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -282,30 +282,6 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
 
 constexpr int kFinThreads = 1024;
 
-// block sum of doubles, fixed order (bit-reproducible): 8 independent loads per thread and round
-__device__ __forceinline__ double fin_block_sum(const double *__restrict__ v, int n, double *sh) {
-    const int tid = threadIdx.x;
-    double acc = 0.0;
-    int i = tid;
-    for (; i + 7 * kFinThreads < n; i += 8 * kFinThreads) {
-        double t[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) t[u] = v[i + u * kFinThreads];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) acc += t[u];
-    }
-    for (; i < n; i += kFinThreads) acc += v[i];
-    sh[tid] = acc;
-    __syncthreads();
-    for (int o = kFinThreads / 2; o > 0; o >>= 1) {
-        if (tid < o) sh[tid] += sh[tid + o];
-        __syncthreads();
-    }
-    const double r = sh[0];
-    __syncthreads();
-    return r;
-}
-
 __global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb, int N, int tiles, int n_wsum_parts,
                                                                   int has_prior, int from_logits, uint64_t seed,
                                                                   float ess_threshold, float *log_evidence_out,
@@ -313,9 +289,37 @@ __global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb
                                                                   int32_t *resampled_out) {
     __shared__ double sh[kFinThreads];
     const int tid = threadIdx.x;
-    const double sum_v = fin_block_sum(sb.tile_sumv, tiles, sh);
-    const double sum_v2 = fin_block_sum(sb.tile_sumv + tiles, tiles, sh);
-    const double sum_wp = has_prior ? fin_block_sum(sb.part_wsum, n_wsum_parts, sh) : 0.0;
+    // prior-weight partials (one per 32 particles: 32768 at N = 2^20): all 1024 threads, 8 independent
+    // loads per round (the loop is latency-bound); fixed order, so the sum is bit-reproducible
+    double acc = 0.0;
+    if (has_prior) {
+        int i = tid;
+        for (; i + 7 * kFinThreads < n_wsum_parts; i += 8 * kFinThreads) {
+            double t[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) t[u] = sb.part_wsum[i + u * kFinThreads];
+            acc += ((t[0] + t[1]) + (t[2] + t[3])) + ((t[4] + t[5]) + (t[6] + t[7]));
+        }
+        for (; i < n_wsum_parts; i += kFinThreads) acc += sb.part_wsum[i];
+    }
+    sh[tid] = acc;
+    __syncthreads();
+    for (int o = kFinThreads / 2; o > 0; o >>= 1) {
+        if (tid < o) sh[tid] += sh[tid + o];
+        __syncthreads();
+    }
+    const double sum_wp = sh[0];
+    __syncthreads();
+    // sum v (threads [0, 512)) and sum v^2 (threads [512, 1024)) of the scan tiles: two trees at once
+    acc = 0.0;
+    for (int i = tid & 511; i < tiles; i += 512) acc += sb.tile_sumv[(tid < 512 ? 0 : tiles) + i];
+    sh[tid] = acc;
+    __syncthreads();
+    for (int o = 256; o > 0; o >>= 1) {
+        if ((tid & 511) < o) sh[tid] += sh[tid + o];
+        __syncthreads();
+    }
+    const double sum_v = sh[0], sum_v2 = sh[512];
     if (tid == 0) {
         const double sum_w = has_prior ? sum_wp : (double)N;
         const u64 W = sb.state->total_q;
@@ -332,6 +336,7 @@ __global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb
         const u64 lo = x0 * W, hi = __umul64hi(x0, W);
         sb.state->offset_u = (hi << 32) | (lo >> 32);
         sb.state->sum_v = sum_v;
+        sb.state->inv_sum_v = sum_v > 0.0 ? 1.0 / sum_v : 0.0;
         sb.state->sum_w = sum_w;
         sb.state->max_logit = m;
         sb.state->status = status;
@@ -406,12 +411,13 @@ __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, in
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int k0 = blockIdx.x * 256, k = k0 + tid;
     const int rows = min(256, N - k0);
-    const ScanState st = *sb.state;
-    const u64 W = st.total_q, U = st.offset_u;
+    // only the fields needed on the common path stay in registers (the whole struct cost 8 more)
+    const u64 W = sb.state->total_q, U = sb.state->offset_u;
+    const int st_status = sb.state->status, st_resample = sb.state->resample;
     u64 rhs_lo = (u64)k * W, rhs_hi = __umul64hi((u64)k, W);
     rhs_lo += U;
     rhs_hi += (rhs_lo < U) ? 1ull : 0ull;
-    if (st.status == 0 && st.resample) {
+    if (st_status == 0 && st_resample) {
         // Ancestors are non-decreasing in k: bracket the CTA's outputs with the ancestors of its
         // first and last output (warps 0 and 1, one cooperative search each).
         if (warp < 2) {
@@ -459,10 +465,10 @@ __global__ void __launch_bounds__(256) resample_gather_kernel(ScanBuffers sb, in
         if (ancestors_out) ancestors_out[k] = anc_s[tid];
         if (weights_out) {
             float w = 1.0f / (float)N;
-            if (st.status == 0 && !st.resample) {  // no resampling: carry the normalised weights v_k / sum v
+            if (st_status == 0 && !st_resample) {  // no resampling: carry the normalised weights v_k / sum v
                 const float x = w_in[k];
-                const float v = from_logits ? expf(x - st.max_logit) : x;
-                w = (float)((double)v / st.sum_v);
+                const float v = from_logits ? expf(x - sb.state->max_logit) : x;
+                w = (float)((double)v * sb.state->inv_sum_v);  // one DMUL (a double division here costs 8 registers)
             }
             weights_out[k] = w;
         }

@@ -75,6 +75,7 @@ struct ScanState {
     unsigned int tile_counter;
     int resample;        // 1: resample (always, unless adaptive resampling found ESS >= threshold * N)
     double ess;          // effective sample size (sum v)^2 / sum v^2 of the posterior weights
+    double inv_sum_v;    // 1 / sum v (normalised weights without resampling)
 };
 
 }  // namespace voila
