@@ -181,6 +181,24 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
 voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
                                void *cuda_stream);
 
+/* One level of the PORPP preference backup (Eq. 1) on a belief tree
+ * stored as tensors: the level has n_belief belief nodes with n_actions action nodes each (action
+ * node j = b * n_actions + a); action node j owns the observation branches
+ * child_idx[child_off[j] .. child_off[j+1]) (belief nodes of the NEXT level) with weights
+ * child_w = Z(b,a,o):
+ *   Psi(b,a) = logpi0[j] / eta + R[j] + gamma * sum_c child_w[c] * v_next[child_idx[c]]
+ *   V(b)     = (1/eta) log sum_a exp(eta * Psi(b,a))           (max-shifted)
+ * Call once per level, deepest level first, feeding v_out of a level as v_next of the one above.
+ *   R, logpi0 dev [n_belief * n_actions] fp32; child_off dev [n_belief * n_actions + 1] int32;
+ *   child_idx dev int32 / child_w dev fp32 [child_off[last]] (may be NULL when there are no
+ *   branches); v_next dev fp32 (may be NULL when there are no branches);
+ *   psi_out dev [n_belief * n_actions] fp32, v_out dev [n_belief] fp32.
+ * Errors: VOILA_ERR_INVALID_ARG for NULL / non-positive sizes, eta <= 0, gamma < 0. */
+voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const float *logpi0,
+                                      const int32_t *child_off, const int32_t *child_idx, const float *child_w,
+                                      const float *v_next, int n_belief, int n_actions, float eta, float gamma,
+                                      float *psi_out, float *v_out, void *cuda_stream);
+
 /* Root action selection for an open-loop sequence sweep: q* = argmax_q values[q] (ties -> lowest q,
  * NaN never wins), best_action_out[0] = action_seqs[q*][0], best_q_out[0] = q* (the
  * planner returns an action for the current belief; DESIGN.md input recipe, config 5).

@@ -563,6 +563,23 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
     return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st, v, false);
 }
 
+voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const float *logpi0,
+                                      const int32_t *child_off, const int32_t *child_idx, const float *child_w,
+                                      const float *v_next, int n_belief, int n_actions, float eta, float gamma,
+                                      float *psi_out, float *v_out, void *cuda_stream) {
+    if (!ctx || !R || !logpi0 || !child_off || !psi_out || !v_out || n_belief < 1 || n_actions < 1)
+        return VOILA_ERR_INVALID_ARG;
+    if (!(eta > 0.0f) || !(gamma >= 0.0f)) return VOILA_ERR_INVALID_ARG;
+    if ((long long)n_belief * n_actions >= (1ll << 31)) return VOILA_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    const cudaError_t e = launch_porpp_backup_level(R, logpi0, child_off, child_idx, child_w, v_next, n_belief,
+                                                    n_actions, eta, gamma, psi_out, v_out,
+                                                    reinterpret_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 1;
+    return VOILA_OK;
+}
+
 voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
                                void *cuda_stream) {
     if (!ctx || which < 0 || which > 3 || !x || !y || rows < 1) return VOILA_ERR_INVALID_ARG;

@@ -48,6 +48,12 @@ cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *pro
                                    int32_t *ancestors_out, cudaStream_t st, const float *w_in,
                                    bool from_logits);
 
+// ---- porpp.cu : one level of the PORPP preference backup (Eq. 1) ----
+cudaError_t launch_porpp_backup_level(const float *R, const float *logpi0, const int32_t *child_off,
+                                      const int32_t *child_idx, const float *child_w, const float *v_next,
+                                      int n_belief, int A, float eta, float gamma, float *psi_out, float *v_out,
+                                      cudaStream_t st);
+
 // ---- rollout_tc.cu : tcgen05 / TMEM / bulk-copy path (bf16 mode) ----
 bool tc_supported(const voila_model_desc *desc, std::string *why);
 void *tc_create(const voila_model_desc *desc, int sm_count, std::vector<void *> *allocs,

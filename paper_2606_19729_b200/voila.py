@@ -22,7 +22,7 @@ PREC_FP32, PREC_BF16 = 0, 1
 EXPORTS = [
     "voila_create", "voila_destroy", "voila_workspace_bytes", "voila_reserve", "voila_set_kernel",
     "voila_tcgen05_supported", "voila_rollout_values", "voila_belief_update", "voila_belief_update_ess",
-    "voila_resample_systematic", "voila_mlp_forward", "voila_best_action",
+    "voila_resample_systematic", "voila_mlp_forward", "voila_best_action", "voila_porpp_backup_level",
     "voila_rollout_values_host",
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
@@ -91,6 +91,8 @@ def load_library():
     lib.voila_mlp_forward.restype = i32
     lib.voila_best_action.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
     lib.voila_best_action.restype = i32
+    lib.voila_porpp_backup_level.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, C.c_float, C.c_float, vp, vp, vp]
+    lib.voila_porpp_backup_level.restype = i32
     lib.voila_rollout_values_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp]
     lib.voila_rollout_values_host.restype = i32
     lib.voila_belief_update_host.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp,
@@ -346,6 +348,29 @@ class Voila:
         self._check(self.lib.voila_best_action(self._h, _dptr(values), _dptr(action_seqs), Q, H,
                                                _dptr(bq), _dptr(ba), self._stream()), "voila_best_action")
         return bq, ba
+
+    def voila_porpp_backup(self, levels, leaf_values, eta, gamma):
+        """PORPP preference backup (Eq. 1) of a whole tree: `levels[d]` = dict of device tensors
+        R, logpi0 [nb, A] fp32, child_off [nb*A+1] int32, child_idx int32, child_w fp32; one
+        voila_porpp_backup_level call per level, deepest first.  -> (V, Psi) lists over depth."""
+        torch = self._torch
+        D = len(levels)
+        V, Psi = [None] * D, [None] * D
+        v_next = leaf_values
+        for d in range(D - 1, -1, -1):
+            lv = levels[d]
+            nb, A = lv["R"].shape
+            psi = torch.empty((nb, A), dtype=torch.float32, device=lv["R"].device)
+            v = torch.empty(nb, dtype=torch.float32, device=lv["R"].device)
+            self._check(self.lib.voila_porpp_backup_level(
+                self._h, _dptr(lv["R"]), _dptr(lv["logpi0"]), _dptr(lv["child_off"]),
+                _dptr(lv["child_idx"] if lv["child_idx"].numel() else None),
+                _dptr(lv["child_w"] if lv["child_w"].numel() else None),
+                _dptr(v_next if v_next is not None and v_next.numel() else None), nb, A,
+                C.c_float(eta), C.c_float(gamma), _dptr(psi), _dptr(v), self._stream()), "voila_porpp_backup_level")
+            V[d], Psi[d] = v, psi
+            v_next = v
+        return V, Psi
 
     # -- host-buffer variants (pinned torch CPU tensors or numpy arrays) --------------------------
     def voila_rollout_values_host(self, particles, action_seqs, weights, seed, values_out,
