@@ -152,6 +152,38 @@ def _oracle_one_thread(cfg, model, inp, target_s=2.0):
         oracle.set_num_threads(n)
 
 
+def _porpp_leg(ctx, dev, peaks):
+    """one level of the PORPP preference backup (Eq. 1) on a wide synthetic level:
+    2^18 belief nodes x 16 actions x 4 observation branches (inputs 200 MB > L2)."""
+    import torch
+    nb, A, B = 1 << 18, 16, 4
+    na = nb * A
+    g = torch.Generator(device=dev)
+    g.manual_seed(20260619)
+    lv = dict(R=torch.randn((nb, A), generator=g, device=dev),
+              logpi0=torch.full((nb, A), -float(np.log(A)), device=dev),
+              child_off=torch.arange(0, na * B + 1, B, dtype=torch.int32, device=dev),
+              child_idx=torch.randint(0, 1 << 20, (na * B,), generator=g, device=dev, dtype=torch.int32),
+              child_w=torch.full((na * B,), 1.0 / B, device=dev))
+    leaves = torch.randn(1 << 20, generator=g, device=dev)
+    for _ in range(3):
+        ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    a.record()
+    for _ in range(10):
+        ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
+    b.record()
+    torch.cuda.synchronize(dev)
+    ms = a.elapsed_time(b) / 10
+    bytes_alg = na * 16 + na * B * 8 + nb * 4  # R, log pi0, row offset, Psi out; index + weight per branch; V out
+    gbs = bytes_alg / (ms * 1e-3) / 1e9
+    return {"workload": f"{nb} belief nodes x {A} actions x {B} branches, one level", "latency_us": 1e3 * ms,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "bytes_per_action_node": bytes_alg / na,
+                         "note": "random 4-byte gathers of V(child) (L2-resident) bound it, not HBM"}}
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     from paper_2606_19729_b200 import synth
@@ -390,6 +422,8 @@ def run_voila(args):
             r["nominal_peak"] = nominal
             r["frac_of_nominal"] = r["achieved"] / nominal
 
+    porpp = _porpp_leg(ctx, dev, peaks)
+
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     cpu_1t = _oracle_one_thread(cfg, model, inp)
     line = {
@@ -405,7 +439,7 @@ def run_voila(args):
         "roofline": roof,
         "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                          "value_one_thread": cpu_1t},
-        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "porpp_backup": porpp,
     }
     print(json.dumps(line))
     if dist is not None:
