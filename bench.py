@@ -184,6 +184,151 @@ def _porpp_leg(ctx, dev, peaks):
                          "note": "random 4-byte gathers of V(child) (L2-resident) bound it, not HBM"}}
 
 
+def _belief_roofs(N, row_bytes, kt, flop_particle, peaks, belief_kernel, unique_frac=None):
+    """Sub-rooflines of one belief update from the library's per-kernel event pairs (ms lists)."""
+    out = {}
+    if kt[1] and "belief_tc2" in belief_kernel:
+        tf = N * flop_particle / (np.mean(kt[1]) * 1e-3) / 1e12
+        out["propose_score_roofline"] = {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"],
+                                         "unit": "TFLOP/s", "frac": tf / peaks["bf16_burst"],
+                                         "kernel": belief_kernel, "flop_per_particle": flop_particle}
+    if kt[2]:
+        b = N * (4 + 8)  # logit read, CDF write
+        gbs = b / (np.mean(kt[2]) * 1e-3) / 1e9
+        out["scan_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                "frac": gbs / peaks["hbm_gbs"], "bytes_per_particle": 12}
+    if kt[3]:
+        # CDF read 8, row gather, row write, index 4, weight 4.  SURVEY 8(d) also states the count with
+        # only the DISTINCT ancestor rows read (u = measured fraction of distinct ancestors).
+        b = N * (8 + 2 * row_bytes + 8)
+        gbs = b / (np.mean(kt[3]) * 1e-3) / 1e9
+        r = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+             "frac": gbs / peaks["hbm_gbs"], "bytes_per_particle": 8 + 2 * row_bytes + 8}
+        if unique_frac is not None:
+            bu = 8 + row_bytes * unique_frac + row_bytes + 8
+            gu = N * bu / (np.mean(kt[3]) * 1e-3) / 1e9
+            r.update({"unique_ancestor_frac": unique_frac, "bytes_per_particle_unique_rows": bu,
+                      "achieved_unique_rows": gu, "frac_unique_rows": gu / peaks["hbm_gbs"]})
+        out["resample_roofline"] = r
+    for r in out.values():
+        nominal = 2250.0 if r["bound"] == "tensor" else 8000.0
+        r["nominal_peak"] = nominal
+        r["frac_of_nominal"] = r["achieved"] / nominal
+    return out
+
+
+def _leg_belief_cfg4(vl, synth, dev, local, peaks, flush, calls=20):
+    """The belief-update half of the metric at the size it is defined on (BASELINE.json config 4:
+    2^20 particles, skewed prior weights): >= 20 timed calls, L2 flushed between calls, CUDA events
+    on the launching stream; per-kernel times from the library's event pairs; e2e through
+    voila_belief_update_host (pinned host buffers, copies inside the timed region)."""
+    import torch
+    cfg = synth.CONFIGS[4]
+    model = synth.make_model(cfg)
+    inp = synth.make_inputs(cfg)
+    N = cfg.N
+    ctx = vl.Voila(model, device=local)
+    ctx.voila_reserve(0, 0, 0, N)
+    parts = ctx.to_particles(inp.bu_particles)
+    obs = torch.from_numpy(inp.observation).to(dev)
+    w = torch.from_numpy(inp.bu_weights).to(dev)
+    bufs = ctx.belief_update_buffers(parts, want_debug=False)
+    stream = torch.cuda.current_stream(dev)
+    for k in range(3):
+        ctx.voila_belief_update(parts, inp.bu_action, obs, w, 7000 + k, want_debug=False, out=bufs)
+    torch.cuda.synchronize(dev)
+    ctx.voila_set_profiling(True)
+    for which in range(4):
+        ctx.voila_profile_read(which)
+    l0 = ctx.voila_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+    for k in range(calls):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record(stream)
+        ctx.voila_belief_update(parts, inp.bu_action, obs, w, 7100 + k, want_debug=False, out=bufs)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize(dev)
+    launches = ctx.voila_launch_count() - l0
+    ms = [a.elapsed_time(b) for a, b in ev]
+    kt = [ctx.voila_profile_read(which) for which in range(4)]
+    ctx.voila_set_profiling(False)
+    assert int(bufs["status"].item()) == 0
+    uniq = float(torch.unique(bufs["ancestors"]).numel()) / N  # measurement only (distinct ancestor rows)
+    row = cfg.S * 2
+    leg = {"workload": f"{cfg.name}: N={N} particles, prior log-weights ~ N(0,4)", "calls": calls,
+           "latency_us": 1e3 * float(np.mean(ms)), "latency_us_best": 1e3 * float(np.min(ms)),
+           "particles_per_s": N / (float(np.mean(ms)) * 1e-3),
+           "propose_score_us": 1e3 * float(np.mean(kt[1])) if kt[1] else None,
+           "scan_us": 1e3 * float(np.mean(kt[2])) if kt[2] else None,
+           "resample_gather_us": 1e3 * float(np.mean(kt[3])) if kt[3] else None,
+           "gpu_launches_per_call": launches / calls, "l2": "flushed between calls (256 MiB write)"}
+    leg.update(_belief_roofs(N, row, kt, synth.flops_per_belief_particle(model), peaks,
+                             ctx.voila_last_belief_kernel(), unique_frac=uniq))
+    # end to end: host buffers in, resampled particles + ancestors out
+    h_p = parts.cpu().pin_memory()
+    h_w = w.cpu().pin_memory()
+    h_o = obs.cpu().pin_memory()
+    h_out = torch.empty_like(h_p).pin_memory()
+    h_anc = torch.empty(N, dtype=torch.int32).pin_memory()
+    h_le = torch.empty(1, dtype=torch.float32).pin_memory()
+    h_st = torch.empty(1, dtype=torch.int32).pin_memory()
+    ctx.voila_belief_update_host(h_p, inp.bu_action, h_o, h_w, 7200, h_out, None, h_anc, h_le, h_st)
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    n_e2e = 5
+    for k in range(n_e2e):
+        ctx.voila_belief_update_host(h_p, inp.bu_action, h_o, h_w, 7201 + k, h_out, None, h_anc, h_le, h_st)
+    torch.cuda.synchronize(dev)
+    dt = (time.perf_counter() - t0) / n_e2e
+    leg["e2e"] = {"latency_us": 1e6 * dt, "particles_per_s": N / dt, "api": "voila_belief_update_host",
+                  "h2d_bytes_per_call": N * row + N * 4 + cfg.O * 4, "d2h_bytes_per_call": N * row + N * 4 + 8}
+    ctx.close()
+    return leg
+
+
+def _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush, calls=5):
+    """The rollout on the paper-shaped config (BASELINE.json config 3: 48-dim state, 256-wide
+    generators; PAPER.md:165, :171 give 39-45-dim states): full size, L2 flushed between calls."""
+    import torch
+    cfg = synth.CONFIGS[3]
+    model = synth.make_model(cfg)
+    inp = synth.make_inputs(cfg)
+    ctx = vl.Voila(model, device=local)
+    ctx.voila_reserve(cfg.P, cfg.Q, cfg.H, 0)
+    parts = ctx.to_particles(inp.particles)
+    seqs = torch.from_numpy(inp.action_seqs).to(dev)
+    for k in range(3):
+        ctx.voila_rollout_values(parts, seqs, None, 8000 + k)
+    torch.cuda.synchronize(dev)
+    ctx.voila_set_profiling(True)
+    ctx.voila_profile_read(0)
+    stream = torch.cuda.current_stream(dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+    for k in range(calls):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record(stream)
+        out = ctx.voila_rollout_values(parts, seqs, None, 8100 + k)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize(dev)
+    ms = [a.elapsed_time(b) for a, b in ev]
+    kt = ctx.voila_profile_read(0)
+    ctx.voila_set_profiling(False)
+    assert bool(torch.isfinite(out["values"]).all())
+    units = cfg.P * cfg.Q * cfg.H
+    flop = synth.flops_per_rollout_step(model, algorithmic=True)
+    k_ms = float(np.mean(kt)) if kt else float(np.mean(ms))
+    tf = units * flop / (k_ms * 1e-3) / 1e12
+    leg = {"workload": f"{cfg.name}: P={cfg.P} Q={cfg.Q} H={cfg.H}", "calls": calls,
+           "rollout_ms": float(np.mean(ms)), "value": units / (float(np.mean(ms)) * 1e-3), "unit": UNIT,
+           "roofline": {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"], "unit": "TFLOP/s",
+                        "frac": tf / peaks["bf16_burst"], "kernel": ctx.voila_last_rollout_kernel(),
+                        "kernel_ms": k_ms, "flop_per_unit": flop, "units_per_launch": units,
+                        "nominal_peak": 2250.0, "frac_of_nominal": tf / 2250.0,
+                        "peak_kind": f"bf16 burst, {peaks['src']}"}}
+    ctx.close()
+    return leg
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     from paper_2606_19729_b200 import synth
@@ -377,52 +522,37 @@ def run_voila(args):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": None,
                 "peak_kind": "fp32 FFMA: SMs x 128 lanes x 2 flop x max SM clock (CUDA-core kernel)"}
-    # DRAM bytes of one launch from the committed `ncu --set full` capture of this kernel (inputs are
-    # read once and stay in L2; the horizon loop never touches HBM): profiles/r01f_rollout_tc2x_cfg5.md
-    if cfg.name.startswith("cfg5") and "rollout_tc2" in ctx.voila_last_rollout_kernel():
-        roof["traffic"] = 4435968
-        roof["traffic_from"] = "profiles/r01f_rollout_tc2x_cfg5.md (ncu --set full, Q=37 launch of the same shapes)"
+    # roof["traffic"] (DRAM bytes per launch) is only ever a value measured by ncu on a launch of the
+    # SAME size; none is committed for the full-size launch, so the key stays null (the Q=37 capture,
+    # profiles/r01f_rollout_tc2x_cfg5.md, read 4.4 MB: inputs once, the horizon loop never touches HBM)
     roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
                  "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
                  "share_of_step": k_ms / ms_per_step})
     # HBM-bound tail of the belief update (scan + resample/gather), algorithmic bytes per particle
     row = cfg.S * esize
-    bytes_resample = N * (8 + 2 * row + 4 + 4)      # CDF read, row gather, row write, index, weight
-    bytes_scan = N * (4 + 8)                        # logit read, CDF write
     belief = {"latency_us": 1e3 * float(np.mean(bu_ms)),
               "propose_score_us": 1e3 * float(np.mean(kt[1])) if kt[1] else None,
               "scan_us": 1e3 * float(np.mean(kt[2])) if kt[2] else None,
               "resample_gather_us": 1e3 * float(np.mean(kt[3])) if kt[3] else None}
-    if kt[1] and ctx.prec == vl.PREC_BF16 and "belief_tc2_" in ctx.voila_last_belief_kernel():
-        tf = N * synth.flops_per_belief_particle(model) / (np.mean(kt[1]) * 1e-3) / 1e12
-        belief["propose_score_roofline"] = {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"],
-                                            "unit": "TFLOP/s", "frac": tf / peaks["bf16_burst"],
-                                            "kernel": ctx.voila_last_belief_kernel(),
-                                            "flop_per_particle": synth.flops_per_belief_particle(model)}
-    if kt[3]:
-        gbs = bytes_resample / (np.mean(kt[3]) * 1e-3) / 1e9
-        belief["resample_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"],
-                                       "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
-                                       "bytes_per_particle": bytes_resample / N}
-    if kt[2]:
-        gbs = bytes_scan / (np.mean(kt[2]) * 1e-3) / 1e9
-        belief["scan_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"],
-                                   "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
-                                   "bytes_per_particle": bytes_scan / N}
-
+    belief.update(_belief_roofs(N, row, kt, synth.flops_per_belief_particle(model), peaks,
+                                ctx.voila_last_belief_kernel() if ctx.prec == vl.PREC_BF16 else ""))
     if N < (1 << 17):  # belief updates of a few thousand particles are launch-latency-bound
         for k in ("resample_roofline", "scan_roofline", "propose_score_roofline"):
             if k in belief:
                 belief[k]["note"] = "latency-bound at this N: report the microseconds, not the fraction"
 
     # SURVEY 8d / north_star also quote the nominal figures: 2250 TFLOP/s dense bf16, ~8 TB/s HBM3e
-    for r in [roof] + [belief[k] for k in ("propose_score_roofline", "resample_roofline", "scan_roofline") if k in belief]:
-        nominal = 2250.0 if r["bound"] == "tensor" else 8000.0 if r["bound"] == "hbm" else None
-        if nominal:
-            r["nominal_peak"] = nominal
-            r["frac_of_nominal"] = r["achieved"] / nominal
+    if roof["bound"] == "tensor":
+        roof["nominal_peak"] = 2250.0
+        roof["frac_of_nominal"] = roof["achieved"] / 2250.0
 
     porpp = _porpp_leg(ctx, dev, peaks)
+    extra = {}
+    if args.config == DEFAULT_CONFIG and not reduced and not args.no_legs:
+        # BASELINE.json's metric is "rollout steps/sec AND belief-update latency": the latency half is
+        # defined on config 4 (2^20 particles), the paper-shaped rollout on config 3
+        extra["belief_update_cfg4"] = _leg_belief_cfg4(vl, synth, dev, local, peaks, flush)
+        extra["rollout_cfg3"] = _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush)
 
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     cpu_1t = _oracle_one_thread(cfg, model, inp)
@@ -441,6 +571,7 @@ def run_voila(args):
                          "value_one_thread": cpu_1t},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "porpp_backup": porpp,
     }
+    line.update(extra)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -455,6 +586,8 @@ def main():
     ap.add_argument("--impl", default="voila", choices=["voila", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "ffma", "tcgen05"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-legs", action="store_true",
+                    help="skip the config-4 belief-update and config-3 rollout legs of the default line")
     # size overrides for profiling runs (ncu replays every launch ~40 times); the line then says
     # "reduced": true in config and is not a bench value
     for name in ("P", "Q", "H", "N"):

@@ -38,16 +38,36 @@ using namespace tcc;
 __device__ unsigned long long g_t2_trace[64];
 #define T2_TRACE_T0() const long long _t0 = clock64()
 #define T2_TRACE_ADD(var) var += clock64() - _t0
+// Timeline of the leader CTA of cluster 0 (one SM, so clock64 is one clock): (tag, cycle) pairs.
+// tag = kind << 24 | layer-or-step << 8 | chunk-or-tile; kinds: 1 tile ready, 2 tile issued,
+// 3 / 5 epilogue set 0 / 1 starts a chunk or layer (waits done), 4 / 6 it publishes the event.
+constexpr unsigned kT2TlCap = 16384;
+__device__ unsigned long long g_t2_tl[2 * kT2TlCap];
+__device__ unsigned int g_t2_tl_n;
+__device__ int g_t2_tl_win[2] = {40, 44};  // steps [win0, win1) are recorded
+// every recording thread owns a region of the buffer and a private cursor: plain stores only
+// (an atomic's round trip would stall the recorded thread for ~700 cycles per event)
+__device__ __forceinline__ void t2_tl(bool on, uint32_t tag, uint32_t region, uint32_t &cursor) {
+    if (on && cursor < kT2TlCap / 4) {
+        const unsigned i = region * (kT2TlCap / 4) + cursor++;
+        g_t2_tl[2 * i] = tag;
+        g_t2_tl[2 * i + 1] = (unsigned long long)clock64();
+    }
+}
+#define T2_TL(on, tag) t2_tl(on, tag, (es.tl_kind - 1u) >> 1, es.tl_n)
+#define T2_TL_ISSUER(on, tag) t2_tl(on, tag, 0u, tl_n)
 #else
 #define T2_TRACE_T0()
 #define T2_TRACE_ADD(var)
+#define T2_TL(on, tag)
+#define T2_TL_ISSUER(on, tag)
 #endif
 
 struct T2Params {
     const float *bias;        // global: all bias rows (SiLU hidden layers pre-halved)
     const float *sbias_init;  // image of the shared-memory bias table (action rows left empty)
     const T2Layer *layers;
-    const T2Tile *tiles;
+    const T2TileDev *tiles;
     T2Header hdr;
     const uint16_t *particles;  // [P][S] bf16
     const int32_t *seqs;        // [Q][H]
@@ -84,7 +104,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     m.ring = m.a + (uint32_t)h.a_chunks * kT2ChunkBytes;
     m.layers = m.ring + (uint32_t)h.n_stages * kT2StageBytes;
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
-    m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2Tile) + 15u) & ~15u);
+    m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2TileDev) + 15u) & ~15u);
     m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing + kT2FreeRing) * 8;
     m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
     m.total = m.sbias + (((uint32_t)h.sbias_floats * 4u + 15u) & ~15u);
@@ -158,6 +178,9 @@ struct EpiSync {
     uint32_t ld_seq = 0, free_seq = 0;
     int lane;
     long long tr_layer = 0, tr_free = 0, tr_bar = 0;  // wait-cycle trace (VOILA_T2_TRACE)
+    bool tl_on = false;     // timeline trace: this warp records the current step
+    uint32_t tl_kind = 3u;  // 3: first epilogue set, 5: second set
+    uint32_t tl_layer = 0, tl_n = 0;
 
     __device__ __forceinline__ void arrive_event() {
         __syncwarp();
@@ -209,6 +232,7 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
             }
             tc_fence_after();
         }
+        T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | (uint32_t)j);
         hidden_store16<ACT>(va, bj, row_addr, ec.sw[0], ec.sw[1]);
         tmem_ld_wait();
         // the next chunk may belong to a block that is still being accumulated: then publish this
@@ -219,6 +243,7 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
         fence_proxy_async_smem();
         tc_fence_before();
         es.arrive_event();
+        T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | (uint32_t)j);
         if (next_blk) {
             es.wait_layer();
             tmem_ld16(ec.taddr0 + (uint32_t)(64 * (j + 1)), va);
@@ -270,12 +295,14 @@ __device__ __forceinline__ void epi_hidden_loop_par(EpiSync &es, const T2Layer &
             }
             tc_fence_after();
         }
+        T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | (uint32_t)j);
         hidden_store16<ACT>(va, bj, row_addr, ec.sw[0], ec.sw[1]);
         tmem_ld_wait();
         hidden_store16<ACT>(vb, bj + 64u, row_addr, ec.sw[2], ec.sw[3]);
         fence_proxy_async_smem();
         tc_fence_before();
         es.arrive_event();
+        T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | (uint32_t)j);
     }
     es.ld_seq += (uint32_t)(n_blocks - blocks_waited);
     es.free_seq += (uint32_t)(n_sig - free_have);
@@ -304,9 +331,14 @@ __device__ __forceinline__ void t2_helper_epilogue(const T2Params &p, const T2La
     es.lane = lane;
     const EpiConst ec = make_epi_const(a_u32, lane_taddr, sbias, row, half);
     es.ev = 1;  // the first set publishes the initial-input event
+    es.tl_kind = 5u;
     for (int step = 0; step < total_steps; ++step) {
+#ifdef VOILA_T2_TRACE
+        es.tl_on = blockIdx.x == 0 && warp == 12 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+#endif
         for (int li = 0; li < n_layers; ++li) {
             const T2Layer l = L[li];
+            es.tl_layer = (uint32_t)li;
             if (l.epi == T2_EPI_HIDDEN) {
                 epi_hidden_layer_par(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ec, 1);
             } else {
@@ -439,8 +471,12 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         }
         for (int step = 0; step < total_steps; ++step) {
             const int a_t = __ldg(p.seqs + (size_t)q * p.H + t);
+#ifdef VOILA_T2_TRACE
+            es.tl_on = blockIdx.x == 0 && warp == 4 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+#endif
             for (int li = 0; li < n_layers; ++li) {
                 const T2Layer l = L[li];
+                es.tl_layer = (uint32_t)li;
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
                     const int boff = (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
@@ -448,6 +484,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     else epi_hidden_layer(es, l, boff, ec);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
+                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 0) {
                         float r = 0.0f;
 #pragma unroll
@@ -470,6 +507,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     }
                     tc_fence_before();
                     arrive_event();
+                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
                 } else if (l.epi == T2_EPI_STATE) {
                     // w_Z(t) is independent of the state: draw it while the output layer's MMAs run
                     if (half == 1) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
@@ -477,6 +515,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     else if (unit_i + 1 < n_my_units)
                         refresh_issue((cluster_id + (unit_i + 1) * n_clusters) / p.blocks_per_q, 0);
                     wait_layer();
+                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 0) {
 #pragma unroll
                         for (int g = 0; g < 4; ++g) {
@@ -501,11 +540,13 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
+                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
                 } else {  // T2_EPI_OBS: last layer of the step
                     const bool last_step = (t == p.H - 1);
                     if (half == 0 && !last_step)
                         gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)(t + 1), kStreamRolloutT, Nz);
                     wait_layer();
+                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 1) {
 #pragma unroll
                         for (int g = 0; g < 4; ++g) {
@@ -588,6 +629,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
+                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
                 }
             }
         }
@@ -690,9 +732,14 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             es.arrive_event();
         }
     }
+    es.tl_kind = my_slot > 0 ? 5u : 3u;
     for (int step = 0; step < n_my_units; ++step) {
+#ifdef VOILA_T2_TRACE
+        es.tl_on = blockIdx.x == 0 && ew == 0 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+#endif
         for (int li = 0; li < n_layers; ++li) {
             const T2Layer l = L[li];
+            es.tl_layer = (uint32_t)li;
             const int slot = l.slot;
             const float *bias = sbias + l.sbias_off;
             const uint32_t a_slot = a_u32 + (uint32_t)l.chunk_off * kT2ChunkBytes;
@@ -713,6 +760,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 const int i_idx = row_index(step, slot);
                 const bool valid = i_idx < p.P;
                 es.wait_layer();
+                T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                 if (half == 0) {
                     // the stored particle is what the filter carries forward: bf16(s'); 16 columns
                     // at a time: TMEM -> + bias -> bf16 -> operand buffer (g's input) and HBM
@@ -751,6 +799,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 fence_proxy_async_smem();
                 tc_fence_before();
                 es.arrive_event();
+                T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
             } else {  // T2_EPI_SCORE: last layer of the slot's unit
                 const int i_idx = row_index(step, slot);
                 const bool valid = i_idx < p.P;
@@ -760,6 +809,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                     lw = w > 0.0f ? logf(w) : -INFINITY;
                 }
                 es.wait_layer();
+                T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                 if (half == 0) {
                     float ell = 0.0f;
 #pragma unroll
@@ -803,6 +853,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 fence_proxy_async_smem();
                 tc_fence_before();
                 es.arrive_event();
+                T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
             }
         }
     }
@@ -820,7 +871,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     uint8_t *smem = smem_raw + (((raw_u32 + 1023u) & ~1023u) - raw_u32);
     const Smem2 map = smem2_map(p.hdr);
     T2Layer *L = reinterpret_cast<T2Layer *>(smem + map.layers);
-    T2Tile *T = reinterpret_cast<T2Tile *>(smem + map.tiles);
+    T2TileDev *T = reinterpret_cast<T2TileDev *>(smem + map.tiles);
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + map.bars);
     uint64_t *empty = full + 8;
     uint64_t *evt = empty + 8;
@@ -842,7 +893,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         for (int i = threadIdx.x; i < n_layers * (int)(sizeof(T2Layer) / 4); i += NTHREADS) dst[i] = src[i];
         src = reinterpret_cast<const uint32_t *>(p.tiles);
         dst = reinterpret_cast<uint32_t *>(T);
-        for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2Tile) / 4); i += NTHREADS) dst[i] = src[i];
+        for (int i = threadIdx.x; i < n_tiles * (int)(sizeof(T2TileDev) / 4); i += NTHREADS) dst[i] = src[i];
         for (int i = threadIdx.x; i < p.hdr.sbias_floats; i += NTHREADS) sbias[i] = p.sbias_init[i];
         uint4 *az = reinterpret_cast<uint4 *>(smem + map.a);
         for (int i = threadIdx.x; i < p.hdr.a_chunks * kT2ChunkBytes / 16; i += NTHREADS)
@@ -884,16 +935,16 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
-                    const T2Tile t = T[i];
+                    const uint32_t src_row = T[i].src_row;
+                    const int rows = (int)(T[i].misc >> 16);
                     {
                         T2_TRACE_T0();
                         mbar_wait(&empty[stage], phase ^ 1u);
                         T2_TRACE_ADD(tr_empty);
                     }
                     if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2u * kT2StageBytes);
-                    const int rows = (int)t.nk * (int)t.rows8 * 8;
                     tma_load_2d_2cta(smem + map.ring + stage * kT2StageBytes, &wmap, &full[stage], 0,
-                                     (int32_t)t.src_row + (int32_t)rank * rows);
+                                     (int32_t)src_row + (int32_t)rank * rows);
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
@@ -913,6 +964,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         // warp-uniform); one elected lane issues the MMAs and commits. =====
         if (rank == 0) {
             uint32_t stage = 0, phase = 0;
+            uint32_t tl_n = 0;
+            (void)tl_n;
             int waited0 = -1, waited1 = -1;  // latest event waited for, per publishing set (T2Tile::need2)
             const uint32_t a_desc_lo = (uint32_t)umma_desc_sw128(a_u32), ring_desc_lo = (uint32_t)umma_desc_sw128(ring_u32);
             const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0u) >> 32);
@@ -923,65 +976,75 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
-                    const T2Tile t = T[i];
-                    const int need = base + (int)t.need, need2 = base + (int)t.need2;
-                    // events needed from set 0 and from set 1 (equal entries: one set only)
-                    const int n0 = t.need_set ? need2 : need, n1 = t.need_set ? need : need2;
+                    const uint4 r0 = *reinterpret_cast<const uint4 *>(T + i);
+                    const uint4 r1 = *(reinterpret_cast<const uint4 *>(T + i) + 1);
+#ifdef VOILA_T2_TRACE
+                    const bool tl_on = cluster_id == 0 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+#endif
+                    // events needed from epilogue set 0 and set 1 (-100000: nothing to wait for)
+                    const int n0 = base + (int)r1.x, n1 = base + (int)r1.y;
+                    T2_TL_ISSUER(tl_on, (7u << 24) | (uint32_t)i);
                     if (n0 > waited0) {
                         T2_TRACE_T0();
                         mbar_wait(&evt[n0 & (kT2EvtRing - 1)], (uint32_t)(n0 / kT2EvtRing) & 1u);
                         T2_TRACE_ADD(tr_evt);
                         waited0 = n0;
                     }
-                    if (need2 != need && n1 > waited1) {
+                    if (n1 > waited1) {
                         T2_TRACE_T0();
                         mbar_wait(&evt[n1 & (kT2EvtRing - 1)], (uint32_t)(n1 / kT2EvtRing) & 1u);
                         T2_TRACE_ADD(tr_evt);
                         waited1 = n1;
                     }
+                    T2_TL_ISSUER(tl_on, (8u << 24) | (uint32_t)i);
                     {
                         T2_TRACE_T0();
                         mbar_wait(&full[stage], phase);
                         T2_TRACE_ADD(tr_full);
                     }
+                    T2_TL_ISSUER(tl_on, (9u << 24) | (uint32_t)i);
                     tc_fence_after();
+                    T2_TL_ISSUER(tl_on, (1u << 24) | (uint32_t)i);
+                    const uint32_t misc = r1.w;
                     if (elect_one_sync()) {
-                    const uint32_t d = tmem_base + (uint32_t)t.d_col16 * 16u;
-                    const uint32_t chunk_b = (uint32_t)t.rows8 * 1024u;  // bytes of one K chunk in the stage
-                    uint32_t acc = (t.flags & 1u) ? 0u : 1u;
+                    const uint32_t d = tmem_base + r0.w;
+                    const uint32_t nk = misc & 15u;
+                    uint32_t acc = (misc & 16u) ? 0u : 1u;
 #ifdef VOILA_T2_TRACE
                     const long long tm0 = clock64();
 #endif
                     // descriptors differ only in their 14-bit address field (units of 16 bytes): add
                     // offsets to the low word instead of rebuilding them (the rebuilt form was ~100
                     // uniform-datapath instructions per tile)
-                    uint32_t a_lo = a_desc_lo + (uint32_t)t.kc0 * (kT2ChunkBytes >> 4);
+                    uint32_t a_lo = a_desc_lo + r0.z;
                     uint32_t b_lo = ring_desc_lo + stage * (kT2StageBytes >> 4);
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {  // a stage holds up to 4 K chunks
-                        if (c >= (int)t.nk) break;
+                        if (c >= (int)nk) break;
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {  // 64-wide chunk = 4 x (K = 16); +32 bytes per K step
                             umma_ss_2cta(d, ((uint64_t)desc_hi << 32) | (a_lo + 2u * k),
-                                         ((uint64_t)desc_hi << 32) | (b_lo + 2u * k), t.idesc, acc);
+                                         ((uint64_t)desc_hi << 32) | (b_lo + 2u * k), r0.y, acc);
                             acc = 1u;
                         }
                         a_lo += kT2ChunkBytes >> 4;
-                        b_lo += chunk_b >> 4;
+                        b_lo += r1.z;
                     }
 #ifdef VOILA_T2_TRACE
                     const long long tm1 = clock64();
                     tr_mma += tm1 - tm0;
 #endif
                     umma_commit_2cta(&empty[stage], 3);
-                    if (t.flags & 4u) umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
-                    if (t.flags & 2u) umma_commit_2cta(&layer_done[(blk_base + (int)t.blk) & (kT2AccRing - 1)], 3);
+                    if (misc & 64u) umma_commit_2cta(&cfree[free_seq & (kT2FreeRing - 1)], 3);
+                    if (misc & 32u)
+                        umma_commit_2cta(&layer_done[((uint32_t)blk_base + ((misc >> 8) & 255u)) & (kT2AccRing - 1)], 3);
 #ifdef VOILA_T2_TRACE
                     tr_commit += clock64() - tm1;
 #endif
                     }
                     __syncwarp();
-                    if (t.flags & 4u) ++free_seq;
+                    T2_TL_ISSUER(tl_on, (2u << 24) | (uint32_t)i);
+                    free_seq += (misc >> 6) & 1u;
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
@@ -1080,7 +1143,11 @@ std::vector<int> hidden_blocks(int n, int policy) {
     int left = n;
     if (policy == 0 && n <= 256) policy = 2;  // a 256-wide layer as two 128 blocks: the epilogue of the
                                               // first overlaps the MMAs of the second (measured, CFG3)
-    if (policy == 0) {  // default: all 256 (N < 256 MMAs run below the tensor pipe's floor: A re-read)
+    if (policy == 4 && n > 256) {  // 256s, then the last 256 columns as two 128 blocks (short last epilogue)
+        while (left > 256) { b.push_back(256); left -= 256; }
+        while (left >= 128) { b.push_back(128); left -= 128; }
+    }
+    if (policy == 0 || policy == 3 || policy == 4) {  // all 256 (N < 256 MMAs run below the tensor pipe's floor: A re-read)
         while (left >= 256) { b.push_back(256); left -= 256; }
     } else if (policy == 2) {  // all 128
         while (left >= 128) { b.push_back(128); left -= 128; }
@@ -1379,6 +1446,23 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     while (g.hdr.n_stages > 2 && smem2_map(g.hdr).total + 1024 > kMaxDynSmem2) --g.hdr.n_stages;
     g.smem_bytes = smem2_map(g.hdr).total + 1024;
     if (g.smem_bytes > kMaxDynSmem2) return "model does not fit the shared-memory budget of the tcgen05 pair kernel";
+    // device form of the tile records (see T2TileDev)
+    std::vector<T2TileDev> dev_tiles;
+    for (const T2Tile &t : pb.tiles) {
+        T2TileDev d{};
+        d.src_row = t.src_row;
+        d.idesc = t.idesc;
+        d.a_off = (uint32_t)t.kc0 * (uint32_t)(kT2ChunkBytes >> 4);
+        d.d_off = (uint32_t)t.d_col16 * 16u;
+        const int need = t.need, need2 = t.need2;
+        const int s0 = t.need_set ? need2 : need, s1 = t.need_set ? need : need2;
+        d.need_s0 = s0;
+        d.need_s1 = need2 != need ? s1 : -100000;
+        d.chunk_b16 = ((uint32_t)t.rows8 * 1024u) >> 4;
+        d.misc = (uint32_t)t.nk | ((uint32_t)(t.flags & 7u) << 4) | ((uint32_t)t.blk << 8) |
+                 ((uint32_t)((int)t.nk * (int)t.rows8 * 8) << 16);
+        dev_tiles.push_back(d);
+    }
     auto upload = [&](const void *src, size_t bytes, void **dst) -> bool {
         if (cudaMalloc(dst, bytes) != cudaSuccess) return false;
         allocs->push_back(*dst);
@@ -1388,7 +1472,7 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         !upload(pb.bias.data(), pb.bias.size() * sizeof(float), &g.d_bias) ||
         !upload(pb.sbias_init.data(), pb.sbias_init.size() * sizeof(float), &g.d_sbias) ||
         !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &g.d_layers) ||
-        !upload(pb.tiles.data(), pb.tiles.size() * sizeof(T2Tile), &g.d_tiles) ||
+        !upload(dev_tiles.data(), dev_tiles.size() * sizeof(T2TileDev), &g.d_tiles) ||
         cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem_bytes) != cudaSuccess)
         return cudaGetErrorString(cudaGetLastError());
     // weight stream as a 2-D tensor [rows][64 bf16]; box = one ring stage (128 rows x 128 bytes).
@@ -1519,7 +1603,7 @@ T2Params base_params(const T2Program &g, const ModelDev &m) {
     p.bias = reinterpret_cast<const float *>(g.d_bias);
     p.sbias_init = reinterpret_cast<const float *>(g.d_sbias);
     p.layers = reinterpret_cast<const T2Layer *>(g.d_layers);
-    p.tiles = reinterpret_cast<const T2Tile *>(g.d_tiles);
+    p.tiles = reinterpret_cast<const T2TileDev *>(g.d_tiles);
     p.hdr = g.hdr;
     p.S = m.S; p.O = m.O; p.A = m.A; p.Nz = m.Nz;
     p.gamma = m.gamma;
@@ -1595,5 +1679,22 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
 #ifdef VOILA_T2_TRACE
 extern "C" __attribute__((visibility("default"))) int voila_debug_t2_trace(unsigned long long *out64) {
     return (int)cudaMemcpyFromSymbol(out64, voila::g_t2_trace, sizeof(unsigned long long) * 64);
+}
+// Timeline: sets the recorded step window and clears the buffer / reads it back (returns the count).
+extern "C" __attribute__((visibility("default"))) int voila_debug_t2_timeline_arm(int step0, int step1) {
+    const int win[2] = {step0, step1};
+    const unsigned zero = 0;
+    cudaMemcpyToSymbol(voila::g_t2_tl_win, win, sizeof(win));
+    void *p = nullptr;
+    cudaGetSymbolAddress(&p, voila::g_t2_tl);
+    cudaMemset(p, 0, sizeof(unsigned long long) * 2 * voila::kT2TlCap);
+    return (int)cudaMemcpyToSymbol(voila::g_t2_tl_n, &zero, sizeof(zero));
+}
+extern "C" __attribute__((visibility("default"))) int voila_debug_t2_timeline_read(unsigned long long *out, int cap_pairs) {
+    // regions are zero-filled by arm(); unused entries stay (0, 0)
+    unsigned n = voila::kT2TlCap;
+    if ((int)n > cap_pairs) n = (unsigned)cap_pairs;
+    cudaMemcpyFromSymbol(out, voila::g_t2_tl, sizeof(unsigned long long) * 2 * n);
+    return (int)n;
 }
 #endif

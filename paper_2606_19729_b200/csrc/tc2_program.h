@@ -90,6 +90,22 @@ struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block 
 };
 static_assert(sizeof(T2Tile) == 20, "T2Tile is copied to shared memory as 32-bit words");
 
+// The tile record as the device reads it (32 bytes = two 16-byte shared-memory loads, every field
+// a ready-to-use 32-bit word: the MMA issuer's loop is a dependent chain that shares its scheduler
+// with four epilogue warps, and ncu showed a quarter of its time in the byte / halfword loads and
+// unpacking of the 20-byte host record).
+struct T2TileDev {
+    uint32_t src_row;   // producer: first 128-byte row of the tile in the weight stream
+    uint32_t idesc;     // tcgen05 instruction descriptor
+    uint32_t a_off;     // operand descriptor offset of the first K chunk (16-byte units)
+    uint32_t d_off;     // accumulator column offset in TMEM
+    int32_t need_s0;    // event of epilogue set 0 to wait for (relative to the step), -100000: none
+    int32_t need_s1;    // event of epilogue set 1 to wait for, -100000: none
+    uint32_t chunk_b16; // weight bytes of one K chunk in the stage / 16 (descriptor units)
+    uint32_t misc;      // nk | flags << 4 | blk << 8 | rows << 16   (rows = weight rows per CTA in the stage)
+};
+static_assert(sizeof(T2TileDev) == 32, "T2TileDev is read with two 16-byte loads");
+
 struct T2Header {
     int n_layers, n_tiles, evt_per_step, a_chunks;
     int tmem_cols, n_stages, in_chunks, blocks_per_step;  // accumulator blocks (hand-offs) per step
