@@ -53,6 +53,7 @@
 typedef VO_REAL real;
 
 #define VO_MAX_LAYERS 8
+#define VO_MAX_TERM 8
 #define VO_ACT_NONE 0
 #define VO_ACT_RELU 1
 #define VO_ACT_SILU 2
@@ -83,6 +84,12 @@ typedef struct {
     real *reward_param; /* goal[S] | M[S][S] | c[S+1] */
     real *action_cost;  /* [A] or NULL */
     int emulate_bf16;   /* debugging hook, see vo_model_set_emulate_bf16 */
+    /* terminal regions, see vo_model_set_terminal */
+    int n_term;
+    int term_dim[VO_MAX_TERM];
+    float *term_center[VO_MAX_TERM];
+    float term_radius[VO_MAX_TERM], term_reward[VO_MAX_TERM];
+    int term_stop[VO_MAX_TERM];
 } vo_model;
 
 /* ------------------------------------------------------------------------------------------
@@ -205,6 +212,36 @@ int vo_model_set_reward(vo_model *m, int kind, const float *param, const float *
     return 0;
 }
 
+/* Terminal regions.  The paper's three domains pay terminal rewards and end the
+ * episode when the state reaches a region of the state space: FloorPositioning +100 at the correct
+ * goal (terminates) and -100 at the incorrect goal (does not), -1 per non-terminal action
+ * (PAPER.md:161); LeggedNavigation +500 in a goal disc of radius 2 m, -500 on collision, both
+ * terminate; TargetFinding +100 / -500.  Reading (R25):
+ * region k is a ball over the LEADING dim_k state coordinates, || s[0:dim_k] - c_k ||_2 <= r_k;
+ * at a step t that is still alive, every region containing s_t pays reward_k; if one of them has
+ * stop_k the episode ends there: the step reward R(s_t, a_t) (incl. the action cost) is NOT paid,
+ * the state is frozen, nothing accrues afterwards; otherwise R(s_t, a_t) is paid as usual.
+ * Membership is decided in fp32: d2 = fma chain over j = 0..dim_k-1 of (s_j - c_j)^2, inside iff
+ * d2 <= r_k * r_k (both sides take the decision in this precision and order). */
+int vo_model_set_terminal(vo_model *m, int n, const int *dims, const float *centers, const float *radii,
+                          const float *rewards, const int *stops) {
+    if (n < 0 || n > VO_MAX_TERM) return -1;
+    for (int k = 0; k < VO_MAX_TERM; ++k) { free(m->term_center[k]); m->term_center[k] = NULL; }
+    m->n_term = n;
+    size_t off = 0;
+    for (int k = 0; k < n; ++k) {
+        if (dims[k] < 1 || dims[k] > m->S) return -1;
+        m->term_dim[k] = dims[k];
+        m->term_center[k] = (float *)malloc(sizeof(float) * (size_t)dims[k]);
+        for (int j = 0; j < dims[k]; ++j) m->term_center[k][j] = centers[off + j];
+        off += (size_t)dims[k];
+        m->term_radius[k] = radii[k];
+        m->term_reward[k] = rewards[k];
+        m->term_stop[k] = stops[k] ? 1 : 0;
+    }
+    return 0;
+}
+
 /* bf16-emulation hook: when on, weights (already stored) are rounded once to bf16 and every
  * layer's INPUT vector is rounded to bf16 before the affine map; accumulation, bias, activation
  * stay in `real`.  Call after all vo_model_set_mlp calls.  Not part of the oracle proper. */
@@ -222,6 +259,7 @@ void vo_model_destroy(vo_model *m) {
     if (!m) return;
     for (int w = 0; w < 4; ++w)
         for (int l = 0; l < VO_MAX_LAYERS; ++l) { free(m->mlp[w].W[l]); free(m->mlp[w].b[l]); }
+    for (int k = 0; k < VO_MAX_TERM; ++k) free(m->term_center[k]);
     free(m->reward_param); free(m->action_cost); free(m);
 }
 
@@ -316,6 +354,34 @@ static real reward(const vo_model *m, const real *s, int a) {
     return r;
 }
 
+/* One alive step's reward with the terminal regions (see vo_model_set_terminal): returns the reward
+ * paid at this step and sets *stop when the episode ends here.  *margin (optional) is lowered to the
+ * smallest | ||s - c_k|| - r_k | seen: how close the membership decisions were to flipping. */
+static real step_reward_term(const vo_model *m, const real *s, int a, int *stop, float *margin) {
+    real bonus = 0;
+    *stop = 0;
+    for (int k = 0; k < m->n_term; ++k) {
+        float d2 = 0.0f;
+        for (int j = 0; j < m->term_dim[k]; ++j) {
+            float sj = (float)s[j];
+            if (m->emulate_bf16) sj = bf16_round(sj); /* bf16 mode stores particle states in bf16 (R18) */
+            const float d = sj - m->term_center[k][j];
+            d2 = fmaf(d, d, d2);
+        }
+        const float r = m->term_radius[k];
+        if (margin) {
+            const float mg = fabsf(sqrtf(d2) - r);
+            if (mg < *margin) *margin = mg;
+        }
+        if (d2 <= r * r) {
+            bonus += (real)m->term_reward[k];
+            if (m->term_stop[k]) *stop = 1;
+        }
+    }
+    if (*stop) return bonus;
+    return bonus + reward(m, s, a);
+}
+
 typedef struct { real *x, *b0, *b1, *s, *sn, *o; float *omega; } scratch;
 
 static scratch scratch_alloc(const vo_model *m) {
@@ -350,9 +416,19 @@ double vo_rollout_trajectory(const vo_model *m, const float *s0, const int32_t *
     for (int i = 0; i < S; ++i) z.s[i] = (real)s0[i];
     real G = 0, disc = 1;
     for (int i = 0; i < S; ++i) if (states_out) states_out[i] = (float)z.s[i];
+    int alive = 1;
     for (int t = 0; t < H; ++t) {
         int a = actions[t];
-        G += disc * reward(m, z.s, a);
+        if (alive) {
+            int stop = 0;
+            G += disc * step_reward_term(m, z.s, a, &stop, NULL);
+            if (stop) alive = 0;
+        }
+        if (!alive) { /* terminated: the state stays frozen, no observation, nothing accrues */
+            if (states_out) for (int i = 0; i < S; ++i) states_out[(size_t)(t + 1) * S + i] = (float)z.s[i];
+            if (obs_out) for (int i = 0; i < O; ++i) obs_out[(size_t)t * O + i] = 0.0f;
+            continue;
+        }
         gen_step(m, 0, z.s, a, seed, p, q, (uint32_t)t, VO_STREAM_ROLLOUT_T, &z, z.sn);
         gen_step(m, 1, z.sn, a, seed, p, q, (uint32_t)t, VO_STREAM_ROLLOUT_Z, &z, z.o);
         disc *= (real)m->gamma;
@@ -370,9 +446,25 @@ double vo_rollout_trajectory(const vo_model *m, const float *s0, const int32_t *
  * values_out [Q]; witness_out [Q][O] or NULL (reading R10); returns_out [Q][P] or NULL
  * (per-(p,q) discounted returns, for pins).
  * ---------------------------------------------------------------------------------------- */
+int vo_rollout_values_term(const vo_model *m, const float *particles, int P, const int32_t *action_seqs,
+                           int Q, int H, const float *weights, uint64_t seed, int q_offset,
+                           float *values_out, float *witness_out, float *returns_out,
+                           float *final_states_out, int32_t *t_term_out, float *margin_out);
+
 int vo_rollout_values(const vo_model *m, const float *particles, int P, const int32_t *action_seqs,
                       int Q, int H, const float *weights, uint64_t seed, int q_offset,
                       float *values_out, float *witness_out, float *returns_out) {
+    return vo_rollout_values_term(m, particles, P, action_seqs, Q, H, weights, seed, q_offset, values_out,
+                                  witness_out, returns_out, NULL, NULL, NULL);
+}
+
+/* The same with the per-trajectory detail the termination tests need: final_states_out [Q][P][S]
+ * (s_H, or the frozen state of a terminated trajectory), t_term_out [Q][P] (step at which the
+ * episode ended, H if it did not), margin_out [Q][P] (see step_reward_term).  Any may be NULL. */
+int vo_rollout_values_term(const vo_model *m, const float *particles, int P, const int32_t *action_seqs,
+                           int Q, int H, const float *weights, uint64_t seed, int q_offset,
+                           float *values_out, float *witness_out, float *returns_out,
+                           float *final_states_out, int32_t *t_term_out, float *margin_out) {
     int S = m->S, O = m->O;
     double wsum = 0;
     for (int p = 0; p < P; ++p) wsum += weights ? (double)weights[p] : 1.0;
@@ -388,9 +480,14 @@ int vo_rollout_values(const vo_model *m, const float *particles, int P, const in
             for (int i = 0; i < S; ++i) z.s[i] = (real)particles[(size_t)p * S + i];
             for (int i = 0; i < O; ++i) wit[i] = 0;
             real G = 0, disc = 1;
+            int t_term = H;
+            float margin = INFINITY;
             for (int t = 0; t < H; ++t) {
                 int a = action_seqs[(size_t)q * H + t];
-                G += disc * reward(m, z.s, a); /* reward on CURRENT state, gamma^t, t from 0 */
+                int stop = 0;
+                /* reward on CURRENT state, gamma^t, t from 0; terminal regions: vo_model_set_terminal */
+                G += disc * step_reward_term(m, z.s, a, &stop, &margin);
+                if (stop) { t_term = t; break; } /* state frozen, nothing accrues afterwards */
                 gen_step(m, 0, z.s, a, seed, (uint32_t)p, (uint32_t)(q + q_offset), (uint32_t)t,
                          VO_STREAM_ROLLOUT_T, &z, z.sn);
                 gen_step(m, 1, z.sn, a, seed, (uint32_t)p, (uint32_t)(q + q_offset), (uint32_t)t,
@@ -402,6 +499,10 @@ int vo_rollout_values(const vo_model *m, const float *particles, int P, const in
             V += wbar * (double)G;
             for (int i = 0; i < O; ++i) Wit[i] += wbar * (double)wit[i];
             if (returns_out) returns_out[(size_t)q * P + p] = (float)G;
+            if (final_states_out)
+                for (int i = 0; i < S; ++i) final_states_out[((size_t)q * P + p) * S + i] = (float)z.s[i];
+            if (t_term_out) t_term_out[(size_t)q * P + p] = t_term;
+            if (margin_out) margin_out[(size_t)q * P + p] = margin;
         }
         values_out[q] = (float)V;
         if (witness_out) for (int i = 0; i < O; ++i) witness_out[(size_t)q * O + i] = (float)Wit[i];

@@ -54,6 +54,10 @@ def _lib(real: str = "f32"):
     lib.vo_rollout_trajectory.restype = f64
     lib.vo_rollout_values.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, i32, vp, vp, vp]
     lib.vo_rollout_values.restype = i32
+    lib.vo_rollout_values_term.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, i32, vp, vp, vp, vp, vp, vp]
+    lib.vo_rollout_values_term.restype = i32
+    lib.vo_model_set_terminal.argtypes = [vp, i32, vp, vp, vp, vp, vp]
+    lib.vo_model_set_terminal.restype = i32
     lib.vo_resample_systematic_x0.argtypes = [vp, i32, u32, vp]
     lib.vo_resample_systematic_x0.restype = i32
     lib.vo_resample_systematic.argtypes = [vp, i32, u64, vp]
@@ -159,6 +163,14 @@ class OracleModel:
         assert rc == 0
         if emulate_bf16:
             self.lib.vo_model_set_emulate_bf16(self.h, 1)
+        term = getattr(model, "terminal", None)
+        if term is not None and len(term.radii):
+            dims = np.asarray([len(c) for c in term.centers], dtype=np.int32)
+            cen = np.concatenate([np.asarray(c, np.float32).ravel() for c in term.centers])
+            rc = self.lib.vo_model_set_terminal(self.h, len(dims), _p(dims), _p(cen),
+                                                _p(_f32(term.radii)), _p(_f32(term.rewards)),
+                                                _p(np.asarray(term.stops, dtype=np.int32)))
+            assert rc == 0
 
     def __del__(self):
         try:
@@ -202,6 +214,25 @@ class OracleModel:
         if want_returns:
             return values, witness, returns
         return values, witness
+
+    def rollout_values_term(self, particles, action_seqs, weights, seed, q_offset=0):
+        """Rollout with the per-trajectory detail of the termination tests: dict with values [Q],
+        witness [Q][O], returns [Q][P], final_states [Q][P][S], t_term [Q][P] (H = never),
+        margin [Q][P] (closest any membership decision came to its boundary)."""
+        particles = _f32(particles)
+        action_seqs = np.ascontiguousarray(action_seqs, dtype=np.int32)
+        weights = _f32(weights)
+        P, (Q, H) = particles.shape[0], action_seqs.shape
+        out = {"values": np.zeros(Q, np.float32), "witness": np.zeros((Q, self.O), np.float32),
+               "returns": np.zeros((Q, P), np.float32), "final_states": np.zeros((Q, P, self.S), np.float32),
+               "t_term": np.zeros((Q, P), np.int32), "margin": np.zeros((Q, P), np.float32)}
+        rc = self.lib.vo_rollout_values_term(self.h, _p(particles), P, _p(action_seqs), Q, H, _p(weights),
+                                             int(seed), int(q_offset), _p(out["values"]), _p(out["witness"]),
+                                             _p(out["returns"]), _p(out["final_states"]), _p(out["t_term"]),
+                                             _p(out["margin"]))
+        if rc != 0:
+            raise RuntimeError(f"vo_rollout_values_term -> {rc}")
+        return out
 
     def belief_update(self, particles, action, observation, weights, seed, ess_threshold=None):
         """ess_threshold=None: the plain SIR update (always resample); a float: adaptive resampling

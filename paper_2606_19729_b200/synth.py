@@ -42,6 +42,16 @@ class MLPSpec:
 
 
 @dataclass
+class TerminalSpec:
+    """Terminal regions (R25): ball k over the leading len(centers[k]) state coordinates,
+    radius radii[k]; pays rewards[k] when an alive state is inside; stops[k] = 1 ends the episode."""
+    centers: List[np.ndarray]
+    radii: np.ndarray
+    rewards: np.ndarray
+    stops: np.ndarray
+
+
+@dataclass
 class ModelSpec:
     S: int
     O: int
@@ -58,6 +68,7 @@ class ModelSpec:
     reward_param: np.ndarray = None
     action_cost: Optional[np.ndarray] = None
     prec: int = PREC_FP32
+    terminal: Optional[TerminalSpec] = None
 
     def mlps(self):
         return [self.f_T, self.f_Z, self.lik_obs, self.lik_state]
