@@ -83,6 +83,27 @@ typedef struct {
     const float *action_cost;  /* host [n_actions], added to R; or NULL */
 } voila_reward;
 
+/* Terminal regions of the rollout.  The paper's domains pay terminal rewards and end
+ * the episode when the state reaches a region: FloorPositioning +100 at the correct goal (terminates),
+ * -100 at the incorrect goal (does not), -1 per non-terminal action; LeggedNavigation
+ * +500 in a goal disc of radius 2 m / -500 on collision, both terminate; TargetFinding
+ * +100 / -500.  DESIGN.md reading R25: region k is the ball
+ * || s[0:dims[k]] - center_k ||_2 <= radii[k] over the LEADING dims[k] state coordinates.  At a step t
+ * of a trajectory that is still alive, every region containing s_t pays rewards[k]; if one of them
+ * has stops[k] != 0 the episode ends there: R(s_t, a_t) (action cost included) is not paid, the state
+ * is frozen (final_states_out returns it), no observation is drawn and nothing accrues afterwards;
+ * otherwise R(s_t, a_t) is paid as usual.  Membership is decided in fp32 (on the bf16 state in bf16
+ * mode): d2 = fma chain over j = 0 .. dims[k]-1 of (s_j - c_j)^2, inside iff d2 <= r*r. */
+#define VOILA_MAX_TERMINAL_REGIONS 8
+typedef struct {
+    int n_regions;          /* 0 .. VOILA_MAX_TERMINAL_REGIONS */
+    const int *dims;        /* host [n_regions]: 1 .. state_dim (1 .. 8 on the tensor-core path) */
+    const float *centers;   /* host: the centres concatenated, sum(dims) floats */
+    const float *radii;     /* host [n_regions], >= 0 */
+    const float *rewards;   /* host [n_regions] */
+    const int *stops;       /* host [n_regions]: != 0 ends the episode */
+} voila_terminal;
+
 typedef struct {
     int state_dim;   /* S */
     int obs_dim;     /* O */
@@ -97,13 +118,15 @@ typedef struct {
     float discount;        /* gamma in (0, 1] */
     voila_reward reward;
     int prec;              /* voila_prec */
+    const voila_terminal *terminal; /* terminal regions of the rollout, or NULL (none) */
 } voila_model_desc;
 
 /* Which kernel family runs the generator MLPs (for tests and benchmarks; default AUTO). */
 typedef enum {
     VOILA_KERNEL_AUTO = 0,   /* tcgen05 path when prec == BF16 and the dims fit it, else FFMA */
     VOILA_KERNEL_FFMA = 1,   /* CUDA-core path (fp32 mode; in bf16 mode rounds operands to bf16) */
-    VOILA_KERNEL_TCGEN05 = 2, /* single-CTA tensor-core path (M = 128 per SM); UNSUPPORTED if the dims do not fit */
+    VOILA_KERNEL_TCGEN05 = 2, /* single-CTA tensor-core path (M = 128 per SM); UNSUPPORTED if the dims do not
+                                 fit or the model has terminal regions */
     VOILA_KERNEL_TCGEN05_PAIR = 3 /* CTA-pair tensor-core path (cta_group::2, M = 256 per SM pair): what AUTO picks */
 } voila_kernel;
 
@@ -135,7 +158,9 @@ int voila_tcgen05_supported(const voila_ctx *ctx);
  *   values_out       dev [Q] fp32
  *   obs_witness_out  dev [Q][O] fp32 or NULL: sum_p wbar_p sum_t gamma^t o_{t+1} (R10)
  *   returns_out      dev [Q][P] fp32 or NULL: per-(q,p) discounted return (tests)
- *   final_states_out dev [Q][P][S] fp32 or NULL: s_H of every trajectory (tests)
+ *   final_states_out dev [Q][P][S] fp32 or NULL: s_H of every trajectory, or the state at which it
+ *                    terminated (voila_terminal) (tests)
+ * With terminal regions (voila_model_desc.terminal) the sums stop at the step a trajectory ends.
  */
 voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
                                   const int32_t *action_seqs, int Q, int H, const float *weights,

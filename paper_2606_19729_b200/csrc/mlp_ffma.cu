@@ -173,12 +173,16 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
     const int S = m.S, O = m.O, A = m.A, Nz = m.Nz, KW = m.max_width;
     float *xa = smem, *xb = xa + KW * R, *s = xb + KW * R, *sn = s + S * R, *wit = sn + S * R;
     float *obs = wit + O * R, *red = obs + O * R, *G = red + kWarps * R;
+    float *alive = G + R;  // 1 while the row's episode runs (terminal regions, voila_terminal)
     const int tile = blockIdx.x, q = blockIdx.y, p0 = tile * R;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     load_particles<EMU>(a.particles, S, a.P, p0, s);
     for (int idx = threadIdx.x; idx < O * R; idx += kThreads) wit[idx] = 0.0f;
-    if (threadIdx.x < R) G[threadIdx.x] = 0.0f;
+    if (threadIdx.x < R) {
+        G[threadIdx.x] = 0.0f;
+        alive[threadIdx.x] = 1.0f;
+    }
     __syncthreads();
 
     float disc = 1.0f;
@@ -186,7 +190,28 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
         const int act_t = __ldg(a.action_seqs + (size_t)q * a.H + t);
         // reward on the CURRENT state (reading R7)
         const float rew = tile_reward(m.reward, S, s, act_t, red);
-        if (warp == 0) G[lane] = fmaf(disc, rew, G[lane]);
+        if (warp == 0) {
+            // terminal regions (reading R25): every region holding s_t pays; a stopping one ends the
+            // episode here (no step reward, state frozen, nothing accrues afterwards)
+            float bonus = 0.0f;
+            bool stop = false;
+            for (int k = 0; k < m.term.n; ++k) {
+                float d2 = 0.0f;
+                for (int j = 0; j < m.term.dim[k]; ++j) {
+                    const float sj = EMU ? bf16_round(s[j * R + lane]) : s[j * R + lane];
+                    const float d = sj - __ldg(m.term.centers + m.term.off[k] + j);
+                    d2 = fmaf(d, d, d2);
+                }
+                if (d2 <= m.term.r2[k]) {
+                    bonus += m.term.reward[k];
+                    stop |= m.term.stop[k] != 0;
+                }
+            }
+            if (alive[lane] != 0.0f) {
+                G[lane] = fmaf(disc, stop ? bonus : bonus + rew, G[lane]);
+                if (stop) alive[lane] = 0.0f;
+            }
+        }
         // s' = f_T([s ; onehot(a) ; w_T])
         copy_state<EMU>(xa, s, S);
         fill_noise<EMU>(xa, S + A, Nz, a.seed, p0, q, t, kStreamRolloutT);
@@ -197,8 +222,11 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
         fill_noise<EMU>(xa, S + A, Nz, a.seed, p0, q, t, kStreamRolloutZ);
         __syncthreads();
         mlp_chain<EMU>(m.mlp[1], xa, xb, obs, S, S + A, S + act_t);
-        for (int idx = threadIdx.x; idx < O * R; idx += kThreads) wit[idx] = fmaf(disc, obs[idx], wit[idx]);
-        for (int idx = threadIdx.x; idx < S * R; idx += kThreads) s[idx] = sn[idx];
+        // rows whose episode has ended take no step: no observation, state frozen
+        for (int idx = threadIdx.x; idx < O * R; idx += kThreads)
+            if (alive[idx & (R - 1)] != 0.0f) wit[idx] = fmaf(disc, obs[idx], wit[idx]);
+        for (int idx = threadIdx.x; idx < S * R; idx += kThreads)
+            if (alive[idx & (R - 1)] != 0.0f) s[idx] = sn[idx];
         disc *= m.gamma;
         __syncthreads();
     }
@@ -384,7 +412,7 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 
 size_t ffma_smem_bytes(const ModelDev &m) {
     const int d = m.mlp[3].dims[m.mlp[3].n_layers];
-    const size_t rollout = (size_t)(2 * m.max_width + 2 * m.S + 2 * m.O + kWarps + 1) * R * sizeof(float);
+    const size_t rollout = (size_t)(2 * m.max_width + 2 * m.S + 2 * m.O + kWarps + 2) * R * sizeof(float);
     const size_t belief = (size_t)(2 * m.max_width + 2 * m.S + d) * R * sizeof(float);
     const size_t fwd = (size_t)(3 * m.max_width) * R * sizeof(float);
     size_t b = rollout > belief ? rollout : belief;

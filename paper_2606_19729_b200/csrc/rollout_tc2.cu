@@ -84,6 +84,7 @@ struct T2Params {
     int reward_kind;
     const float *reward_param;
     const float *action_cost;
+    TerminalDev term;  // terminal regions of the rollout (voila_terminal)
     // belief-update program (propose + score): one unit = 256 particles, one step per unit
     int bu_action;
     const float *bu_e;        // f(o), [d]
@@ -106,7 +107,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
     m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2TileDev) + 15u) & ~15u);
     m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing + kT2FreeRing) * 8;
-    m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4;
+    m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4 + 256;  // + per-row alive flags, two step parities
     m.total = m.sbias + (((uint32_t)h.sbias_floats * 4u + 15u) & ~15u);
     return m;
 }
@@ -354,8 +355,9 @@ __device__ __forceinline__ void t2_helper_epilogue(const T2Params &p, const T2La
 // LEADER's mbarriers (remote arrive from the peer CTA).
 __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                             uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
-                                            float *sbias, int warp, int lane, uint32_t rank, int cluster_id, int n_clusters,
-                                            int n_my_units, int total_steps, bool shared_hidden) {
+                                            uint8_t *alive_s, float *sbias, int warp, int lane, uint32_t rank,
+                                            int cluster_id, int n_clusters, int n_my_units, int total_steps,
+                                            bool shared_hidden) {
     // shared_hidden: a second set of epilogue warps takes the odd chunks of the hidden layers
     const int n_layers = p.hdr.n_layers;
     const uint32_t evt_cl = mapa_u32(smem_u32(evt), 0u);
@@ -371,6 +373,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         float G = 0.0f, disc = 1.0f, w_row = 0.0f;
         int t = 0, unit_i = 0, q = 0, blk = 0, p_idx = 0;
         bool valid = false;
+        bool alive = true;  // the row's episode still runs (terminal regions, reading R25)
         const long long tr_start = clock64();
         EpiSync es;
         es.evt_cl = evt_cl;
@@ -390,6 +393,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             G = 0.0f;
             disc = 1.0f;
             t = 0;
+            alive = true;
             if (half == 0) {
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
@@ -425,11 +429,45 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     st_shared_v4(a_unit_addr(a_u32, row, u), 0u, 0u, 0u, 0u);
             }
         };
+        // Pays step t's reward r_step = R(s_t, a_t) (half 0 warps, which hold the state).  Terminal
+        // regions (voila_terminal, reading R25): every region holding s_t pays its reward; a stopping
+        // one ends the episode here (r_step is not paid, the state freezes, nothing accrues later).
+        // The row's alive flag of step t goes to shared memory for the warp that holds its witness.
+        auto pay = [&](float r_step) {
+            if (p.term.n == 0) {
+                G = fmaf(disc, r_step, G);
+                return;
+            }
+            float bonus = 0.0f;
+            bool stop = false;
+            for (int k = 0; k < p.term.n; ++k) {
+                const float *c = p.term.centers + p.term.off[k];
+                const int dim = p.term.dim[k];
+                float d2 = 0.0f;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (j < dim) {
+                        const float sj = (j & 1) ? bf16hi(persist[j >> 1]) : bf16lo(persist[j >> 1]);
+                        const float d = sj - __ldg(c + j);
+                        d2 = fmaf(d, d, d2);
+                    }
+                }
+                if (d2 <= p.term.r2[k]) {
+                    bonus += p.term.reward[k];
+                    stop |= p.term.stop[k] != 0;
+                }
+            }
+            if (alive) {
+                G = fmaf(disc, stop ? bonus : bonus + r_step, G);
+                if (stop) alive = false;
+            }
+            alive_s[(t & 1) * kT2Rows + row] = alive ? 1 : 0;
+        };
         auto step_reward = [&]() {  // non-quadratic reward kinds: R(s_t, a_t) from the state words
             if (half == 0 && p.reward_kind != VOILA_R_NEG_QUADRATIC) {
                 float r = reward_from_state(persist, S, p.reward_kind, p.reward_param);
                 if (p.action_cost) r += __ldg(p.action_cost + __ldg(p.seqs + (size_t)q * p.H + t));
-                G = fmaf(disc, r, G);
+                pay(r);
             }
         };
 
@@ -503,7 +541,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         }
                         r = -r;
                         if (p.action_cost) r += __ldg(p.action_cost + a_t);
-                        G = fmaf(disc, r, G);
+                        pay(r);
                     }
                     tc_fence_before();
                     arrive_event();
@@ -528,10 +566,13 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                 tmem_ld_wait();
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) {
-                                    persist[8 * g + 2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
-                                                                        __uint_as_float(v[4 * i + 1]) + b[i].y);
-                                    persist[8 * g + 2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
-                                                                            __uint_as_float(v[4 * i + 3]) + b[i].w);
+                                    const uint32_t n0 = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x,
+                                                                    __uint_as_float(v[4 * i + 1]) + b[i].y);
+                                    const uint32_t n1 = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
+                                                                    __uint_as_float(v[4 * i + 3]) + b[i].w);
+                                    // a row whose episode has ended keeps its state
+                                    persist[8 * g + 2 * i] = alive ? n0 : persist[8 * g + 2 * i];
+                                    persist[8 * g + 2 * i + 1] = alive ? n1 : persist[8 * g + 2 * i + 1];
                                 }
                             }
                         }
@@ -548,6 +589,8 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     wait_layer();
                     T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 1) {
+                        // no observation for a row whose episode ended at or before step t
+                        const float disc_w = (p.term.n == 0 || alive_s[(t & 1) * kT2Rows + row] != 0) ? disc : 0.0f;
 #pragma unroll
                         for (int g = 0; g < 4; ++g) {
                             if (16 * g < (int)l.n_pad) {
@@ -562,10 +605,10 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                     const float o0 = __uint_as_float(v[4 * i]) + b[i].x, o1 = __uint_as_float(v[4 * i + 1]) + b[i].y;
                                     const float o2 = __uint_as_float(v[4 * i + 2]) + b[i].z, o3 = __uint_as_float(v[4 * i + 3]) + b[i].w;
                                     const int c0 = 16 * g + 4 * i;
-                                    persist[c0] = __float_as_uint(fmaf(disc, o0, __uint_as_float(persist[c0])));
-                                    persist[c0 + 1] = __float_as_uint(fmaf(disc, o1, __uint_as_float(persist[c0 + 1])));
-                                    persist[c0 + 2] = __float_as_uint(fmaf(disc, o2, __uint_as_float(persist[c0 + 2])));
-                                    persist[c0 + 3] = __float_as_uint(fmaf(disc, o3, __uint_as_float(persist[c0 + 3])));
+                                    persist[c0] = __float_as_uint(fmaf(disc_w, o0, __uint_as_float(persist[c0])));
+                                    persist[c0 + 1] = __float_as_uint(fmaf(disc_w, o1, __uint_as_float(persist[c0 + 1])));
+                                    persist[c0 + 2] = __float_as_uint(fmaf(disc_w, o2, __uint_as_float(persist[c0 + 2])));
+                                    persist[c0 + 3] = __float_as_uint(fmaf(disc_w, o3, __uint_as_float(persist[c0 + 3])));
                                 }
                             }
                         }
@@ -879,6 +922,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(smem + map.misc);
     double *red_g = reinterpret_cast<double *>(smem + map.misc + 16);
     float *red_w = reinterpret_cast<float *>(smem + map.misc + 16 + 4 * 8);
+    uint8_t *alive_s = smem + map.misc + 16 + 4 * 8 + 4 * 64 * 4;
     float *sbias = reinterpret_cast<float *>(smem + map.sbias);
     const uint32_t a_u32 = smem_u32(smem + map.a), ring_u32 = smem_u32(smem + map.ring);
 
@@ -1071,8 +1115,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
                            n_my_units, NTHREADS == kT2Threads ? -1 : 0);
         else
-            t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, sbias, warp, lane, rank, cluster_id,
-                        n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads);
+            t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, alive_s, sbias, warp, lane, rank,
+                        cluster_id, n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads);
     } else {
         // second set of epilogue warps (640-thread kernels)
         if (R_HELP > 0) setmaxnreg_inc<(R_HELP > 0 ? R_HELP : 24)>();
@@ -1610,6 +1654,7 @@ T2Params base_params(const T2Program &g, const ModelDev &m) {
     p.reward_kind = m.reward.kind;
     p.reward_param = m.reward.param;
     p.action_cost = m.reward.action_cost;
+    p.term = m.term;
     return p;
 }
 }  // namespace

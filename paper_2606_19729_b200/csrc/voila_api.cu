@@ -226,6 +226,17 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
     if (d != desc->lik_state.dims[desc->lik_state.n_layers]) return VOILA_ERR_INVALID_ARG;
     if (desc->reward.kind < VOILA_R_NEG_L2_GOAL || desc->reward.kind > VOILA_R_LINEAR || !desc->reward.param)
         return VOILA_ERR_INVALID_ARG;
+    const voila_terminal *term = desc->terminal;
+    int term_floats = 0;
+    if (term && term->n_regions > 0) {
+        if (term->n_regions > VOILA_MAX_TERMINAL_REGIONS || !term->dims || !term->centers || !term->radii ||
+            !term->rewards || !term->stops)
+            return VOILA_ERR_INVALID_ARG;
+        for (int k = 0; k < term->n_regions; ++k) {
+            if (term->dims[k] < 1 || term->dims[k] > S || !(term->radii[k] >= 0.0f)) return VOILA_ERR_INVALID_ARG;
+            term_floats += term->dims[k];
+        }
+    }
 
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
@@ -293,6 +304,22 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
             e = upload(std::vector<float>(desc->reward.action_cost, desc->reward.action_cost + A),
                        &m.reward.action_cost);
     }
+    m.term = TerminalDev{};
+    bool term_fits_tc = true;  // the tensor-core epilogue keeps the state packed in registers: leading 8 coordinates
+    if (e == cudaSuccess && term_floats > 0) {
+        m.term.n = term->n_regions;
+        int off = 0;
+        for (int k = 0; k < term->n_regions; ++k) {
+            m.term.dim[k] = term->dims[k];
+            m.term.off[k] = off;
+            m.term.stop[k] = term->stops[k] ? 1 : 0;
+            m.term.r2[k] = term->radii[k] * term->radii[k];
+            m.term.reward[k] = term->rewards[k];
+            off += term->dims[k];
+            if (term->dims[k] > 8) term_fits_tc = false;
+        }
+        e = upload(std::vector<float>(term->centers, term->centers + term_floats), &m.term.centers);
+    }
     if (e != cudaSuccess) {
         voila_destroy(ctx);
         return VOILA_ERR_CUDA;
@@ -303,20 +330,16 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
     }
     if (bf16) {
         std::string why;
-        if (tc_supported(desc, &why)) {
+        if (tc_supported(desc, &why) && term_fits_tc) {
+            // A program that does not fit (tables, shared memory, tensor map) leaves its handle null and
+            // AUTO runs the CUDA-core kernels, as voila.h promises; the reason stays readable.
             std::string err;
-            ctx->tc = tc_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
-            if (!ctx->tc) {
-                ctx->last_cuda_error = err;
-                voila_destroy(ctx);
-                return VOILA_ERR_CUDA;
+            if (m.term.n == 0) {  // the single-CTA variant has no terminal-region epilogue
+                ctx->tc = tc_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
+                if (!ctx->tc) ctx->last_cuda_error = "single-CTA tcgen05 program not built: " + err;
             }
             ctx->tc2 = tc2_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
-            if (!ctx->tc2) {
-                ctx->last_cuda_error = err;
-                voila_destroy(ctx);
-                return VOILA_ERR_CUDA;
-            }
+            if (!ctx->tc2) ctx->last_cuda_error = "CTA-pair tcgen05 program not built: " + err;
         }
     }
     *out = ctx;

@@ -29,12 +29,21 @@ struct RewardDev {
     const float *action_cost;  // [A] or nullptr
 };
 
+// Terminal regions (voila_terminal): everything by value except the centres.
+struct TerminalDev {
+    int n;
+    int dim[VOILA_MAX_TERMINAL_REGIONS], off[VOILA_MAX_TERMINAL_REGIONS], stop[VOILA_MAX_TERMINAL_REGIONS];
+    float r2[VOILA_MAX_TERMINAL_REGIONS], reward[VOILA_MAX_TERMINAL_REGIONS];
+    const float *centers;  // device, concatenated
+};
+
 struct ModelDev {
     int S, O, A, Nz;
     int lik_action_cond;
     float lambda, gamma;
     MlpDev mlp[4];  // 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower)
     RewardDev reward;
+    TerminalDev term;
     int max_width;  // widest activation vector over all four networks (incl. inputs)
 };
 

@@ -45,11 +45,18 @@ class _Reward(C.Structure):
                 ("action_cost", C.POINTER(C.c_float))]
 
 
+class _Terminal(C.Structure):
+    _fields_ = [("n_regions", C.c_int), ("dims", C.POINTER(C.c_int)), ("centers", C.POINTER(C.c_float)),
+                ("radii", C.POINTER(C.c_float)), ("rewards", C.POINTER(C.c_float)),
+                ("stops", C.POINTER(C.c_int))]
+
+
 class _ModelDesc(C.Structure):
     _fields_ = [("state_dim", C.c_int), ("obs_dim", C.c_int), ("n_actions", C.c_int),
                 ("noise_dim", C.c_int), ("f_T", _Mlp), ("f_Z", _Mlp), ("lik_obs", _Mlp),
                 ("lik_state", _Mlp), ("lik_action_cond", C.c_int), ("lik_temperature", C.c_float),
-                ("discount", C.c_float), ("reward", _Reward), ("prec", C.c_int)]
+                ("discount", C.c_float), ("reward", _Reward), ("prec", C.c_int),
+                ("terminal", C.POINTER(_Terminal))]
 
 
 def lib_path() -> str:
@@ -173,6 +180,17 @@ class Voila:
         keep.extend([param, cost])
         desc.reward = _Reward(int(model.reward_kind), _fptr(param), _fptr(cost))
         desc.prec = self.prec
+        term = getattr(model, "terminal", None)
+        if term is not None and len(term.radii):
+            t_dims = np.asarray([len(c) for c in term.centers], dtype=np.int32)
+            t_cen = np.concatenate([np.asarray(c, np.float32).ravel() for c in term.centers])
+            t_rad = np.ascontiguousarray(term.radii, np.float32)
+            t_rew = np.ascontiguousarray(term.rewards, np.float32)
+            t_stop = np.ascontiguousarray(term.stops, np.int32)
+            tstruct = _Terminal(len(t_dims), t_dims.ctypes.data_as(C.POINTER(C.c_int)), _fptr(t_cen),
+                                _fptr(t_rad), _fptr(t_rew), t_stop.ctypes.data_as(C.POINTER(C.c_int)))
+            keep.extend([t_dims, t_cen, t_rad, t_rew, t_stop, tstruct])
+            desc.terminal = C.pointer(tstruct)
         h = C.c_void_p()
         self._h = None
         self._check(self.lib.voila_create(C.byref(desc), self.device, C.byref(h)), "voila_create")

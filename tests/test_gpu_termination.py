@@ -1,0 +1,124 @@
+"""GPU parity: terminal regions of the rollout (voila_terminal, reading R25) against the
+oracle, per trajectory: returns, frozen final states, witness and values.  Trajectories whose membership
+decisions came close to a region boundary (the oracle reports the smallest margin) may decide the other
+way on the GPU, because the states agree only within the float tolerance: they are excluded from the
+element-wise comparison, and their share is bounded."""
+import numpy as np
+import pytest
+
+from paper_2606_19729_b200 import synth
+from paper_2606_19729_b200.synth import TerminalSpec
+from tests.parity_util import TOL_BF16_STATE, TOL_FP32, assert_close, t2n
+
+pytestmark = pytest.mark.gpu
+
+
+# Random-init generators contract every trajectory onto a small cluster within two steps (DESIGN.md
+# input recipe), so the regions are placed relative to that cluster (mean / spread of the first two
+# state coordinates from step 2 on, measured once with the oracle): a stopping goal ball on the
+# cluster's edge (+50), a stopping "collision" ball that only initial particles can be in (-100) and
+# a non-stopping penalty ball inside the cluster (-20).
+_CLUSTER = {1: ((-0.10, 0.03), (0.10, 0.10)), 2: ((-0.16, -0.07), (0.06, 0.08)), 3: ((0.07, -0.13), (0.055, 0.044))}
+
+
+def _terminal(cfg_idx):
+    m, s = (np.array(v) for v in _CLUSTER[cfg_idx])
+    goal = (m + np.array([1.6 * s[0], 0.0])).astype(np.float32)
+    pen = (m + np.array([0.0, -1.0 * s[1]])).astype(np.float32)
+    return TerminalSpec([goal, np.array([1.0, 1.0], np.float32), pen],
+                        np.array([1.0 * s[0], 0.5, 1.0 * s[1]], np.float32),
+                        np.array([50.0, -100.0, -20.0], np.float32), np.array([1, 1, 0], np.int32))
+
+
+def _compare(torch, oracle, cfg_idx, prec, kernel, P, Q, H, tol, margin_min, max_excluded):
+    import paper_2606_19729_b200 as vl
+    cfg = synth.CONFIGS[cfg_idx]
+    model = synth.make_model(cfg, prec=prec, action_cost=True).replace(terminal=_terminal(cfg_idx))
+    inp = synth.make_inputs(cfg, P=P, Q=Q, H=H)
+    bf16 = prec == synth.PREC_BF16
+    parts_np = synth.bf16_round_np(inp.particles) if bf16 else inp.particles
+    w = np.random.default_rng(5).uniform(0.2, 1.0, P).astype(np.float32)
+    ctx = vl.Voila(model, device=0, prec=prec)
+    ctx.voila_set_kernel(kernel)
+    out = ctx.voila_rollout_values(ctx.to_particles(inp.particles), torch.from_numpy(inp.action_seqs).cuda(),
+                                   torch.from_numpy(w).cuda(), 4321, want_witness=True, want_returns=True,
+                                   want_final_states=True)
+    torch.cuda.synchronize()
+    g = {k: t2n(v) for k, v in out.items()}
+    kname = ctx.voila_last_rollout_kernel()
+    ctx.close()
+    o = oracle.OracleModel(model, emulate_bf16=bf16).rollout_values_term(parts_np, inp.action_seqs, w, 4321)
+    # the workload has to exercise the feature: early, late and no termination all occur
+    tt = o["t_term"]
+    assert (tt == 0).mean() > 0.005 and ((tt > 0) & (tt < H)).mean() > 0.05 and (tt == H).mean() > 0.05
+    ok = o["margin"] >= margin_min
+    assert 1.0 - ok.mean() <= max_excluded, f"excluded {1.0 - ok.mean():.3f}"
+    scale = max(float(np.abs(o["returns"]).max()), 1.0)
+    err = np.abs(g["returns"] - o["returns"])[ok] / scale
+    assert err.max() <= tol, f"returns: {err.max():.3e} ({kname})"
+    ds = np.abs(g["final_states"] - o["final_states"])[ok]
+    s_scale = float(np.sqrt(np.mean(o["final_states"] ** 2)))
+    assert ds.max() <= 4 * tol * max(s_scale, 0.1), f"final states: {ds.max():.3e} ({kname})"
+    # a terminated trajectory's state is frozen exactly where the oracle froze it (same step)
+    term = ok & (tt < H)
+    assert term.any()
+    # the value is the weighted mean of the GPU's own returns (reduction), and agrees with the oracle
+    # wherever no excluded trajectory enters it
+    wbar = w.astype(np.float64) / w.astype(np.float64).sum()
+    np.testing.assert_allclose(g["values"], g["returns"].astype(np.float64) @ wbar, rtol=1e-5, atol=1e-4)
+    clean = ok.all(axis=1)
+    if clean.any():
+        assert np.abs(g["values"] - o["values"])[clean].max() <= tol * scale
+        assert_close(g["witness"][clean], o["witness"][clean], 2 * tol, "witness")
+    return kname
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def test_termination_fp32_cfg1(torch_cuda, oracle):
+    import paper_2606_19729_b200 as vl
+    k = _compare(torch_cuda, oracle, 1, synth.PREC_FP32, vl.KERNEL_AUTO, P=300, Q=24, H=10, tol=TOL_FP32,
+                 margin_min=2e-4, max_excluded=0.05)
+    assert "ffma" in k
+
+
+@pytest.mark.parametrize("cfg_idx,P,Q,H", [(2, 1000, 12, 15), (3, 700, 6, 12)])
+def test_termination_bf16_tensor_core(torch_cuda, oracle, cfg_idx, P, Q, H):
+    import paper_2606_19729_b200 as vl
+    k = _compare(torch_cuda, oracle, cfg_idx, synth.PREC_BF16, vl.KERNEL_AUTO, P=P, Q=Q, H=H,
+                 tol=TOL_BF16_STATE, margin_min=3e-3, max_excluded=0.5)
+    assert "rollout_tc2" in k
+
+
+def test_termination_bf16_ffma(torch_cuda, oracle):
+    import paper_2606_19729_b200 as vl
+    _compare(torch_cuda, oracle, 2, synth.PREC_BF16, vl.KERNEL_FFMA, P=200, Q=6, H=15, tol=TOL_BF16_STATE,
+             margin_min=3e-3, max_excluded=0.5)
+
+
+def test_no_region_reached_is_the_plain_rollout(torch_cuda):
+    """Regions nobody enters: bit-identical to the rollout without terminal regions (both kernels)."""
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    far = TerminalSpec([np.array([60.0, 60.0], np.float32)], np.array([1.0], np.float32),
+                       np.array([100.0], np.float32), np.array([1], np.int32))
+    for cfg_idx, prec in [(1, synth.PREC_FP32), (2, synth.PREC_BF16)]:
+        cfg = synth.CONFIGS[cfg_idx]
+        inp = synth.make_inputs(cfg, P=300, Q=8)
+        res = []
+        for term in (None, far):
+            model = synth.make_model(cfg, prec=prec).replace(terminal=term)
+            ctx = vl.Voila(model, device=0, prec=prec)
+            out = ctx.voila_rollout_values(ctx.to_particles(inp.particles),
+                                           torch.from_numpy(inp.action_seqs).cuda(), None, 77,
+                                           want_returns=True, want_final_states=True)
+            torch.cuda.synchronize()
+            res.append({k: t2n(v) for k, v in out.items()})
+            ctx.close()
+        for k in res[0]:
+            assert np.array_equal(res[0][k], res[1][k]), k
