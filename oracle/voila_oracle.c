@@ -66,6 +66,8 @@ typedef VO_REAL real;
 #define VO_STREAM_ROLLOUT_Z 2u
 #define VO_STREAM_BELIEF_T 3u
 #define VO_STREAM_RESAMPLE 4u
+#define VO_STREAM_PW_OBS 5u    /* progressive widening: noise of the sampled observation o_i */
+#define VO_STREAM_PW_ATTACH 6u /* progressive widening: word that picks an existing branch */
 
 typedef struct {
     int n_layers;                 /* number of affine layers */
@@ -614,9 +616,14 @@ int vo_belief_update_ess(const vo_model *m, const float *particles, int N, int a
     }
     free(e);
     float mx = -INFINITY;
-    for (int i = 0; i < N; ++i) if (L[i] > mx) mx = L[i];
+    int has_nan = 0;
+    for (int i = 0; i < N; ++i) {
+        if (L[i] > mx) mx = L[i];
+        if (L[i] != L[i]) has_nan = 1;
+    }
     int status = 0;
-    if (!(mx > -INFINITY) || !(mx < INFINITY)) status = -2; /* all zero weights or NaN/inf */
+    /* reading R20: all weights zero, or ANY non-finite score (a NaN never wins a comparison) */
+    if (!(mx > -INFINITY) || !(mx < INFINITY) || has_nan) status = -2;
     double sv = 0, sw = 0;
     for (int i = 0; i < N; ++i) {
         v[i] = status ? 0.0f : expf(L[i] - mx);
@@ -652,6 +659,184 @@ int vo_belief_update(const vo_model *m, const float *particles, int N, int actio
     return vo_belief_update_ess(m, particles, N, action, observation, weights, seed, INFINITY, proposals_out,
                                 logits_out, post_weights_out, log_evidence_out, ancestors_out, particles_out,
                                 weights_out, NULL, NULL);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * f1. Vectorised progressive widening with batched likelihood (section 4.3;
+ * SURVEY 8f f1).  "Parallel simulations are grouped by their parent action nodes, after which the
+ * PW operations are performed for all action-node groups in parallel".
+ *
+ * Inputs: N simulations (particles [N][S]) grouped by parent action node: group g owns the
+ * simulations [group_off[g], group_off[g+1]) and has action group_action[g], visit count
+ * visit_count[g] = N(a), branch count branch_count[g] = |C(a)| and stored branch observations
+ * branch_obs[g][0 .. |C(a)|) (rows of O floats, M_max rows reserved per group).
+ * For every simulation i of group g, in index order (readings R26-R29 of DESIGN.md):
+ *   s'_i = f_T(s_i, a_g, w_T(i))                       (stream 3, counter (i,0,0), as the belief update)
+ *   o_i  = f_Z(s'_i, a_g, w_Z(i))                      (stream 5)
+ *   N(a) += 1;  if |C(a)| < min(M_max, T(N(a))) the simulation opens branch |C(a)| with the
+ *   observation o_i and is attached to it; otherwise it is attached to an existing branch picked
+ *   uniformly, b = (x_i * |C(a)|) >> 32 with x_i one Philox word (stream 6)
+ *   T(n) = ceil(k_o * n^alpha_o * (1 - 1e-9)) in fp64: the criterion |C(a)| < k_o N(a)^alpha_o with a
+ *   relative tolerance, so that exact powers do not depend on the last bit of pow().
+ * Then "the likelihood model is used to weight successor states according to the observation
+ * stored at the selected branch, followed by resampling": with e_{g,m} = f(obs_{g,m})
+ * (all branch observations go through the tower as one batch),
+ *   L_i = log w_i + <e_{g,b(i)}, g(s'_i)> / lambda,
+ * and every (action node, branch) pair that received simulations is one child belief: its members
+ * (in index order) are resampled among themselves with the exact-integer systematic resampler (O7),
+ * v = exp(L - max over the members), offset word = Philox word of (seed, stream 4, counter (g*M_max+m,0,0)).
+ * The r-th member receives the r-th draw: particles_out[i_r] = s'_{ancestor}, ancestors_out[i_r] = the
+ * ancestor's simulation index.  A child whose weights are all zero / not finite keeps its members
+ * (identity) and sets seg_status_out[g*M_max+m] = 1.
+ * Outputs (any may be NULL): proposals_out [N][S], obs_out [N][O], sim_branch_out [N], opened_out [N]
+ * (1 if the simulation opened its branch), logits_out [N], post_weights_out [N] (v_i),
+ * ancestors_out [N], particles_out [N][S], weights_out [N] (1 / members), seg_status_out [G*M_max].
+ * visit_count, branch_count and branch_obs are updated in place.  Returns 0 or -1 (bad arguments).
+ * ---------------------------------------------------------------------------------------- */
+static int pw_threshold(double k_o, double alpha_o, int n) {
+    const double x = k_o * pow((double)n, alpha_o) * (1.0 - 1e-9);
+    if (!(x < 2147483647.0)) return 2147483647;
+    const int t = (int)ceil(x);
+    return t < 0 ? 0 : t;
+}
+
+int vo_pw_update(const vo_model *m, const float *particles, int N, const int32_t *group_off, int G,
+                 const int32_t *group_action, int32_t *visit_count, int32_t *branch_count,
+                 float *branch_obs, int M_max, double k_o, double alpha_o, const float *weights,
+                 uint64_t seed, float *proposals_out, float *obs_out, int32_t *sim_branch_out,
+                 int32_t *opened_out, float *logits_out, float *post_weights_out, int32_t *ancestors_out,
+                 float *particles_out, float *weights_out, int32_t *seg_status_out) {
+    int S = m->S, O = m->O, A = m->A;
+    const vo_mlp *tf = &m->mlp[2], *tg = &m->mlp[3];
+    int d = tf->dims[tf->n_layers];
+    if (N < 1 || G < 1 || M_max < 1 || !(k_o > 0) || !(alpha_o > 0)) return -1;
+    if (group_off[0] != 0 || group_off[G] != N) return -1;
+    for (int g = 0; g < G; ++g)
+        if (group_off[g + 1] < group_off[g] || group_action[g] < 0 || group_action[g] >= A ||
+            branch_count[g] < 0 || branch_count[g] > M_max || visit_count[g] < 0) return -1;
+    float *prop = (float *)malloc(sizeof(float) * (size_t)N * S);
+    float *obs = (float *)malloc(sizeof(float) * (size_t)N * O);
+    float *L = (float *)malloc(sizeof(float) * (size_t)N);
+    float *v = (float *)calloc((size_t)N, sizeof(float));
+    int32_t *br = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    int32_t *anc = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    int32_t *gid = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    for (int g = 0; g < G; ++g)
+        for (int i = group_off[g]; i < group_off[g + 1]; ++i) gid[i] = g;
+    /* 1. successor states and sampled observations of every simulation */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        scratch z = scratch_alloc(m);
+        const int a = group_action[gid[i]];
+        for (int k = 0; k < S; ++k) z.s[k] = (real)particles[(size_t)i * S + k];
+        gen_step(m, 0, z.s, a, seed, (uint32_t)i, 0, 0, VO_STREAM_BELIEF_T, &z, z.sn);
+        for (int k = 0; k < S; ++k) prop[(size_t)i * S + k] = (float)z.sn[k];
+        gen_step(m, 1, z.sn, a, seed, (uint32_t)i, 0, 0, VO_STREAM_PW_OBS, &z, z.o);
+        for (int k = 0; k < O; ++k) obs[(size_t)i * O + k] = (float)z.o[k];
+        scratch_free(&z);
+    }
+    /* 2. progressive widening, simulation by simulation within each action node */
+    for (int g = 0; g < G; ++g) {
+        int C = branch_count[g], n = visit_count[g];
+        for (int i = group_off[g]; i < group_off[g + 1]; ++i) {
+            ++n;
+            int T = pw_threshold(k_o, alpha_o, n);
+            if (T > M_max) T = M_max;
+            int opened = 0;
+            if (C < T) {
+                memcpy(branch_obs + ((size_t)g * M_max + C) * O, obs + (size_t)i * O, sizeof(float) * (size_t)O);
+                br[i] = C;
+                ++C;
+                opened = 1;
+            } else {
+                const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+                const uint32_t ctr[4] = {(uint32_t)i, 0, 0, VO_STREAM_PW_ATTACH << 16};
+                uint32_t x[4];
+                vo_philox4x32_10(ctr, key, x);
+                br[i] = (int32_t)(((uint64_t)x[0] * (uint64_t)C) >> 32); /* C >= 1 here: T(n) >= 1 */
+            }
+            if (opened_out) opened_out[i] = opened;
+        }
+        branch_count[g] = C;
+        visit_count[g] = n;
+    }
+    /* 3. batched likelihood: every stored branch observation through the tower f, then the scores */
+    real *E = (real *)calloc((size_t)G * M_max * d, sizeof(real));
+#pragma omp parallel for schedule(static)
+    for (int gm = 0; gm < G * M_max; ++gm) {
+        if (gm % M_max >= branch_count[gm / M_max]) continue;
+        scratch z = scratch_alloc(m);
+        for (int k = 0; k < O; ++k) z.x[k] = (real)branch_obs[(size_t)gm * O + k];
+        mlp_forward_one(tf, m->emulate_bf16, z.x, E + (size_t)gm * d, z.b0, z.b1);
+        scratch_free(&z);
+    }
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        scratch z = scratch_alloc(m);
+        real *gout = (real *)malloc(sizeof(real) * d);
+        const int g = gid[i], a = group_action[g];
+        for (int k = 0; k < S; ++k) z.x[k] = (real)prop[(size_t)i * S + k];
+        if (m->lik_action_cond)
+            for (int k = 0; k < A; ++k) z.x[S + k] = (k == a) ? (real)1 : (real)0;
+        mlp_forward_one(tg, m->emulate_bf16, z.x, gout, z.b0, z.b1);
+        const real *e = E + ((size_t)g * M_max + br[i]) * d;
+        real ell = 0;
+        for (int k = 0; k < d; ++k) ell += e[k] * gout[k];
+        float lw = 0.0f;
+        if (weights) lw = weights[i] > 0 ? logf(weights[i]) : -INFINITY;
+        L[i] = lw + (float)ell / m->lambda;
+        free(gout);
+        scratch_free(&z);
+    }
+    free(E);
+    /* 4. every (action node, branch) child belief: normalise, resample among its members */
+    for (int i = 0; i < N; ++i) anc[i] = i;
+    if (seg_status_out) for (int gm = 0; gm < G * M_max; ++gm) seg_status_out[gm] = 0;
+    int32_t *mem = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    float *vm = (float *)malloc(sizeof(float) * (size_t)N);
+    int32_t *am = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    for (int g = 0; g < G; ++g)
+        for (int b = 0; b < branch_count[g]; ++b) {
+            int n = 0;
+            for (int i = group_off[g]; i < group_off[g + 1]; ++i) if (br[i] == b) mem[n++] = i;
+            if (n == 0) continue;
+            float mx = -INFINITY;
+            int bad = 0;
+            for (int r = 0; r < n; ++r) {
+                if (L[mem[r]] > mx) mx = L[mem[r]];
+                if (L[mem[r]] != L[mem[r]]) bad = 1;
+            }
+            if (!(mx > -INFINITY) || !(mx < INFINITY)) bad = 1;
+            int st = bad ? -2 : 0;
+            if (!bad) {
+                for (int r = 0; r < n; ++r) vm[r] = expf(L[mem[r]] - mx);
+                const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+                const uint32_t ctr[4] = {(uint32_t)(g * M_max + b), 0, 0, VO_STREAM_RESAMPLE << 16};
+                uint32_t x[4];
+                vo_philox4x32_10(ctr, key, x);
+                st = vo_resample_systematic_x0(vm, n, x[0], am);
+                for (int r = 0; r < n; ++r) v[mem[r]] = vm[r];
+            }
+            if (weights_out) for (int r = 0; r < n; ++r) weights_out[mem[r]] = 1.0f / (float)n;
+            if (st) {
+                if (seg_status_out) seg_status_out[g * M_max + b] = 1;
+                continue; /* members keep themselves */
+            }
+            for (int r = 0; r < n; ++r) anc[mem[r]] = mem[am[r]];
+        }
+    free(mem); free(vm); free(am);
+    for (int i = 0; i < N; ++i) {
+        if (particles_out)
+            for (int j = 0; j < S; ++j) particles_out[(size_t)i * S + j] = prop[(size_t)anc[i] * S + j];
+        if (ancestors_out) ancestors_out[i] = anc[i];
+        if (sim_branch_out) sim_branch_out[i] = br[i];
+    }
+    if (proposals_out) memcpy(proposals_out, prop, sizeof(float) * (size_t)N * S);
+    if (obs_out) memcpy(obs_out, obs, sizeof(float) * (size_t)N * O);
+    if (logits_out) memcpy(logits_out, L, sizeof(float) * (size_t)N);
+    if (post_weights_out) memcpy(post_weights_out, v, sizeof(float) * (size_t)N);
+    free(prop); free(obs); free(L); free(v); free(br); free(anc); free(gid);
+    return 0;
 }
 
 /* Normalised weights as the resampler sees them (O6): wbar_i = q_i / W in double. */

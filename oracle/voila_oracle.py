@@ -56,6 +56,9 @@ def _lib(real: str = "f32"):
     lib.vo_rollout_values.restype = i32
     lib.vo_rollout_values_term.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, i32, vp, vp, vp, vp, vp, vp]
     lib.vo_rollout_values_term.restype = i32
+    lib.vo_pw_update.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp, i32, f64, f64, vp, u64,
+                                 vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vo_pw_update.restype = i32
     lib.vo_model_set_terminal.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     lib.vo_model_set_terminal.restype = i32
     lib.vo_resample_systematic_x0.argtypes = [vp, i32, u32, vp]
@@ -232,6 +235,34 @@ class OracleModel:
                                              _p(out["margin"]))
         if rc != 0:
             raise RuntimeError(f"vo_rollout_values_term -> {rc}")
+        return out
+
+    def pw_update(self, particles, group_off, group_action, visit_count, branch_count, branch_obs, k_o,
+                  alpha_o, weights, seed):
+        """Vectorised progressive widening with batched likelihood (vo_pw_update).  visit_count,
+        branch_count, branch_obs ([G][M_max][O]) are NOT modified: updated copies come back in the
+        result dict next to the per-simulation outputs."""
+        particles = _f32(particles)
+        weights = _f32(weights)
+        group_off = np.ascontiguousarray(group_off, dtype=np.int32)
+        group_action = np.ascontiguousarray(group_action, dtype=np.int32)
+        vc = np.array(visit_count, dtype=np.int32)
+        bc = np.array(branch_count, dtype=np.int32)
+        bo = np.array(branch_obs, dtype=np.float32)
+        N, G, M_max = particles.shape[0], group_action.shape[0], bo.shape[1]
+        out = {"proposals": np.zeros((N, self.S), np.float32), "obs": np.zeros((N, self.O), np.float32),
+               "sim_branch": np.zeros(N, np.int32), "opened": np.zeros(N, np.int32),
+               "logits": np.zeros(N, np.float32), "post_weights": np.zeros(N, np.float32),
+               "ancestors": np.zeros(N, np.int32), "particles": np.zeros((N, self.S), np.float32),
+               "weights": np.zeros(N, np.float32), "seg_status": np.zeros(G * M_max, np.int32)}
+        rc = self.lib.vo_pw_update(self.h, _p(particles), N, _p(group_off), G, _p(group_action), _p(vc), _p(bc),
+                                   _p(bo), M_max, float(k_o), float(alpha_o), _p(weights), int(seed),
+                                   _p(out["proposals"]), _p(out["obs"]), _p(out["sim_branch"]), _p(out["opened"]),
+                                   _p(out["logits"]), _p(out["post_weights"]), _p(out["ancestors"]),
+                                   _p(out["particles"]), _p(out["weights"]), _p(out["seg_status"]))
+        if rc != 0:
+            raise RuntimeError(f"vo_pw_update -> {rc}")
+        out.update({"visit_count": vc, "branch_count": bc, "branch_obs": bo})
         return out
 
     def belief_update(self, particles, action, observation, weights, seed, ess_threshold=None):
