@@ -248,6 +248,48 @@ voila_status voila_belief_update_ess(voila_ctx *ctx, const void *particles, int 
                                      float *log_evidence_out, float *ess_out, int32_t *resampled_out,
                                      int32_t *dev_status_out, void *cuda_stream);
 
+/* Vectorised progressive widening with batched likelihood (section 4.3:
+ * "an action node a is expanded with a sampled observation whenever |C(a)| < k_o N(a)^alpha_o ...
+ * Otherwise, the sampled successor state is associated with a previously existing observation branch
+ * of the same action node.  The likelihood model l(s', a, o) is then used to weight successor states
+ * according to the observation stored at the selected branch, followed by resampling ... parallel
+ * simulations are grouped by their parent action nodes, after which the above PW operations are
+ * performed for all action-node groups in parallel").  DESIGN.md readings R26-R29 fix what the paper
+ * leaves open.  N simulations, grouped: action node g owns the simulations
+ * [group_off[g], group_off[g+1]) and has the action group_action[g], the visit count visit_count[g] =
+ * N(a), branch_count[g] = |C(a)| stored observation branches branch_obs[g][0 .. |C(a)|) (M_max rows of O
+ * floats reserved per node).  For every simulation i of node g, in index order:
+ *   s'_i = f_T(s_i, a_g, w_T(i)) (Philox stream 3, counter (i,0,0)),
+ *   N(a) += 1; if |C(a)| < min(M_max, ceil(k_o N(a)^alpha_o (1 - 1e-9))) the simulation opens branch |C(a)|,
+ *   storing o_i = f_Z(s'_i, a_g, w_Z(i)) (stream 5), and is attached to it; otherwise it is attached to
+ *   the existing branch (x_i |C(a)|) >> 32, x_i one Philox word (stream 6);
+ *   L_i = log w_i + <f(obs_{g,b(i)}), g(s'_i)> / lambda  (every stored observation goes through the tower f
+ *   as one batch).
+ * Every (node, branch) pair that received simulations is a child belief: its members (in index order)
+ * are resampled among themselves with the exact-integer systematic resampler (v = exp(L - max over the
+ * child), offset word keyed by g*M_max+b); the r-th member receives the r-th draw.
+ *   particles      dev [N][S] fp32 | bf16        group_off dev [G+1] int32 (group_off[0] = 0, [G] = N)
+ *   group_action   dev [G] int32 in [0, A)       visit_count, branch_count dev [G] int32, updated in place
+ *   branch_obs     dev [G][M_max][O] fp32, rows of opened branches are written      1 <= M_max <= 64
+ *   weights        dev [N] fp32 >= 0 or NULL     k_o > 0, alpha_o > 0
+ *   particles_out  dev [N][S] or NULL: s' of the simulation's draw;  weights_out dev [N] or NULL: 1 / members
+ *   ancestors_out  dev [N] int32 or NULL: simulation index of the draw (a member of the same child)
+ *   sim_branch_out dev [N] int32 or NULL;  opened_out dev [N] int32 or NULL (1: opened its branch)
+ *   post_weights_out dev [N] fp32 or NULL: v_i;  proposals_out dev [N][S] or NULL: s'_i
+ *   seg_status_out dev [G*M_max] int32 or NULL: 1 for a child whose weights are all zero / not finite
+ *                  (its members keep themselves), else 0
+ * The group arrays are not validated on the device (offsets must be non-decreasing, actions in range,
+ * 0 <= branch_count <= M_max).  Needs voila_pw_reserve(N, G, M_max) first (VOILA_ERR_WORKSPACE otherwise).
+ * Errors: VOILA_ERR_INVALID_ARG for NULL / non-positive sizes, M_max > 64, k_o <= 0, alpha_o <= 0. */
+size_t voila_pw_workspace_bytes(const voila_ctx *ctx, int N, int G, int M_max);
+voila_status voila_pw_reserve(voila_ctx *ctx, int N, int G, int M_max);
+voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const int32_t *group_off, int G,
+                             const int32_t *group_action, int32_t *visit_count, int32_t *branch_count,
+                             float *branch_obs, int M_max, double k_o, double alpha_o, const float *weights,
+                             uint64_t seed, void *particles_out, float *weights_out, int32_t *ancestors_out,
+                             int32_t *sim_branch_out, int32_t *opened_out, float *post_weights_out,
+                             void *proposals_out, int32_t *seg_status_out, void *cuda_stream);
+
 /* Host-buffer variants: every pointer is HOST memory (pinned for best speed); inputs are copied to
  * ctx-owned device staging buffers, the device entry point runs, outputs are copied back and the
  * stream is synchronised.  Optional outputs as above (NULL to skip). */

@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["voila_api.cu", "mlp_ffma.cu", "belief.cu", "porpp.cu", "rollout_tc.cu", "rollout_tc2.cu"]
+SOURCES = ["voila_api.cu", "mlp_ffma.cu", "belief.cu", "porpp.cu", "pw.cu", "rollout_tc.cu", "rollout_tc2.cu"]
 HEADERS = ["voila_device.cuh", "voila_internal.h", "voila_kernels.h", "sm100_ptx.cuh", "tc_program.h", "tc2_program.h", "tc_common.cuh",
            "../../include/voila.h"]
 LIB = os.path.join(HERE, "libvoila.so")

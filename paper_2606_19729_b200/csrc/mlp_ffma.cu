@@ -256,6 +256,142 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Progressive widening (voila_pw_update): the MLP stages on the CUDA cores.
+// Every row carries its own action (simulations of different action nodes share a tile), so the
+// one-hot block is part of the operand here (same sum: the zeros contribute exactly 0 and the block
+// sits between the state and the noise rows, where the folded form adds its weight row).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fill_onehot(float *x, int base, int A, const int *act_row) {
+    for (int idx = threadIdx.x; idx < A * R; idx += kThreads) {
+        const int r = idx & (R - 1), k = idx / R;
+        x[(base + k) * R + r] = (k == act_row[r]) ? 1.0f : 0.0f;
+    }
+}
+template <bool EMU>
+__device__ __forceinline__ void load_rows(const void *rows_in, int S, const int *src_row, float *x) {
+    for (int idx = threadIdx.x; idx < S * R; idx += kThreads) {
+        const int r = idx / S, i = idx - r * S;
+        float v = 0.0f;
+        if (src_row[r] >= 0) {
+            const size_t g = (size_t)src_row[r] * S + i;
+            v = EMU ? bf16_to_float(reinterpret_cast<const uint16_t *>(rows_in)[g])
+                    : reinterpret_cast<const float *>(rows_in)[g];
+        }
+        x[i * R + r] = v;
+    }
+}
+
+// s'_i = f_T(s_i, a_g(i), w_T(i)): stream 3, counter (i, 0, 0), as the belief update draws it.
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) pw_propose_ffma_kernel(const ModelDev m, const PwArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ int act_row[R], src_row[R];
+    const int S = m.S, A = m.A, Nz = m.Nz, KW = m.max_width;
+    float *xa = smem, *xb = xa + KW * R, *sn = xb + KW * R;
+    const int i0 = blockIdx.x * R;
+    if (threadIdx.x < R) {
+        const int i = i0 + threadIdx.x;
+        src_row[threadIdx.x] = i < a.N ? i : -1;
+        act_row[threadIdx.x] = i < a.N ? __ldg(a.group_action + a.sim_group[i]) : 0;
+    }
+    __syncthreads();
+    load_rows<EMU>(a.particles, S, src_row, xa);
+    fill_onehot(xa, S, A, act_row);
+    fill_noise<EMU>(xa, S + A, Nz, a.seed, i0, 0u, 0u, kStreamBeliefT);
+    __syncthreads();
+    const int K0 = S + A + Nz;
+    mlp_chain<EMU>(m.mlp[0], xa, xb, sn, K0, K0, -1);
+    for (int idx = threadIdx.x; idx < S * R; idx += kThreads) {
+        const int r = idx / S, i = idx - r * S;
+        if (i0 + r < a.N) {
+            const float v = sn[i * R + r];
+            const size_t gidx = (size_t)(i0 + r) * S + i;
+            if (EMU) reinterpret_cast<uint16_t *>(a.proposals)[gidx] = bf16_bits(v);
+            else reinterpret_cast<float *>(a.proposals)[gidx] = v;
+        }
+    }
+}
+
+// o_i = f_Z(s'_i, a, w_Z(i)) (stream 5) for the simulations that opened a branch: one row per
+// (action node, branch) slot, stored as the branch's observation.
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) pw_obs_ffma_kernel(const ModelDev m, const PwArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ int act_row[R], src_row[R];
+    const int S = m.S, O = m.O, A = m.A, Nz = m.Nz, KW = m.max_width;
+    float *xa = smem, *xb = xa + KW * R, *out = xb + KW * R;
+    const int gm0 = blockIdx.x * R, n_slots = a.G * a.M_max;
+    if (threadIdx.x < R) {
+        const int gm = gm0 + threadIdx.x;
+        src_row[threadIdx.x] = gm < n_slots ? a.new_src[gm] : -1;
+        act_row[threadIdx.x] = gm < n_slots ? __ldg(a.group_action + gm / a.M_max) : 0;
+    }
+    __syncthreads();
+    bool any = false;
+    for (int r = 0; r < R; ++r) any |= src_row[r] >= 0;
+    if (!any) return;  // uniform: no branch was opened in this tile of slots
+    load_rows<EMU>(a.proposals, S, src_row, xa);
+    fill_onehot(xa, S, A, act_row);
+    const int nblk = (Nz + 3) >> 2;
+    for (int idx = threadIdx.x; idx < R * nblk; idx += kThreads) {
+        const int r = idx & (R - 1), blk = idx / R;
+        float z[4];
+        normals4<false>(a.seed, (uint32_t)max(src_row[r], 0), 0u, 0u, kStreamPwObs, (uint32_t)blk, z);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (4 * blk + i < Nz) xa[(S + A + 4 * blk + i) * R + r] = EMU ? bf16_round(z[i]) : z[i];
+    }
+    __syncthreads();
+    const int K0 = S + A + Nz;
+    mlp_chain<EMU>(m.mlp[1], xa, xb, out, K0, K0, -1);
+    for (int idx = threadIdx.x; idx < O * R; idx += kThreads) {
+        const int r = idx / O, k = idx - r * O;
+        if (src_row[r] >= 0) a.branch_obs[(size_t)(gm0 + r) * O + k] = out[k * R + r];
+    }
+}
+
+// L_i = log w_i + <e_{g, b(i)}, g(s'_i [; onehot(a)])> / lambda and the running maximum of its child.
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) pw_score_ffma_kernel(const ModelDev m, const PwArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ int act_row[R], src_row[R];
+    const int S = m.S, A = m.A, KW = m.max_width;
+    const MlpDev &g = m.mlp[3];
+    const int d = g.dims[g.n_layers];
+    float *xa = smem, *xb = xa + KW * R, *gout = xb + KW * R;
+    const int i0 = blockIdx.x * R;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < R) {
+        const int i = i0 + threadIdx.x;
+        src_row[threadIdx.x] = i < a.N ? i : -1;
+        act_row[threadIdx.x] = i < a.N ? __ldg(a.group_action + a.sim_group[i]) : 0;
+    }
+    __syncthreads();
+    load_rows<EMU>(a.proposals, S, src_row, xa);
+    if (m.lik_action_cond) fill_onehot(xa, S, A, act_row);
+    __syncthreads();
+    const int K0 = S + (m.lik_action_cond ? A : 0);
+    mlp_chain<EMU>(g, xa, xb, gout, K0, K0, -1);
+    if (warp == 0) {
+        const int i = i0 + lane;
+        if (i < a.N) {
+            const int seg = a.sim_group[i] * a.M_max + a.sim_branch[i];
+            const float *e = a.E + (size_t)seg * d;
+            float ell = 0.0f;
+            for (int k = 0; k < d; ++k) ell += __ldg(e + k) * gout[k * R + lane];
+            float lw = 0.0f;
+            if (a.weights) {
+                const float w = __ldg(a.weights + i);
+                lw = w > 0.0f ? logf(w) : -INFINITY;
+            }
+            const float L = lw + ell / m.lambda;
+            a.logits[i] = L;
+            atomicMax(a.seg_max + seg, float_to_ordered(L));
+        }
+    }
+}
+
 __global__ void weight_sum_kernel(const float *__restrict__ w, int n, double *out) {
     __shared__ double sh[256];
     double acc = 0.0;
@@ -417,6 +553,30 @@ size_t ffma_smem_bytes(const ModelDev &m) {
     const size_t fwd = (size_t)(3 * m.max_width) * R * sizeof(float);
     size_t b = rollout > belief ? rollout : belief;
     return b > fwd ? b : fwd;
+}
+
+template <typename K>
+static cudaError_t pw_launch(K kernel, int grid, const ModelDev &m, const PwArgs &a, cudaStream_t st) {
+    const size_t smem = ffma_smem_bytes(m);
+    cudaError_t e;
+    if ((e = set_smem(kernel, smem)) != cudaSuccess) return e;
+    kernel<<<grid, kThreads, smem, st>>>(m, a);
+    return cudaGetLastError();
+}
+cudaError_t launch_pw_propose_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st) {
+    const int grid = (a.N + R - 1) / R;
+    return bf16 ? pw_launch(pw_propose_ffma_kernel<true>, grid, m, a, st)
+                : pw_launch(pw_propose_ffma_kernel<false>, grid, m, a, st);
+}
+cudaError_t launch_pw_obs_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st) {
+    const int grid = (a.G * a.M_max + R - 1) / R;
+    return bf16 ? pw_launch(pw_obs_ffma_kernel<true>, grid, m, a, st)
+                : pw_launch(pw_obs_ffma_kernel<false>, grid, m, a, st);
+}
+cudaError_t launch_pw_score_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st) {
+    const int grid = (a.N + R - 1) / R;
+    return bf16 ? pw_launch(pw_score_ffma_kernel<true>, grid, m, a, st)
+                : pw_launch(pw_score_ffma_kernel<false>, grid, m, a, st);
 }
 
 cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cudaStream_t st) {

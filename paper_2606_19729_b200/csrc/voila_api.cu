@@ -360,6 +360,7 @@ void voila_destroy(voila_ctx *ctx) {
         for (void *p : ctx->dev_allocs) cudaFree(p);
         if (ctx->ws) cudaFree(ctx->ws);
         if (ctx->stage) cudaFree(ctx->stage);
+        if (ctx->pw_ws) cudaFree(ctx->pw_ws);
     }
     delete ctx;
 }
@@ -584,6 +585,129 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 3;
     return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st, v, false);
+}
+
+// ---- progressive widening ----
+namespace {
+struct PwLayout {
+    size_t sim_group, sim_branch, sim_rank, perm, seg_of_pos, seg_count, seg_off, new_src, seg_max, E, logits,
+        v_sorted, proposals, total;
+};
+PwLayout make_pw_layout(const voila_ctx *ctx, int N, int G, int M) {
+    PwLayout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t o = off;
+        off += align_up(bytes > 0 ? bytes : 1);
+        return o;
+    };
+    const size_t esize = ctx->prec == VOILA_PREC_BF16 ? 2 : 4;
+    const size_t gm = (size_t)G * M;
+    L.sim_group = take((size_t)N * 4);
+    L.sim_branch = take((size_t)N * 4);
+    L.sim_rank = take((size_t)N * 4);
+    L.perm = take((size_t)N * 4);
+    L.seg_of_pos = take((size_t)N * 4);
+    L.seg_count = take(gm * 4);
+    L.seg_off = take((gm + 1) * 4);
+    L.new_src = take(gm * 4);
+    L.seg_max = take(gm * 4);
+    L.E = take(gm * ctx->d * sizeof(float));
+    L.logits = take((size_t)N * 4);
+    L.v_sorted = take((size_t)N * 4);
+    L.proposals = take((size_t)N * ctx->S * esize);
+    L.total = off;
+    return L;
+}
+}  // namespace
+
+size_t voila_pw_workspace_bytes(const voila_ctx *ctx, int N, int G, int M_max) {
+    if (!ctx || N < 0 || G < 0 || M_max < 0) return 0;
+    return make_pw_layout(ctx, N, G, M_max).total;
+}
+
+voila_status voila_pw_reserve(voila_ctx *ctx, int N, int G, int M_max) {
+    if (!ctx || N < 1 || G < 1 || M_max < 1 || M_max > kPwMaxBranches) return VOILA_ERR_INVALID_ARG;
+    if ((long long)G * M_max >= (1ll << 30)) return VOILA_ERR_INVALID_ARG;
+    // the uint64 scan of the sorted weights uses the belief update's scan buffers
+    if (!ctx->ws || N > ctx->res_N) {
+        const voila_status s = voila_reserve(ctx, ctx->res_P, ctx->res_Q, ctx->res_H, N > ctx->res_N ? N : ctx->res_N);
+        if (s != VOILA_OK) return s;
+    }
+    DeviceGuard guard(ctx->device);
+    cudaDeviceSynchronize();
+    if (ctx->pw_ws) cudaFree(ctx->pw_ws);
+    ctx->pw_ws = nullptr;
+    ctx->pw_N = ctx->pw_G = ctx->pw_M = 0;
+    const cudaError_t e = cudaMalloc(&ctx->pw_ws, make_pw_layout(ctx, N, G, M_max).total);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->pw_N = N; ctx->pw_G = G; ctx->pw_M = M_max;
+    return VOILA_OK;
+}
+
+voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const int32_t *group_off, int G,
+                             const int32_t *group_action, int32_t *visit_count, int32_t *branch_count,
+                             float *branch_obs, int M_max, double k_o, double alpha_o, const float *weights,
+                             uint64_t seed, void *particles_out, float *weights_out, int32_t *ancestors_out,
+                             int32_t *sim_branch_out, int32_t *opened_out, float *post_weights_out,
+                             void *proposals_out, int32_t *seg_status_out, void *cuda_stream) {
+    if (!ctx || !particles || !group_off || !group_action || !visit_count || !branch_count || !branch_obs)
+        return VOILA_ERR_INVALID_ARG;
+    if (N < 1 || G < 1 || M_max < 1 || M_max > kPwMaxBranches || !(k_o > 0.0) || !(alpha_o > 0.0))
+        return VOILA_ERR_INVALID_ARG;
+    if (particles_out == particles || proposals_out == particles || (particles_out && particles_out == proposals_out))
+        return VOILA_ERR_INVALID_ARG;
+    if (misaligned(particles) || misaligned(weights) || misaligned(particles_out) || misaligned(proposals_out) ||
+        misaligned(branch_obs))
+        return VOILA_ERR_INVALID_ARG;
+    if (!ctx->pw_ws || !ctx->ws || N > ctx->pw_N || N > ctx->res_N ||
+        (long long)G * M_max > (long long)ctx->pw_G * ctx->pw_M)
+        return VOILA_ERR_WORKSPACE;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const bool bf16 = ctx->prec == VOILA_PREC_BF16;
+    const size_t esize = bf16 ? 2 : 4;
+    // carve for the reserved maxima (G * M_max slots may be split differently than reserved)
+    const PwLayout L = make_pw_layout(ctx, ctx->pw_N, ctx->pw_G, ctx->pw_M);
+    uint8_t *w = reinterpret_cast<uint8_t *>(ctx->pw_ws);
+    PwArgs a{};
+    a.particles = particles; a.weights = weights;
+    a.N = N; a.G = G; a.M_max = M_max;
+    a.group_off = group_off; a.group_action = group_action;
+    a.visit_count = visit_count; a.branch_count = branch_count; a.branch_obs = branch_obs;
+    a.k_o = k_o; a.alpha_o = alpha_o; a.seed = seed;
+    a.sim_group = reinterpret_cast<int32_t *>(w + L.sim_group);
+    a.sim_branch = reinterpret_cast<int32_t *>(w + L.sim_branch);
+    a.sim_rank = reinterpret_cast<int32_t *>(w + L.sim_rank);
+    a.perm = reinterpret_cast<int32_t *>(w + L.perm);
+    a.seg_of_pos = reinterpret_cast<int32_t *>(w + L.seg_of_pos);
+    a.seg_count = reinterpret_cast<int32_t *>(w + L.seg_count);
+    a.seg_off = reinterpret_cast<int32_t *>(w + L.seg_off);
+    a.new_src = reinterpret_cast<int32_t *>(w + L.new_src);
+    a.seg_max = reinterpret_cast<int *>(w + L.seg_max);
+    a.E = reinterpret_cast<float *>(w + L.E);
+    a.logits = reinterpret_cast<float *>(w + L.logits);
+    a.v_sorted = reinterpret_cast<float *>(w + L.v_sorted);
+    a.proposals = proposals_out ? proposals_out : (void *)(w + L.proposals);
+    a.particles_out = particles_out; a.weights_out = weights_out; a.post_weights_out = post_weights_out;
+    a.ancestors_out = ancestors_out; a.sim_branch_out = sim_branch_out; a.opened_out = opened_out;
+    a.seg_status_out = seg_status_out;
+
+    const Layout SL = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
+    const ScanBuffers sb = scan_buffers(ctx, SL);
+    cudaError_t e = launch_pw_widen(a, st);                                  // branches, children, sorted order
+    if (e == cudaSuccess) e = launch_pw_propose_ffma(ctx->model, a, bf16, st);  // s' of every simulation
+    if (e == cudaSuccess) e = launch_pw_obs_ffma(ctx->model, a, bf16, st);      // o of the opened branches
+    if (e == cudaSuccess)                                                     // e = f(o) of every stored branch: one batch
+        e = launch_mlp_forward_ffma(ctx->model, 2, branch_obs, G * M_max, a.E, bf16, st);
+    if (e == cudaSuccess) e = launch_pw_score_ffma(ctx->model, a, bf16, st);    // L_i, child maxima
+    if (e == cudaSuccess) e = launch_pw_weights(a, st);                       // v in sorted order
+    if (e == cudaSuccess) e = launch_bu_init(sb, N, st);
+    if (e == cudaSuccess) e = launch_weight_scan(sb, a.v_sorted, N, false, nullptr, st);  // uint64 CDF over the sorted order
+    if (e == cudaSuccess) e = launch_pw_resample(a, sb.cdf, ctx->S * (int)esize, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->launches += 11 + (seg_status_out ? 1 : 0);
+    return VOILA_OK;
 }
 
 voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const float *logpi0,

@@ -73,6 +73,30 @@ struct BeliefArgs {
     double *part_wsum;     // [tiles]
 };
 
+// voila_pw_update (progressive widening, pw.cu): arguments, outputs and workspace of one call.
+constexpr int kPwMaxBranches = 64;  // M_max limit (per-warp counters in shared memory)
+struct PwArgs {
+    const void *particles;  // [N][S]
+    const float *weights;   // [N] or nullptr
+    int N, G, M_max;
+    const int32_t *group_off, *group_action;
+    int32_t *visit_count, *branch_count;
+    float *branch_obs;      // [G][M_max][O]
+    double k_o, alpha_o;
+    uint64_t seed;
+    // workspace
+    int32_t *sim_group, *sim_branch, *sim_rank, *perm, *seg_of_pos;  // [N]
+    int32_t *seg_count, *seg_off, *new_src;                         // [G*M_max] (+1 for seg_off)
+    int *seg_max;                                                   // [G*M_max] ordered-int maxima
+    float *E;                                                       // [G*M_max][d] tower embeddings
+    float *logits, *v_sorted;                                       // [N]
+    void *proposals;                                                // [N][S]
+    // outputs (any may be null)
+    void *particles_out;
+    float *weights_out, *post_weights_out;
+    int32_t *ancestors_out, *sim_branch_out, *opened_out, *seg_status_out;
+};
+
 // Bookkeeping block of the scan / resample kernels (device memory, zeroed per call by a kernel).
 struct ScanState {
     unsigned long long total_q;  // W
@@ -100,6 +124,9 @@ struct voila_ctx {
     void *ws = nullptr;
     size_t ws_bytes = 0;
     int res_P = 0, res_Q = 0, res_H = 0, res_N = 0;
+    // workspace of voila_pw_update (voila_pw_reserve)
+    void *pw_ws = nullptr;
+    int pw_N = 0, pw_G = 0, pw_M = 0;
     // staging for *_host entry points
     void *stage = nullptr;
     size_t stage_bytes = 0;

@@ -48,6 +48,14 @@ cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *pro
                                    int32_t *ancestors_out, cudaStream_t st, const float *w_in,
                                    bool from_logits);
 
+// ---- pw.cu / mlp_ffma.cu : vectorised progressive widening with batched likelihood (voila_pw_update) ----
+cudaError_t launch_pw_widen(const PwArgs &a, cudaStream_t st);          // widen + child offsets + sorted order (3 launches)
+cudaError_t launch_pw_propose_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);
+cudaError_t launch_pw_obs_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);
+cudaError_t launch_pw_score_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);
+cudaError_t launch_pw_weights(const PwArgs &a, cudaStream_t st);
+cudaError_t launch_pw_resample(const PwArgs &a, const unsigned long long *cdf, int row_bytes, cudaStream_t st);  // 1-2 launches
+
 // ---- porpp.cu : one level of the PORPP preference backup (Eq. 1) ----
 cudaError_t launch_porpp_backup_level(const float *R, const float *logpi0, const int32_t *child_off,
                                       const int32_t *child_idx, const float *child_w, const float *v_next,

@@ -26,7 +26,7 @@ EXPORTS = [
     "voila_rollout_values_host",
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
-    "voila_profile_read",
+    "voila_profile_read", "voila_pw_workspace_bytes", "voila_pw_reserve", "voila_pw_update",
 ]
 
 
@@ -119,6 +119,13 @@ def load_library():
     lib.voila_set_profiling.restype = i32
     lib.voila_profile_read.argtypes = [vp, i32, C.POINTER(C.c_float), i32]
     lib.voila_profile_read.restype = i32
+    lib.voila_pw_workspace_bytes.argtypes = [vp, i32, i32, i32]
+    lib.voila_pw_workspace_bytes.restype = sz
+    lib.voila_pw_reserve.argtypes = [vp, i32, i32, i32]
+    lib.voila_pw_reserve.restype = i32
+    lib.voila_pw_update.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp, i32, C.c_double, C.c_double, vp, u64,
+                                    vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.voila_pw_update.restype = i32
     lib.voila_version.argtypes = []
     lib.voila_version.restype = i32
     _LIB = lib
@@ -332,6 +339,41 @@ class Voila:
             _dptr(out["ancestors"]), _dptr(out.get("post_weights")), _dptr(out.get("proposals")),
             _dptr(out["log_evidence"]), _dptr(out["ess"]), _dptr(out["resampled"]), _dptr(out["status"]),
             self._stream()), "voila_belief_update_ess")
+        return out
+
+    def voila_pw_update(self, particles, group_off, group_action, visit_count, branch_count, branch_obs, k_o,
+                        alpha_o, weights, seed, want_debug=True):
+        """Vectorised progressive widening with batched likelihood (include/voila.h).  visit_count,
+        branch_count ([G] int32) and branch_obs ([G][M_max][O] fp32) are device tensors updated IN PLACE."""
+        torch = self._torch
+        N, S = particles.shape
+        G, M_max = branch_obs.shape[0], branch_obs.shape[1]
+        assert S == self.S and particles.dtype == self.particle_dtype and particles.is_contiguous()
+        assert group_off.dtype == torch.int32 and group_off.numel() == G + 1 and group_action.dtype == torch.int32
+        assert visit_count.dtype == torch.int32 and branch_count.dtype == torch.int32
+        assert branch_obs.dtype == torch.float32 and branch_obs.is_contiguous() and branch_obs.shape[2] == self.O
+        self._ensure(N=N)
+        res = getattr(self, "_pw_res", (0, 0))
+        if res[0] < N or res[1] < G * M_max:
+            self._check(self.lib.voila_pw_reserve(self._h, N, G, M_max), "voila_pw_reserve")
+            self._pw_res = (N, G * M_max)
+        dev = particles.device
+        out = {"particles": torch.empty_like(particles),
+               "weights": torch.empty(N, dtype=torch.float32, device=dev),
+               "ancestors": torch.empty(N, dtype=torch.int32, device=dev),
+               "sim_branch": torch.empty(N, dtype=torch.int32, device=dev),
+               "seg_status": torch.empty(G * M_max, dtype=torch.int32, device=dev)}
+        if want_debug:
+            out["opened"] = torch.empty(N, dtype=torch.int32, device=dev)
+            out["post_weights"] = torch.empty(N, dtype=torch.float32, device=dev)
+            out["proposals"] = torch.empty_like(particles)
+        self._check(self.lib.voila_pw_update(
+            self._h, _dptr(particles), N, _dptr(group_off), G, _dptr(group_action), _dptr(visit_count),
+            _dptr(branch_count), _dptr(branch_obs), M_max, C.c_double(float(k_o)), C.c_double(float(alpha_o)),
+            _dptr(weights), C.c_uint64(int(seed)), _dptr(out["particles"]), _dptr(out["weights"]),
+            _dptr(out["ancestors"]), _dptr(out["sim_branch"]), _dptr(out.get("opened")),
+            _dptr(out.get("post_weights")), _dptr(out.get("proposals")), _dptr(out["seg_status"]),
+            self._stream()), "voila_pw_update")
         return out
 
     def voila_resample_systematic(self, v, seed):
