@@ -331,9 +331,27 @@ __global__ void __launch_bounds__(kThreads) pw_obs_ffma_kernel(const ModelDev m,
     bool any = false;
     for (int r = 0; r < R; ++r) any |= src_row[r] >= 0;
     if (!any) return;  // uniform: no branch was opened in this tile of slots
-    load_rows<EMU>(a.proposals, S, src_row, xa);
-    fill_onehot(xa, S, A, act_row);
     const int nblk = (Nz + 3) >> 2;
+    if (a.obs_from_particles) {
+        // the tensor-core pass that stores the proposals runs later: s' of these few rows here
+        load_rows<EMU>(a.particles, S, src_row, xa);
+        fill_onehot(xa, S, A, act_row);
+        for (int idx = threadIdx.x; idx < R * nblk; idx += kThreads) {
+            const int r = idx & (R - 1), blk = idx / R;
+            float z[4];
+            normals4<false>(a.seed, (uint32_t)max(src_row[r], 0), 0u, 0u, kStreamBeliefT, (uint32_t)blk, z);
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (4 * blk + i < Nz) xa[(S + A + 4 * blk + i) * R + r] = EMU ? bf16_round(z[i]) : z[i];
+        }
+        __syncthreads();
+        mlp_chain<EMU>(m.mlp[0], xa, xb, out, S + A + Nz, S + A + Nz, -1);
+        copy_state<EMU>(xa, out, S);
+        __syncthreads();
+    } else {
+        load_rows<EMU>(a.proposals, S, src_row, xa);
+    }
+    fill_onehot(xa, S, A, act_row);
     for (int idx = threadIdx.x; idx < R * nblk; idx += kThreads) {
         const int r = idx & (R - 1), blk = idx / R;
         float z[4];

@@ -142,6 +142,8 @@ __global__ void pw_perm_kernel(PwArgs a) {
     const int pos = a.seg_off[seg] + a.sim_rank[i];
     a.perm[pos] = i;
     a.seg_of_pos[pos] = seg;
+    a.sim_seg[i] = seg;
+    a.sim_action[i] = a.group_action[a.sim_group[i]];
     if (a.sim_branch_out) a.sim_branch_out[i] = a.sim_branch[i];
 }
 

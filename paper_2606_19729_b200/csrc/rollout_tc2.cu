@@ -94,6 +94,12 @@ struct T2Params {
     double *bu_part_wsum;     // [(N + 31) / 32]: prior-weight sums per 32 particles
     float inv_lambda;
     int d;
+    // progressive widening (voila_pw_update): every row has its own action (one-hot block in the
+    // operand), its own tower embedding e and the running maximum of its own child belief
+    const int32_t *pw_sim_action;  // [N] or nullptr (plain belief update)
+    const int32_t *pw_sim_seg;     // [N] child index g * M_max + b
+    const float *pw_E;             // [children][d]
+    int *pw_seg_max;               // [children] ordered-int maxima
 };
 
 struct Smem2 {
@@ -731,7 +737,8 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 for (int c = tid_e; c < (int)L[li].n_pad; c += 256)
                     sbias[L[li].sbias_off + c] = __ldg(p.bias + L[li].bias_off + (size_t)p.bu_action * L[li].n_pad + c);
         }
-        for (int c = tid_e; c < p.hdr.e_pad; c += 256) sbias[p.hdr.e_off + c] = c < p.d ? __ldg(p.bu_e + c) : 0.0f;
+        for (int c = tid_e; c < p.hdr.e_pad; c += 256)
+            sbias[p.hdr.e_off + c] = (p.bu_e && c < p.d) ? __ldg(p.bu_e + c) : 0.0f;
     }
 
     // particle index of this thread's row in (unit, slot)
@@ -760,7 +767,19 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 st_shared_v4(a_unit_addr(a_slot, row, u0 + u), v.x, v.y, v.z, v.w);
             }
         }
-        for (int u = u0 + (Nz >> 3); u < in_units; ++u) st_shared_v4(a_unit_addr(a_slot, row, u), 0u, 0u, 0u, 0u);
+        int u_next = u0 + (Nz >> 3);
+        if (p.pw_sim_action) {
+            // per-row action: the one-hot block is part of the operand, columns [S + Nz, S + Nz + A)
+            const int a_row = valid ? __ldg(p.pw_sim_action + i_idx) : -1;
+            const int n_u = (p.A + 7) >> 3;
+            for (int u = 0; u < n_u; ++u) {
+                uint32_t wv[4] = {0u, 0u, 0u, 0u};
+                if (a_row >= 0 && (a_row >> 3) == u) wv[(a_row & 7) >> 1] = (a_row & 1) ? 0x3F800000u : 0x00003F80u;
+                st_shared_v4(a_unit_addr(a_slot, row, u_next + u), wv[0], wv[1], wv[2], wv[3]);
+            }
+            u_next += n_u;
+        }
+        for (int u = u_next; u < in_units; ++u) st_shared_v4(a_unit_addr(a_slot, row, u), 0u, 0u, 0u, 0u);
     };
 
     if (n_my_units > 0) {
@@ -851,6 +870,13 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                     w = valid ? __ldg(p.weights + i_idx) : 0.0f;
                     lw = w > 0.0f ? logf(w) : -INFINITY;
                 }
+                // progressive widening: the row's own embedding (rows of e_pad floats, zero-padded)
+                const float *e_row = nullptr;
+                int seg = 0;
+                if (p.pw_sim_seg && half == 0) {
+                    seg = valid ? __ldg(p.pw_sim_seg + i_idx) : 0;
+                    e_row = p.pw_E + (size_t)seg * (size_t)p.hdr.e_pad;
+                }
                 es.wait_layer();
                 T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                 if (half == 0) {
@@ -864,7 +890,8 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 #pragma unroll
                             for (int i = 0; i < 4; ++i) {
                                 b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
-                                e4[i] = *(reinterpret_cast<const float4 *>(e_s + 16 * g) + i);
+                                e4[i] = e_row ? __ldg(reinterpret_cast<const float4 *>(e_row + 16 * g) + i)
+                                              : *(reinterpret_cast<const float4 *>(e_s + 16 * g) + i);
                             }
                             tmem_ld_wait();
 #pragma unroll
@@ -879,13 +906,17 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                     const float Lg = lw + ell * p.inv_lambda;
                     int ord = float_to_ordered(valid ? Lg : -INFINITY);
                     if (valid) p.bu_logits[i_idx] = Lg;
+                    if (p.pw_seg_max) {  // the maximum of the row's own child belief; no evidence sums
+                        if (valid) atomicMax(p.pw_seg_max + seg, ord);
+                        ord = (int)0x80000000;
+                    }
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) ord = max(ord, __shfl_xor_sync(0xffffffffu, ord, o));
                     double ws = valid ? (double)w : 0.0;
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
                     const int i0 = i_idx - lane;  // first particle of this warp's 32 rows
-                    if (lane == 0 && i0 < p.P) {
+                    if (lane == 0 && i0 < p.P && !p.pw_seg_max) {
                         atomicMax(p.bu_max_ordered, ord);
                         p.bu_part_wsum[i0 >> 5] = ws;
                     }
@@ -1428,6 +1459,9 @@ struct T2Handle {
     T2Program belief;       // belief update: f_T + g per 256-particle unit
     T2Program belief_dual;  // the same with two units in flight per CTA pair (narrow models)
     bool has_belief = false, has_belief_dual = false;
+    // progressive widening: the belief program with the one-hot block in the operand (per-row actions)
+    T2Program pw, pw_dual;
+    bool has_pw = false, has_pw_dual = false;
     bool roll_x = false;    // rollout runs the 640-thread kernel (two sets of epilogue warps)
 };
 
@@ -1447,6 +1481,27 @@ void add_generator2(Builder2 &pb, const voila_mlp &f, int S, int A, int Nz, int 
                     b[(size_t)a * N + j] = f.b[0][j] + h_bf16_round(f.W[0][(size_t)j * K + S + a]);
             }
             pb.add_layer(W.data(), N, k0, b.data(), A, last ? last_epi : T2_EPI_HIDDEN, f.act);
+        } else {
+            pb.add_layer(f.W[l], N, K, f.b[l], 1, last ? last_epi : T2_EPI_HIDDEN, f.act);
+        }
+    }
+}
+
+// The same generator with the one-hot block kept in the operand, input order [s ; w ; onehot(a)]
+// (K = S + Nz + A): rows of a tile may carry different actions (progressive widening).
+void add_generator2_dense(Builder2 &pb, const voila_mlp &f, int S, int A, int Nz, int last_epi) {
+    for (int l = 0; l < f.n_layers; ++l) {
+        const int K = f.dims[l], N = f.dims[l + 1];
+        const bool last = l == f.n_layers - 1;
+        if (l == 0) {
+            const int k0 = S + Nz + A;
+            std::vector<float> W((size_t)N * k0);
+            for (int j = 0; j < N; ++j) {
+                for (int k = 0; k < S; ++k) W[(size_t)j * k0 + k] = f.W[0][(size_t)j * K + k];
+                for (int k = 0; k < Nz; ++k) W[(size_t)j * k0 + S + k] = f.W[0][(size_t)j * K + S + A + k];
+                for (int a = 0; a < A; ++a) W[(size_t)j * k0 + S + Nz + a] = f.W[0][(size_t)j * K + S + a];
+            }
+            pb.add_layer(W.data(), N, k0, f.b[0], 1, last ? last_epi : T2_EPI_HIDDEN, f.act);
         } else {
             pb.add_layer(f.W[l], N, K, f.b[l], 1, last ? last_epi : T2_EPI_HIDDEN, f.act);
         }
@@ -1517,7 +1572,8 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         !upload(pb.sbias_init.data(), pb.sbias_init.size() * sizeof(float), &g.d_sbias) ||
         !upload(pb.layers.data(), pb.layers.size() * sizeof(T2Layer), &g.d_layers) ||
         !upload(dev_tiles.data(), dev_tiles.size() * sizeof(T2TileDev), &g.d_tiles) ||
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem_bytes) != cudaSuccess)
+        // several programs share one kernel function: ask for the architectural maximum once
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem2) != cudaSuccess)
         return cudaGetErrorString(cudaGetLastError());
     // weight stream as a 2-D tensor [rows][64 bf16]; box = one ring stage (128 rows x 128 bytes).
     // The tiles are pre-swizzled on the host, so the copy itself does not swizzle.
@@ -1606,32 +1662,40 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         for (int l = 1; l <= d->f_T.n_layers; ++l) widest = std::max(widest, d->f_T.dims[l]);
         for (int l = 0; l <= d->lik_state.n_layers; ++l) widest = std::max(widest, l == 0 ? S : d->lik_state.dims[l]);
         const bool want_dual = widest <= 256 && !getenv("VOILA_T2_BELIEF_1SLOT");
-        for (int dual = 0; dual <= (want_dual ? 1 : 0); ++dual) {
-            Builder2 pb;
-            pb.policy = policy;
-            if (dual) pb.set_dual(4, 256);
-            add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
-            const voila_mlp &g = d->lik_state;
-            if (d->lik_action_cond) {
-                add_generator2(pb, g, S, A, 0, T2_EPI_SCORE);
-            } else {
-                for (int l = 0; l < g.n_layers; ++l)
-                    pb.add_layer(g.W[l], g.dims[l + 1], g.dims[l], g.b[l], 1,
-                                 l == g.n_layers - 1 ? T2_EPI_SCORE : T2_EPI_HIDDEN, g.act);
+        // pw = 1: the progressive-widening form (one-hot block in the operand; its layer-1 K is
+        // S + Nz + A); only without an action-conditioned state tower
+        for (int pw = 0; pw <= (d->lik_action_cond ? 0 : 1); ++pw) {
+            const int in_cols = S + Nz + (pw ? rup(A, 8) : 0);
+            if (pw && (A % 8 != 0 || in_cols > 512)) continue;
+            const bool dual_ok = want_dual && rup(in_cols, 64) / 64 <= 4;
+            for (int dual = 0; dual <= (dual_ok ? 1 : 0); ++dual) {
+                Builder2 pb;
+                pb.policy = policy;
+                if (dual) pb.set_dual(4, 256);
+                if (pw) add_generator2_dense(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
+                else add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
+                const voila_mlp &g = d->lik_state;
+                if (d->lik_action_cond) {
+                    add_generator2(pb, g, S, A, 0, T2_EPI_SCORE);
+                } else {
+                    for (int l = 0; l < g.n_layers; ++l)
+                        pb.add_layer(g.W[l], g.dims[l + 1], g.dims[l], g.b[l], 1,
+                                     l == g.n_layers - 1 ? T2_EPI_SCORE : T2_EPI_HIDDEN, g.act);
+                }
+                T2Program &prog = pw ? (dual ? h->pw_dual : h->pw) : (dual ? h->belief_dual : h->belief);
+                const int dd = g.dims[g.n_layers];
+                prog.hdr.g_in_chunks = rup(S, 64) / 64;
+                prog.hdr.e_pad = rup(dd, 16);
+                prog.hdr.e_off = (int)pb.sbias_init.size();
+                pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
+                const std::string m =
+                    dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(in_cols, 64) / 64, sm_count, allocs,
+                                          kT2ThreadsDual)
+                         : finish_program(pb, prog, belief_tc2_kernel, rup(in_cols, 64) / 64, sm_count, allocs);
+                // without a one-slot program the CUDA-core kernels serve the call
+                bool &flag = pw ? (dual ? h->has_pw_dual : h->has_pw) : (dual ? h->has_belief_dual : h->has_belief);
+                flag = m.empty();
             }
-            T2Program &prog = dual ? h->belief_dual : h->belief;
-            const int dd = g.dims[g.n_layers];
-            prog.hdr.g_in_chunks = rup(S, 64) / 64;
-            prog.hdr.e_pad = rup(dd, 16);
-            prog.hdr.e_off = (int)pb.sbias_init.size();
-            pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
-            const std::string m =
-                dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(S + Nz, 64) / 64, sm_count, allocs,
-                                      kT2ThreadsDual)
-                     : finish_program(pb, prog, belief_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
-            // without a one-slot program the CUDA-core propose+score kernel serves the belief update
-            if (dual) h->has_belief_dual = m.empty();
-            else h->has_belief = m.empty();
         }
     }
     return h;
@@ -1640,6 +1704,8 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
 void tc2_destroy(void *tc) { delete reinterpret_cast<T2Handle *>(tc); }
 
 bool tc2_has_belief(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_belief; }
+bool tc2_has_pw(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_pw; }
+int tc2_pw_e_stride(const void *tc) { return reinterpret_cast<const T2Handle *>(tc)->pw.hdr.e_pad; }
 
 namespace {
 T2Params base_params(const T2Program &g, const ModelDev &m) {
@@ -1716,6 +1782,41 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
     if (n_launches) *n_launches = 1;
+    return cudaGetLastError();
+}
+
+// Progressive widening, propose + score of every simulation (voila_pw_update) on the CTA-pair tcgen05
+// program: per-row actions (one-hot block in the operand), per-row tower embeddings, child maxima.
+cudaError_t launch_pw_propose_score_tc2(void *tc, const ModelDev &m, const PwArgs &a, const int32_t *sim_action,
+                                        const int32_t *sim_seg, cudaStream_t st, std::string *kernel_name) {
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    const bool dual = h->has_pw_dual && a.N > 2 * kT2Rows * h->pw.max_clusters;
+    const T2Program &g = dual ? h->pw_dual : h->pw;
+    T2Params p = base_params(g, m);
+    p.particles = reinterpret_cast<const uint16_t *>(a.particles);
+    p.weights = a.weights;
+    p.P = a.N; p.Q = 1; p.H = 1;
+    p.seed = a.seed;
+    const int unit_rows = 2 * kT2Rows * g.hdr.n_slots;
+    p.n_units = (a.N + unit_rows - 1) / unit_rows;
+    p.bu_action = 0;
+    p.bu_e = nullptr;
+    p.bu_proposals = reinterpret_cast<uint16_t *>(a.proposals);
+    p.bu_logits = a.logits;
+    p.bu_max_ordered = nullptr;
+    p.bu_part_wsum = nullptr;
+    p.inv_lambda = 1.0f / m.lambda;
+    p.d = m.mlp[3].dims[m.mlp[3].n_layers];
+    p.pw_sim_action = sim_action;
+    p.pw_sim_seg = sim_seg;
+    p.pw_E = a.E;
+    p.pw_seg_max = a.seg_max;
+    const int clusters = std::min(g.max_clusters, p.n_units);
+    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (kernel_name)
+        *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, per-row actions>"
+                            : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, per-row actions>";
     return cudaGetLastError();
 }
 

@@ -590,8 +590,8 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
 // ---- progressive widening ----
 namespace {
 struct PwLayout {
-    size_t sim_group, sim_branch, sim_rank, perm, seg_of_pos, seg_count, seg_off, new_src, seg_max, E, logits,
-        v_sorted, proposals, total;
+    size_t sim_group, sim_branch, sim_rank, perm, seg_of_pos, sim_action, sim_seg, seg_count, seg_off, new_src,
+        seg_max, E, logits, v_sorted, proposals, total;
 };
 PwLayout make_pw_layout(const voila_ctx *ctx, int N, int G, int M) {
     PwLayout L{};
@@ -608,6 +608,8 @@ PwLayout make_pw_layout(const voila_ctx *ctx, int N, int G, int M) {
     L.sim_rank = take((size_t)N * 4);
     L.perm = take((size_t)N * 4);
     L.seg_of_pos = take((size_t)N * 4);
+    L.sim_action = take((size_t)N * 4);
+    L.sim_seg = take((size_t)N * 4);
     L.seg_count = take(gm * 4);
     L.seg_off = take((gm + 1) * 4);
     L.new_src = take(gm * 4);
@@ -681,6 +683,8 @@ voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const
     a.sim_rank = reinterpret_cast<int32_t *>(w + L.sim_rank);
     a.perm = reinterpret_cast<int32_t *>(w + L.perm);
     a.seg_of_pos = reinterpret_cast<int32_t *>(w + L.seg_of_pos);
+    a.sim_action = reinterpret_cast<int32_t *>(w + L.sim_action);
+    a.sim_seg = reinterpret_cast<int32_t *>(w + L.sim_seg);
     a.seg_count = reinterpret_cast<int32_t *>(w + L.seg_count);
     a.seg_off = reinterpret_cast<int32_t *>(w + L.seg_off);
     a.new_src = reinterpret_cast<int32_t *>(w + L.new_src);
@@ -695,18 +699,30 @@ voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const
 
     const Layout SL = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
     const ScanBuffers sb = scan_buffers(ctx, SL);
+    // tensor-core path: one fused propose+score pass over all simulations (per-row actions and tower
+    // embeddings); the few rows that open a branch get their s' -> o on the CUDA cores first
+    const bool tc_path = use_tc2(ctx) && tc2_has_pw(ctx->tc2) && ctx->d % 16 == 0;
+    a.obs_from_particles = tc_path ? 1 : 0;
     cudaError_t e = launch_pw_widen(a, st);                                  // branches, children, sorted order
-    if (e == cudaSuccess) e = launch_pw_propose_ffma(ctx->model, a, bf16, st);  // s' of every simulation
+    if (e == cudaSuccess && !tc_path) e = launch_pw_propose_ffma(ctx->model, a, bf16, st);  // s' of every simulation
     if (e == cudaSuccess) e = launch_pw_obs_ffma(ctx->model, a, bf16, st);      // o of the opened branches
     if (e == cudaSuccess)                                                     // e = f(o) of every stored branch: one batch
         e = launch_mlp_forward_ffma(ctx->model, 2, branch_obs, G * M_max, a.E, bf16, st);
-    if (e == cudaSuccess) e = launch_pw_score_ffma(ctx->model, a, bf16, st);    // L_i, child maxima
+    if (e == cudaSuccess) {                                                   // L_i, child maxima
+        ProfScope prof(ctx, VOILA_K_PROPOSE, st);
+        if (tc_path) {
+            e = launch_pw_propose_score_tc2(ctx->tc2, ctx->model, a, a.sim_action, a.sim_seg, st, &ctx->last_belief_kernel);
+        } else {
+            e = launch_pw_score_ffma(ctx->model, a, bf16, st);
+            ctx->last_belief_kernel = bf16 ? "pw_propose/score_ffma_kernel<bf16>" : "pw_propose/score_ffma_kernel<fp32>";
+        }
+    }
     if (e == cudaSuccess) e = launch_pw_weights(a, st);                       // v in sorted order
     if (e == cudaSuccess) e = launch_bu_init(sb, N, st);
     if (e == cudaSuccess) e = launch_weight_scan(sb, a.v_sorted, N, false, nullptr, st);  // uint64 CDF over the sorted order
     if (e == cudaSuccess) e = launch_pw_resample(a, sb.cdf, ctx->S * (int)esize, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    ctx->launches += 11 + (seg_status_out ? 1 : 0);
+    ctx->launches += (tc_path ? 10 : 11) + (seg_status_out ? 1 : 0);
     return VOILA_OK;
 }
 

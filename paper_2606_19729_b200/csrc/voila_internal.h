@@ -86,6 +86,8 @@ struct PwArgs {
     uint64_t seed;
     // workspace
     int32_t *sim_group, *sim_branch, *sim_rank, *perm, *seg_of_pos;  // [N]
+    int32_t *sim_action, *sim_seg;                                  // [N] action / child index of every simulation
+    int obs_from_particles;  // 1: the sampled observations of opened branches recompute s' (no stored proposals yet)
     int32_t *seg_count, *seg_off, *new_src;                         // [G*M_max] (+1 for seg_off)
     int *seg_max;                                                   // [G*M_max] ordered-int maxima
     float *E;                                                       // [G*M_max][d] tower embeddings
