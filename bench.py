@@ -153,8 +153,10 @@ def _oracle_one_thread(cfg, model, inp, target_s=2.0):
 
 
 def _porpp_leg(ctx, dev, peaks):
-    """one level of the PORPP preference backup (Eq. 1) on a wide synthetic level:
-    2^18 belief nodes x 16 actions x 4 observation branches (inputs 200 MB > L2)."""
+    """the PORPP preference backup (Eq. 1) on a wide synthetic level: 2^18 belief nodes x
+    16 actions x 4 observation branches, the children numbered in creation order as the tree tensors
+    grow (every belief node of the next level has exactly one parent), plus the same level with
+    scattered child indices (a worst case no tree produces).  One voila_porpp_backup call each."""
     import torch
     nb, A, B = 1 << 18, 16, 4
     na = nb * A
@@ -163,25 +165,36 @@ def _porpp_leg(ctx, dev, peaks):
     lv = dict(R=torch.randn((nb, A), generator=g, device=dev),
               logpi0=torch.full((nb, A), -float(np.log(A)), device=dev),
               child_off=torch.arange(0, na * B + 1, B, dtype=torch.int32, device=dev),
-              child_idx=torch.randint(0, 1 << 20, (na * B,), generator=g, device=dev, dtype=torch.int32),
+              child_idx=torch.arange(0, na * B, dtype=torch.int32, device=dev),
               child_w=torch.full((na * B,), 1.0 / B, device=dev))
-    leaves = torch.randn(1 << 20, generator=g, device=dev)
-    for _ in range(3):
-        ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize(dev)
-    a.record()
-    for _ in range(10):
-        ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
-    b.record()
-    torch.cuda.synchronize(dev)
-    ms = a.elapsed_time(b) / 10
-    bytes_alg = na * 16 + na * B * 8 + nb * 4  # R, log pi0, row offset, Psi out; index + weight per branch; V out
-    gbs = bytes_alg / (ms * 1e-3) / 1e9
-    return {"workload": f"{nb} belief nodes x {A} actions x {B} branches, one level", "latency_us": 1e3 * ms,
-            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                         "frac": gbs / peaks["hbm_gbs"], "bytes_per_action_node": bytes_alg / na,
-                         "note": "random 4-byte gathers of V(child) (L2-resident) bound it, not HBM"}}
+    leaves = torch.randn(na * B, generator=g, device=dev)
+    out = {}
+    for name in ("tree", "scattered"):
+        if name == "scattered":
+            lv = dict(lv, child_idx=torch.randint(0, 1 << 20, (na * B,), generator=g, device=dev, dtype=torch.int32))
+        for _ in range(3):
+            ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        a.record()
+        for _ in range(10):
+            ctx.voila_porpp_backup([lv], leaves, 2.0, 0.95)
+        b.record()
+        torch.cuda.synchronize(dev)
+        ms = a.elapsed_time(b) / 10
+        # R, log pi0, row offset, Psi out per action node; index + weight (+ V(child), read once in a tree) per
+        # branch; V and the root action out per belief node
+        per_branch = 12 if name == "tree" else 8
+        bytes_alg = na * 16 + na * B * per_branch + nb * 8
+        gbs = bytes_alg / (ms * 1e-3) / 1e9
+        out[name] = {"latency_us": 1e3 * ms,
+                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                  "frac": gbs / peaks["hbm_gbs"], "bytes_per_action_node": bytes_alg / na}}
+    out["scattered"]["roofline"]["note"] = ("child indices drawn at random over 2^20 nodes: 4-byte gathers cost a "
+                                            "32-byte L2 sector each; V(child) is L2-resident and not counted")
+    return {"workload": f"{nb} belief nodes x {A} actions x {B} branches, one level, root action",
+            "latency_us": out["tree"]["latency_us"], "roofline": out["tree"]["roofline"],
+            "scattered_children": out["scattered"]}
 
 
 def _belief_roofs(N, row_bytes, kt, flop_particle, peaks, belief_kernel, unique_frac=None):
@@ -325,6 +338,64 @@ def _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush, calls=5):
                         "kernel_ms": k_ms, "flop_per_unit": flop, "units_per_launch": units,
                         "nominal_peak": 2250.0, "frac_of_nominal": tf / 2250.0,
                         "peak_kind": f"bf16 burst, {peaks['src']}"}}
+    ctx.close()
+    return leg
+
+
+def _leg_pw(vl, synth, dev, local, peaks, flush, calls=10):
+    """vectorised progressive widening with batched likelihood on the
+    quadruped-shaped model (config 3): 2^18 parallel simulations grouped under 2048 action nodes of
+    ragged size, up to 16 observation branches per node, half of them open before the call."""
+    import torch
+    cfg = synth.CONFIGS[3]
+    model = synth.make_model(cfg)
+    N, G, M = 1 << 18, 2048, 16
+    rng = np.random.default_rng(20260619 + 77)
+    parts_np = rng.standard_normal((N, cfg.S)).astype(np.float32)
+    cuts = np.concatenate([[0], np.sort(rng.integers(0, N + 1, G - 1)), [N]]).astype(np.int32)
+    acts = rng.integers(0, cfg.A, G).astype(np.int32)
+    bc0 = rng.integers(0, M // 2 + 1, G).astype(np.int32)
+    vc0 = (bc0 * 8).astype(np.int32)
+    bo0 = rng.standard_normal((G, M, cfg.O)).astype(np.float32)
+    ctx = vl.Voila(model, device=local)
+    parts = ctx.to_particles(parts_np)
+    t = lambda a: torch.from_numpy(a).to(dev)
+    go, ga = t(cuts), t(acts)
+
+    def call(k):
+        return ctx.voila_pw_update(parts, go, ga, t(vc0), t(bc0), t(bo0), 1.5, 0.5, None, 9000 + k, want_debug=False)
+
+    for k in range(3):
+        out = call(k)
+    torch.cuda.synchronize(dev)
+    ctx.voila_set_profiling(True)
+    ctx.voila_profile_read(1)
+    l0 = ctx.voila_launch_count()
+    stream = torch.cuda.current_stream(dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+    for k in range(calls):
+        vc, bc, bo = t(vc0), t(bc0), t(bo0)
+        flush.fill_(k & 0xFF)
+        ev[k][0].record(stream)
+        out = ctx.voila_pw_update(parts, go, ga, vc, bc, bo, 1.5, 0.5, None, 9100 + k, want_debug=False)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize(dev)
+    ms = [a.elapsed_time(b) for a, b in ev]
+    kt = ctx.voila_profile_read(1)
+    launches = (ctx.voila_launch_count() - l0) / calls
+    ctx.voila_set_profiling(False)
+    assert int(out["seg_status"].sum().item()) == 0
+    flop = synth.flops_per_belief_particle(model)
+    leg = {"workload": f"{N} simulations, {G} action nodes (ragged), M_max={M}, config-3 model",
+           "latency_us": 1e3 * float(np.mean(ms)), "simulations_per_s": N / (float(np.mean(ms)) * 1e-3),
+           "branches_opened": int((bc.cpu().numpy() - bc0).sum()), "gpu_launches_per_call": launches,
+           "propose_score_us": 1e3 * float(np.mean(kt)) if kt else None, "kernel": ctx.voila_last_belief_kernel()}
+    if kt and "belief_tc2" in ctx.voila_last_belief_kernel():
+        tf = N * flop / (np.mean(kt) * 1e-3) / 1e12
+        leg["propose_score_roofline"] = {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_burst"],
+                                         "unit": "TFLOP/s", "frac": tf / peaks["bf16_burst"],
+                                         "flop_per_simulation": flop, "nominal_peak": 2250.0,
+                                         "frac_of_nominal": tf / 2250.0}
     ctx.close()
     return leg
 
@@ -553,6 +624,7 @@ def run_voila(args):
         # defined on config 4 (2^20 particles), the paper-shaped rollout on config 3
         extra["belief_update_cfg4"] = _leg_belief_cfg4(vl, synth, dev, local, peaks, flush)
         extra["rollout_cfg3"] = _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush)
+        extra["progressive_widening"] = _leg_pw(vl, synth, dev, local, peaks, flush)
 
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     cpu_1t = _oracle_one_thread(cfg, model, inp)

@@ -224,6 +224,29 @@ voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const floa
                                       const float *v_next, int n_belief, int n_actions, float eta, float gamma,
                                       float *psi_out, float *v_out, void *cuda_stream);
 
+/* The preference backup of a WHOLE belief tree in one call, and the root action (VOPP
+ * stores the tree as "a collection of tensors storing belief nodes, action nodes, and action
+ * preferences" and interleaves forward search with "fully vectorized preference backup"; the planner
+ * then acts on the root preferences).  levels is a HOST array of n_levels records holding DEVICE
+ * pointers, level 0 = the root level; level d's observation branches index the belief nodes of level
+ * d + 1 (the last level's index leaf_values).  Levels are backed up deepest first on the stream, each
+ * level's v_out feeding the level above; psi_out / v_out of every level are written.
+ *   root_action_out dev [levels[0].n_belief] int32 or NULL: argmax_a Psi(b0, a), ties -> lowest a,
+ *                   a NaN preference never wins.
+ * Errors as voila_porpp_backup_level, plus n_levels < 1. */
+typedef struct {
+    const float *R, *logpi0;     /* dev [n_belief * n_actions] */
+    const int32_t *child_off;    /* dev [n_belief * n_actions + 1] */
+    const int32_t *child_idx;    /* dev [child_off[last]] or NULL */
+    const float *child_w;        /* dev [child_off[last]] or NULL */
+    int n_belief;
+    float *psi_out;              /* dev [n_belief * n_actions] */
+    float *v_out;                /* dev [n_belief] */
+} voila_porpp_level;
+voila_status voila_porpp_backup(voila_ctx *ctx, const voila_porpp_level *levels, int n_levels, int n_actions,
+                                const float *leaf_values, float eta, float gamma, int32_t *root_action_out,
+                                void *cuda_stream);
+
 /* Root action selection for an open-loop sequence sweep: q* = argmax_q values[q] (ties -> lowest q,
  * NaN never wins), best_action_out[0] = action_seqs[q*][0], best_q_out[0] = q* (the
  * planner returns an action for the current belief; DESIGN.md input recipe, config 5).

@@ -26,6 +26,20 @@ def log_sum_exp_eta(psi, eta):
     return float(m + np.log(np.sum(np.exp(eta * (psi - m)))) / eta)
 
 
+def root_action(psi_root):
+    """argmax_a Psi(b0, a) for every root belief (ties -> lowest a): the action the planner returns for
+    the current belief (the preferences Psi ARE the policy's scores)."""
+    psi_root = np.asarray(psi_root, np.float64)
+    out = np.zeros(psi_root.shape[0], np.int32)
+    for b in range(psi_root.shape[0]):
+        best = -1
+        for a in range(psi_root.shape[1]):  # a NaN preference never wins; all NaN -> action 0
+            if psi_root[b, a] == psi_root[b, a] and (best < 0 or psi_root[b, a] > psi_root[b, best]):
+                best = a
+        out[b] = max(best, 0)
+    return out
+
+
 def porpp_backup(levels, leaf_values, eta, gamma):
     """levels[d] = dict(R [nb, A], logpi0 [nb, A], child_off [nb*A + 1], child_idx [nnz], child_w [nnz]);
     leaf_values [number of belief nodes below the last action level] (may be empty).

@@ -743,6 +743,32 @@ voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const floa
     return VOILA_OK;
 }
 
+voila_status voila_porpp_backup(voila_ctx *ctx, const voila_porpp_level *levels, int n_levels, int n_actions,
+                                const float *leaf_values, float eta, float gamma, int32_t *root_action_out,
+                                void *cuda_stream) {
+    if (!ctx || !levels || n_levels < 1 || n_actions < 1) return VOILA_ERR_INVALID_ARG;
+    if (!(eta > 0.0f) || !(gamma >= 0.0f)) return VOILA_ERR_INVALID_ARG;
+    for (int d = 0; d < n_levels; ++d) {
+        const voila_porpp_level &lv = levels[d];
+        if (!lv.R || !lv.logpi0 || !lv.child_off || !lv.psi_out || !lv.v_out || lv.n_belief < 1)
+            return VOILA_ERR_INVALID_ARG;
+        if ((long long)lv.n_belief * n_actions >= (1ll << 31)) return VOILA_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const float *v_next = leaf_values;
+    for (int d = n_levels - 1; d >= 0; --d) {
+        const voila_porpp_level &lv = levels[d];
+        const cudaError_t e = launch_porpp_backup_level(lv.R, lv.logpi0, lv.child_off, lv.child_idx, lv.child_w, v_next,
+                                                        lv.n_belief, n_actions, eta, gamma, lv.psi_out, lv.v_out, st,
+                                                        d == 0 ? root_action_out : nullptr);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 1;
+        v_next = lv.v_out;
+    }
+    return VOILA_OK;
+}
+
 voila_status voila_mlp_forward(voila_ctx *ctx, int which, const float *x, int rows, float *y,
                                void *cuda_stream) {
     if (!ctx || which < 0 || which > 3 || !x || !y || rows < 1) return VOILA_ERR_INVALID_ARG;

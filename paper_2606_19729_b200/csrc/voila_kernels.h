@@ -63,7 +63,7 @@ cudaError_t launch_pw_resample(const PwArgs &a, const unsigned long long *cdf, i
 cudaError_t launch_porpp_backup_level(const float *R, const float *logpi0, const int32_t *child_off,
                                       const int32_t *child_idx, const float *child_w, const float *v_next,
                                       int n_belief, int A, float eta, float gamma, float *psi_out, float *v_out,
-                                      cudaStream_t st);
+                                      cudaStream_t st, int32_t *argmax_out = nullptr);
 
 // ---- rollout_tc.cu : tcgen05 / TMEM / bulk-copy path (bf16 mode) ----
 bool tc_supported(const voila_model_desc *desc, std::string *why);

@@ -27,6 +27,7 @@ EXPORTS = [
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read", "voila_pw_workspace_bytes", "voila_pw_reserve", "voila_pw_update",
+    "voila_porpp_backup",
 ]
 
 
@@ -49,6 +50,11 @@ class _Terminal(C.Structure):
     _fields_ = [("n_regions", C.c_int), ("dims", C.POINTER(C.c_int)), ("centers", C.POINTER(C.c_float)),
                 ("radii", C.POINTER(C.c_float)), ("rewards", C.POINTER(C.c_float)),
                 ("stops", C.POINTER(C.c_int))]
+
+
+class _PorppLevel(C.Structure):
+    _fields_ = [("R", C.c_void_p), ("logpi0", C.c_void_p), ("child_off", C.c_void_p), ("child_idx", C.c_void_p),
+                ("child_w", C.c_void_p), ("n_belief", C.c_int), ("psi_out", C.c_void_p), ("v_out", C.c_void_p)]
 
 
 class _ModelDesc(C.Structure):
@@ -126,6 +132,8 @@ def load_library():
     lib.voila_pw_update.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp, i32, C.c_double, C.c_double, vp, u64,
                                     vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.voila_pw_update.restype = i32
+    lib.voila_porpp_backup.argtypes = [vp, C.POINTER(_PorppLevel), i32, i32, vp, C.c_float, C.c_float, vp, vp]
+    lib.voila_porpp_backup.restype = i32
     lib.voila_version.argtypes = []
     lib.voila_version.restype = i32
     _LIB = lib
@@ -409,28 +417,38 @@ class Voila:
                                                _dptr(bq), _dptr(ba), self._stream()), "voila_best_action")
         return bq, ba
 
-    def voila_porpp_backup(self, levels, leaf_values, eta, gamma):
+    def voila_porpp_backup(self, levels, leaf_values, eta, gamma, per_level_calls=False):
         """PORPP preference backup (Eq. 1) of a whole tree: `levels[d]` = dict of device tensors
-        R, logpi0 [nb, A] fp32, child_off [nb*A+1] int32, child_idx int32, child_w fp32; one
-        voila_porpp_backup_level call per level, deepest first.  -> (V, Psi) lists over depth."""
+        R, logpi0 [nb, A] fp32, child_off [nb*A+1] int32, child_idx int32, child_w fp32.  One
+        voila_porpp_backup call for the tree (per_level_calls=True: one voila_porpp_backup_level call
+        per level, deepest first).  -> (V, Psi, root_action): lists over depth, int32 [root beliefs]."""
         torch = self._torch
         D = len(levels)
-        V, Psi = [None] * D, [None] * D
-        v_next = leaf_values
-        for d in range(D - 1, -1, -1):
-            lv = levels[d]
-            nb, A = lv["R"].shape
-            psi = torch.empty((nb, A), dtype=torch.float32, device=lv["R"].device)
-            v = torch.empty(nb, dtype=torch.float32, device=lv["R"].device)
-            self._check(self.lib.voila_porpp_backup_level(
-                self._h, _dptr(lv["R"]), _dptr(lv["logpi0"]), _dptr(lv["child_off"]),
-                _dptr(lv["child_idx"] if lv["child_idx"].numel() else None),
-                _dptr(lv["child_w"] if lv["child_w"].numel() else None),
-                _dptr(v_next if v_next is not None and v_next.numel() else None), nb, A,
-                C.c_float(eta), C.c_float(gamma), _dptr(psi), _dptr(v), self._stream()), "voila_porpp_backup_level")
-            V[d], Psi[d] = v, psi
-            v_next = v
-        return V, Psi
+        dev = levels[0]["R"].device
+        A = levels[0]["R"].shape[1]
+        V = [torch.empty(lv["R"].shape[0], dtype=torch.float32, device=dev) for lv in levels]
+        Psi = [torch.empty(lv["R"].shape, dtype=torch.float32, device=dev) for lv in levels]
+        opt = lambda t: _dptr(t if t is not None and t.numel() else None)
+        raw = lambda t: None if t is None or not t.numel() else t.data_ptr()
+        if per_level_calls:
+            v_next = leaf_values
+            for d in range(D - 1, -1, -1):
+                lv = levels[d]
+                nb = lv["R"].shape[0]
+                self._check(self.lib.voila_porpp_backup_level(
+                    self._h, _dptr(lv["R"]), _dptr(lv["logpi0"]), _dptr(lv["child_off"]), opt(lv["child_idx"]),
+                    opt(lv["child_w"]), opt(v_next), nb, A, C.c_float(eta), C.c_float(gamma), _dptr(Psi[d]),
+                    _dptr(V[d]), self._stream()), "voila_porpp_backup_level")
+                v_next = V[d]
+            return V, Psi, None
+        arr = (_PorppLevel * D)()
+        for d, lv in enumerate(levels):
+            arr[d] = _PorppLevel(raw(lv["R"]), raw(lv["logpi0"]), raw(lv["child_off"]), raw(lv["child_idx"]),
+                                 raw(lv["child_w"]), int(lv["R"].shape[0]), raw(Psi[d]), raw(V[d]))
+        root = torch.empty(levels[0]["R"].shape[0], dtype=torch.int32, device=dev)
+        self._check(self.lib.voila_porpp_backup(self._h, arr, D, A, opt(leaf_values), C.c_float(eta), C.c_float(gamma),
+                                                _dptr(root), self._stream()), "voila_porpp_backup")
+        return V, Psi, root
 
     # -- host-buffer variants (pinned torch CPU tensors or numpy arrays) --------------------------
     def voila_rollout_values_host(self, particles, action_seqs, weights, seed, values_out,

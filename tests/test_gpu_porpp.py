@@ -34,12 +34,23 @@ def test_porpp_backup_matches_oracle(oracle, seed, depth, A, branches, roots, et
     V_ref, Psi_ref = po.porpp_backup(levels, leaves, eta, 0.95)
     ctx = vl.Voila(synth.make_model(synth.CONFIGS[1]))
     dl, dleaves = _to_dev(torch, levels, leaves)
-    V, Psi = ctx.voila_porpp_backup(dl, dleaves, eta, 0.95)
+    # the whole tree in ONE C-ABI call (with the root action), and level by level: same numbers
+    V, Psi, root = ctx.voila_porpp_backup(dl, dleaves, eta, 0.95)
+    V2, Psi2, _ = ctx.voila_porpp_backup(dl, dleaves, eta, 0.95, per_level_calls=True)
     torch.cuda.synchronize()
     for d in range(depth):
         scale = max(1.0, float(np.max(np.abs(V_ref[d]))))
         assert np.max(np.abs(t2n(V[d]) - V_ref[d])) <= TOL_FP32 * scale, f"V level {d}"
         assert np.max(np.abs(t2n(Psi[d]) - Psi_ref[d])) <= TOL_FP32 * scale, f"Psi level {d}"
+        assert torch.equal(V[d], V2[d]) and torch.equal(Psi[d], Psi2[d])
+    # root action: the argmax of the GPU's own root preferences (an integer decided in fp32, ties -> lowest
+    # a), and the oracle's action wherever its two best preferences are further apart than the tolerance
+    psi0 = t2n(Psi[0])
+    assert np.array_equal(root.cpu().numpy(), po.root_action(psi0))
+    ref_root = po.root_action(Psi_ref[0])
+    srt = np.sort(Psi_ref[0], axis=1)
+    clear = (srt[:, -1] - srt[:, -2] > 1e-3 * max(1.0, float(np.abs(Psi_ref[0]).max()))) if A > 1 else np.ones(roots, bool)
+    assert np.array_equal(root.cpu().numpy()[clear], ref_root[clear])
     ctx.close()
 
 

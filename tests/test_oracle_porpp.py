@@ -89,3 +89,28 @@ def test_single_action_and_no_children():
                    child_idx=np.zeros(0, np.int32), child_w=np.zeros(0))]
     V, Psi = po.porpp_backup(levels, np.zeros(0), 3.0, 0.9)
     assert V[0][0] == 1.5 and Psi[0][0, 0] == 1.5
+
+
+def test_root_action_is_the_greedy_action_of_the_max_backup():
+    """eta -> infinity: argmax_a Psi(b0, a) is the greedy action of value iteration on the tree (computed
+    independently here with numpy); for finite eta it is numpy's argmax of the root preferences, ties -> lowest a."""
+    for seed in (3, 5, 9):
+        levels, leaves = synth_tree.make_tree(seed, depth=3, n_actions=5, max_branches=3, root_beliefs=4)
+        V, Psi = po.porpp_backup(levels, leaves, 1e4, 0.9)
+        v_next = np.asarray(leaves, np.float64)
+        for d in range(len(levels) - 1, -1, -1):
+            lv = levels[d]
+            nb, A = lv["R"].shape
+            q = np.zeros((nb, A))
+            for j in range(nb * A):
+                s = slice(lv["child_off"][j], lv["child_off"][j + 1])
+                q[j // A, j % A] = lv["R"][j // A, j % A] + 0.9 * np.dot(lv["child_w"][s], v_next[lv["child_idx"][s]])
+            v_next = q.max(axis=1)
+        srt = np.sort(q, axis=1)
+        clear = srt[:, -1] - srt[:, -2] > 1e-2
+        assert clear.any()
+        assert np.array_equal(po.root_action(Psi[0])[clear], q.argmax(axis=1)[clear])
+        _, Psi2 = po.porpp_backup(levels, leaves, 2.0, 0.9)
+        assert np.array_equal(po.root_action(Psi2[0]), np.argmax(Psi2[0], axis=1))
+    tie = np.array([[1.0, 3.0, 3.0, -1.0], [np.nan, 0.5, 0.5, 0.2]])
+    assert po.root_action(tie).tolist() == [1, 1]
