@@ -19,7 +19,7 @@ constexpr int kPsiRegs = 4;  // preferences kept in registers per lane (A <= 4 G
 
 // G = lanes per belief node: the power of two >= A (capped at 32; A > 32 strides over the lanes),
 // so a warp serves 32 / G belief nodes and narrow action sets (|A| = 4 ... 16) keep every lane busy.
-__global__ void __launch_bounds__(256) porpp_backup_level_kernel(const float *__restrict__ R,
+__global__ void __launch_bounds__(256, 8) porpp_backup_level_kernel(const float *__restrict__ R,
                                                                  const float *__restrict__ logpi0,
                                                                  const int32_t *__restrict__ child_off,
                                                                  const int32_t *__restrict__ child_idx,
@@ -37,36 +37,41 @@ __global__ void __launch_bounds__(256) porpp_backup_level_kernel(const float *__
     float m = -INFINITY;
     int am = 0x7fffffff;
     float psi_reg[kPsiRegs];
-    if (live) {
-        int slot = 0;
-        for (int a = a0; a < A; a += G, ++slot) {
-            const int j = b * A + a;
-            const int c0 = __ldg(child_off + j), c1 = __ldg(child_off + j + 1);
-            float fut = 0.0f;
-            for (int c = c0; c < c1; c += 4) {
-                int idx[4];
-                float w[4], v[4];
+    auto preference = [&](int a) {
+        const int j = b * A + a;
+        const int c0 = __ldg(child_off + j), c1 = __ldg(child_off + j + 1);
+        float fut = 0.0f;
+        for (int c = c0; c < c1; c += 4) {
+            int idx[4];
+            float w[4], v[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (c + u < c1) {
-                        idx[u] = __ldg(child_idx + c + u);
-                        w[u] = __ldg(child_w + c + u);
-                    }
+            for (int u = 0; u < 4; ++u)
+                if (c + u < c1) {
+                    idx[u] = __ldg(child_idx + c + u);
+                    w[u] = __ldg(child_w + c + u);
+                }
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (c + u < c1) v[u] = __ldg(v_next + idx[u]);
+            for (int u = 0; u < 4; ++u)
+                if (c + u < c1) v[u] = __ldg(v_next + idx[u]);
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (c + u < c1) fut = fmaf(w[u], v[u], fut);
-            }
-            const float psi = fmaf(__ldg(logpi0 + j), inv_eta, __ldg(R + j)) + gamma * fut;
-            __stcs(psi_out + j, psi);
-            if (slot < kPsiRegs) psi_reg[slot] = psi;
-            if (psi == psi && (am == 0x7fffffff || psi > m)) {  // first maximum (a ascends); a NaN never wins
-                m = psi;
-                am = a;
-            }
+            for (int u = 0; u < 4; ++u)
+                if (c + u < c1) fut = fmaf(w[u], v[u], fut);
         }
+        const float psi = fmaf(__ldg(logpi0 + j), inv_eta, __ldg(R + j)) + gamma * fut;
+        __stcs(psi_out + j, psi);
+        if (psi == psi && (am == 0x7fffffff || psi > m)) {  // first maximum (a ascends); a NaN never wins
+            m = psi;
+            am = a;
+        }
+        return psi;
+    };
+    if (live) {
+#pragma unroll
+        for (int slot = 0; slot < kPsiRegs; ++slot) {  // compile-time slots: the array stays in registers
+            const int a = a0 + slot * G;
+            psi_reg[slot] = a < A ? preference(a) : 0.0f;
+        }
+        for (int a = a0 + kPsiRegs * G; a < A; a += G) preference(a);
     }
     for (int o = G >> 1; o > 0; o >>= 1) {
         const float mo = __shfl_xor_sync(0xffffffffu, m, o);
@@ -80,11 +85,10 @@ __global__ void __launch_bounds__(256) porpp_backup_level_kernel(const float *__
     const bool finite = m > -INFINITY && m < INFINITY;
     float s = 0.0f;
     if (live && finite) {
-        int slot = 0;
-        for (int a = a0; a < A; a += G, ++slot) {
-            const float psi = slot < kPsiRegs ? psi_reg[slot] : psi_out[b * A + a];
-            s += expf(eta * (psi - m));
-        }
+#pragma unroll
+        for (int slot = 0; slot < kPsiRegs; ++slot)
+            if (a0 + slot * G < A) s += expf(eta * (psi_reg[slot] - m));
+        for (int a = a0 + kPsiRegs * G; a < A; a += G) s += expf(eta * (psi_out[b * A + a] - m));
     }
     for (int o = G >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (live && a0 == 0) {
