@@ -68,6 +68,8 @@ typedef VO_REAL real;
 #define VO_STREAM_RESAMPLE 4u
 #define VO_STREAM_PW_OBS 5u    /* progressive widening: noise of the sampled observation o_i */
 #define VO_STREAM_PW_ATTACH 6u /* progressive widening: word that picks an existing branch */
+#define VO_STREAM_DIFFUSION 7u /* diffusion teacher: the initial noise x_1 = omega */
+#define VO_TEMB 8              /* width of the diffusion-time embedding (reading R31) */
 
 typedef struct {
     int n_layers;                 /* number of affine layers */
@@ -79,7 +81,7 @@ typedef struct {
 
 typedef struct {
     int S, O, A, Nz;
-    vo_mlp mlp[4]; /* 0: f_T, 1: f_Z, 2: obs tower f, 3: state tower g */
+    vo_mlp mlp[6]; /* 0: f_T, 1: f_Z, 2: obs tower f, 3: state tower g, 4 / 5: diffusion teachers' denoisers v_T / v_Z */
     int lik_action_cond;
     float lambda, gamma;
     int reward_kind;
@@ -182,7 +184,7 @@ vo_model *vo_model_create(int S, int O, int A, int Nz, int lik_action_cond, floa
  * fp32 parameters concatenated in layer order (W[l] is [out][in] row-major). */
 int vo_model_set_mlp(vo_model *m, int which, int n_layers, const int *dims, int act,
                      const float *W_flat, const float *b_flat) {
-    if (which < 0 || which > 3 || n_layers < 1 || n_layers > VO_MAX_LAYERS) return -1;
+    if (which < 0 || which > 5 || n_layers < 1 || n_layers > VO_MAX_LAYERS) return -1;
     vo_mlp *f = &m->mlp[which];
     f->n_layers = n_layers; f->act = act;
     for (int l = 0; l <= n_layers; ++l) f->dims[l] = dims[l];
@@ -250,7 +252,7 @@ int vo_model_set_terminal(vo_model *m, int n, const int *dims, const float *cent
 void vo_model_set_emulate_bf16(vo_model *m, int on) {
     m->emulate_bf16 = on;
     if (!on) return;
-    for (int w = 0; w < 4; ++w)
+    for (int w = 0; w < 6; ++w)
         for (int l = 0; l < m->mlp[w].n_layers; ++l) {
             size_t nw = (size_t)m->mlp[w].dims[l] * m->mlp[w].dims[l + 1];
             for (size_t i = 0; i < nw; ++i) m->mlp[w].W[l][i] = (real)bf16_round((float)m->mlp[w].W[l][i]);
@@ -259,7 +261,7 @@ void vo_model_set_emulate_bf16(vo_model *m, int on) {
 
 void vo_model_destroy(vo_model *m) {
     if (!m) return;
-    for (int w = 0; w < 4; ++w)
+    for (int w = 0; w < 6; ++w)
         for (int l = 0; l < VO_MAX_LAYERS; ++l) { free(m->mlp[w].W[l]); free(m->mlp[w].b[l]); }
     for (int k = 0; k < VO_MAX_TERM; ++k) free(m->term_center[k]);
     free(m->reward_param); free(m->action_cost); free(m);
@@ -306,7 +308,7 @@ static void mlp_forward_one(const vo_mlp *f, int emulate_bf16, const real *x, re
 
 /* rows of x ([rows][dims[0]]) -> rows of y ([rows][dims[n_layers]]), fp32 in/out. */
 int vo_mlp_forward(const vo_model *m, int which, const float *x, int rows, float *y) {
-    if (which < 0 || which > 3) return -1;
+    if (which < 0 || which > 5 || m->mlp[which].n_layers < 1) return -1;
     const vo_mlp *f = &m->mlp[which];
     int w = mlp_max_width(f), K0 = f->dims[0], NL = f->dims[f->n_layers];
     real *b0 = (real *)malloc(sizeof(real) * w * 4), *b1 = b0 + w, *xi = b1 + w, *yo = xi + w;
@@ -389,7 +391,7 @@ typedef struct { real *x, *b0, *b1, *s, *sn, *o; float *omega; } scratch;
 static scratch scratch_alloc(const vo_model *m) {
     scratch z;
     int w = 1;
-    for (int i = 0; i < 4; ++i) { int v = mlp_max_width(&m->mlp[i]); if (v > w) w = v; }
+    for (int i = 0; i < 6; ++i) { int v = mlp_max_width(&m->mlp[i]); if (v > w) w = v; }
     if (m->S + m->A + m->Nz > w) w = m->S + m->A + m->Nz;
     z.x = (real *)malloc(sizeof(real) * w * 6);
     z.b0 = z.x + w; z.b1 = z.b0 + w; z.s = z.b1 + w; z.sn = z.s + w; z.o = z.sn + w;
@@ -836,6 +838,63 @@ int vo_pw_update(const vo_model *m, const float *particles, int N, const int32_t
     if (logits_out) memcpy(logits_out, L, sizeof(float) * (size_t)N);
     if (post_weights_out) memcpy(post_weights_out, v, sizeof(float) * (size_t)N);
     free(prop); free(obs); free(L); free(v); free(br); free(anc); free(gid);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * f4. The diffusion teacher's sampler: the conditional denoiser
+ * v(c, a, x_tau, tau) is trained with the v-prediction objective on x_tau = sqrt(abar) x_0 +
+ * sqrt(1 - abar) eps with a cosine schedule, and samples are drawn with an
+ * "ODE-based diffusion sampler [27]" (DDIM) from the latent noise omega.
+ * Readings R30-R32: abar_tau = cos^2(pi tau / 2), i.e. alpha = cos(pi tau / 2), sigma = sin(pi tau / 2);
+ * denoiser input [c ; onehot(a) ; x_tau ; temb(tau)] with temb = (sin(pi 2^k tau), cos(pi 2^k tau))_{k<4};
+ * uniform grid tau_k = 1 - k / K, x at tau_0 = 1 is omega ~ N(0, I_D) (Philox stream 7, counter (i,0,0));
+ * for k = 0 .. K-1 (one denoiser call each):
+ *     v = v_theta(c, a, x, tau_k);  x0_hat = alpha x - sigma v;  eps_hat = sigma x + alpha v   (v-prediction)
+ *     x <- alpha' x0_hat + sigma' eps_hat                                   (DDIM, eta = 0; ' = at tau_{k+1})
+ * and x at tau_K = 0 is the sample.  which = 0: transition teacher (c = s, D = S), 1: observation
+ * teacher (c = s', D = O).  cond [N][S], actions [N], out [N][D]; traj_out [K+1][D] or NULL: the path
+ * of sample `traj_row`.  Returns 0, -1 bad arguments / no such denoiser.
+ * ---------------------------------------------------------------------------------------- */
+int vo_diffusion_sample(const vo_model *m, int which, const float *cond, const int32_t *actions, int N, int K,
+                        uint64_t seed, float *out, int traj_row, float *traj_out) {
+    if (which < 0 || which > 1 || N < 1 || K < 1) return -1;
+    const vo_mlp *f = &m->mlp[4 + which];
+    const int S = m->S, A = m->A, D = which == 0 ? m->S : m->O;
+    if (f->n_layers < 1 || f->dims[0] != S + A + D + VO_TEMB || f->dims[f->n_layers] != D) return -1;
+    const double half_pi = 1.5707963267948966;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        scratch z = scratch_alloc(m);
+        float *omega = (float *)malloc(sizeof(float) * (size_t)(D + 4));
+        real *x = (real *)malloc(sizeof(real) * (size_t)D), *v = (real *)malloc(sizeof(real) * (size_t)D);
+        vo_normals(seed, (uint32_t)i, 0, 0, VO_STREAM_DIFFUSION, D, omega);
+        for (int j = 0; j < D; ++j) x[j] = (real)omega[j];
+        if (traj_out && i == traj_row) for (int j = 0; j < D; ++j) traj_out[j] = (float)x[j];
+        for (int k = 0; k < K; ++k) {
+            const double tau = 1.0 - (double)k / (double)K, tau_n = 1.0 - (double)(k + 1) / (double)K;
+            for (int j = 0; j < S; ++j) z.x[j] = (real)cond[(size_t)i * S + j];
+            for (int j = 0; j < A; ++j) z.x[S + j] = (j == actions[i]) ? (real)1 : (real)0;
+            for (int j = 0; j < D; ++j) z.x[S + A + j] = x[j];
+            for (int e = 0; e < VO_TEMB / 2; ++e) {
+                const double arg = 3.141592653589793 * (double)(1 << e) * tau;
+                z.x[S + A + D + 2 * e] = (real)sin(arg);
+                z.x[S + A + D + 2 * e + 1] = (real)cos(arg);
+            }
+            mlp_forward_one(f, m->emulate_bf16, z.x, v, z.b0, z.b1);
+            const real al = (real)cos(half_pi * tau), si = (real)sin(half_pi * tau);
+            const real al_n = (real)cos(half_pi * tau_n), si_n = (real)sin(half_pi * tau_n);
+            for (int j = 0; j < D; ++j) {
+                const real x0_hat = al * x[j] - si * v[j];
+                const real eps_hat = si * x[j] + al * v[j];
+                x[j] = al_n * x0_hat + si_n * eps_hat;
+            }
+            if (traj_out && i == traj_row) for (int j = 0; j < D; ++j) traj_out[(size_t)(k + 1) * D + j] = (float)x[j];
+        }
+        for (int j = 0; j < D; ++j) out[(size_t)i * D + j] = (float)x[j];
+        free(omega); free(x); free(v);
+        scratch_free(&z);
+    }
     return 0;
 }
 

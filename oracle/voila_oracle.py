@@ -59,6 +59,8 @@ def _lib(real: str = "f32"):
     lib.vo_pw_update.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp, vp, i32, f64, f64, vp, u64,
                                  vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vo_pw_update.restype = i32
+    lib.vo_diffusion_sample.argtypes = [vp, i32, vp, vp, i32, i32, u64, vp, i32, vp]
+    lib.vo_diffusion_sample.restype = i32
     lib.vo_model_set_terminal.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     lib.vo_model_set_terminal.restype = i32
     lib.vo_resample_systematic_x0.argtypes = [vp, i32, u32, vp]
@@ -160,6 +162,17 @@ class OracleModel:
                                            _p(Wf), _p(bf))
             assert rc == 0
             self.out_dims.append((int(dims[0]), int(dims[-1])))
+        for which, name in ((4, "denoise_T"), (5, "denoise_Z")):
+            f = getattr(model, name, None)
+            if f is not None:
+                dims = np.asarray(f.dims, dtype=np.int32)
+                Wf = np.concatenate([np.asarray(w, np.float32).ravel() for w in f.W])
+                bf = np.concatenate([np.asarray(b, np.float32).ravel() for b in f.b])
+                rc = self.lib.vo_model_set_mlp(self.h, which, len(f.W), _p(dims), int(f.act), _p(Wf), _p(bf))
+                assert rc == 0
+                while len(self.out_dims) <= which:
+                    self.out_dims.append((0, 0))
+                self.out_dims[which] = (int(dims[0]), int(dims[-1]))
         cost = _f32(model.action_cost)
         rc = self.lib.vo_model_set_reward(self.h, int(model.reward_kind),
                                           _p(_f32(model.reward_param).ravel()), _p(cost))
@@ -236,6 +249,21 @@ class OracleModel:
         if rc != 0:
             raise RuntimeError(f"vo_rollout_values_term -> {rc}")
         return out
+
+    def diffusion_sample(self, which, cond, actions, K, seed, traj_row=None):
+        """The diffusion teacher's DDIM-ODE sampler (vo_diffusion_sample).  -> samples [N][D]
+        (and the path [K+1][D] of sample traj_row when given)."""
+        cond = _f32(cond)
+        actions = np.ascontiguousarray(actions, dtype=np.int32)
+        N = cond.shape[0]
+        D = self.S if which == 0 else self.O
+        out = np.zeros((N, D), np.float32)
+        traj = np.zeros((K + 1, D), np.float32) if traj_row is not None else None
+        rc = self.lib.vo_diffusion_sample(self.h, int(which), _p(cond), _p(actions), N, int(K), int(seed), _p(out),
+                                          -1 if traj_row is None else int(traj_row), _p(traj))
+        if rc != 0:
+            raise RuntimeError(f"vo_diffusion_sample -> {rc}")
+        return out if traj is None else (out, traj)
 
     def pw_update(self, particles, group_off, group_action, visit_count, branch_count, branch_obs, k_o,
                   alpha_o, weights, seed):

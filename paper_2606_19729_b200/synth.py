@@ -69,6 +69,9 @@ class ModelSpec:
     action_cost: Optional[np.ndarray] = None
     prec: int = PREC_FP32
     terminal: Optional[TerminalSpec] = None
+    # diffusion teachers: denoisers v(c, a, x_tau, tau), input [c ; onehot(a) ; x ; temb(8)]
+    denoise_T: Optional[MLPSpec] = None   # -> S
+    denoise_Z: Optional[MLPSpec] = None   # -> O
 
     def mlps(self):
         return [self.f_T, self.f_Z, self.lik_obs, self.lik_state]
@@ -134,6 +137,18 @@ def make_mlp(rng: np.random.Generator, dims: List[int], act: int, gain: float = 
         W.append(_xavier(rng, dims[l + 1], dims[l], gain))
         b.append(rng.uniform(-bias_range, bias_range, size=(dims[l + 1],)).astype(np.float32))
     return MLPSpec(list(dims), act, W, b)
+
+
+TEMB = 8  # width of the diffusion-time embedding (R31)
+
+
+def make_denoisers(cfg: Config, hidden: List[int], seed: Optional[int] = None, gain: float = 1.0):
+    """Random-init denoisers of the two diffusion teachers (transition: -> S, observation: -> O)."""
+    seed = BASE_SEED + 500 + cfg.index if seed is None else seed
+    r = [np.random.default_rng(s) for s in np.random.SeedSequence(seed).spawn(2)]
+    vT = make_mlp(r[0], [cfg.S + cfg.A + cfg.S + TEMB] + list(hidden) + [cfg.S], cfg.act, gain)
+    vZ = make_mlp(r[1], [cfg.S + cfg.A + cfg.O + TEMB] + list(hidden) + [cfg.O], cfg.act, gain)
+    return vT, vZ
 
 
 def make_model(cfg: Config, seed: Optional[int] = None, gain: float = 1.0,
