@@ -119,6 +119,10 @@ typedef struct {
     voila_reward reward;
     int prec;              /* voila_prec */
     const voila_terminal *terminal; /* terminal regions of the rollout, or NULL (none) */
+    /* Denoisers of the diffusion teachers, n_layers = 0: none.
+     * v_T : [S + A + S + 8] -> ... -> S, v_Z : [S + A + O + 8] -> ... -> O, input order
+     * [c ; onehot(a) ; x_tau ; temb(tau)], temb = (sin(pi 2^k tau), cos(pi 2^k tau)) for k = 0..3 (reading R31). */
+    voila_mlp denoise_T, denoise_Z;
 } voila_model_desc;
 
 /* Which kernel family runs the generator MLPs (for tests and benchmarks; default AUTO). */
@@ -312,6 +316,22 @@ voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const
                              uint64_t seed, void *particles_out, float *weights_out, int32_t *ancestors_out,
                              int32_t *sim_branch_out, int32_t *opened_out, float *post_weights_out,
                              void *proposals_out, int32_t *seg_status_out, void *cuda_stream);
+
+/* The diffusion teacher's sampler.  The paper distils "an ODE-based diffusion sampler
+ * [27]" of a conditional denoiser trained with the v-prediction objective and a cosine schedule
+ * into f_T / f_Z, and reports the sampling cost of both; this call is
+ * that teacher (readings R30-R32): abar_tau = cos^2(pi tau / 2); uniform grid tau_k = 1 - k/K;
+ * x at tau = 1 is omega ~ N(0, I_D) (Philox stream 7, counter (i, 0, 0)); for k = 0 .. K-1
+ *   v = v_theta(c_i, a_i, x, tau_k);  x0 = alpha x - sigma v;  eps = sigma x + alpha v;
+ *   x <- alpha' x0 + sigma' eps            (DDIM, eta = 0; K denoiser calls per sample)
+ * and x at tau = 0 is the sample.  which = 0: transition teacher (c = s, D = S), 1: observation teacher
+ * (c = s', D = O).
+ *   cond    dev [N][S] fp32 | bf16 (see prec)      actions dev [N] int32 in [0, A) (not range-checked)
+ *   out     dev [N][D] fp32: the samples (also the state of the recursion between the K launches)
+ * Errors: VOILA_ERR_INVALID_ARG for NULL / N < 1 / K < 1 / K > 256, VOILA_ERR_UNSUPPORTED when the model
+ * has no such denoiser. */
+voila_status voila_diffusion_sample(voila_ctx *ctx, int which, const void *cond, const int32_t *actions, int N,
+                                    int K, uint64_t seed, float *out, void *cuda_stream);
 
 /* Host-buffer variants: every pointer is HOST memory (pinned for best speed); inputs are copied to
  * ctx-owned device staging buffers, the device entry point runs, outputs are copied back and the

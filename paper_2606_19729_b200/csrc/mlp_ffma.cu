@@ -410,6 +410,63 @@ __global__ void __launch_bounds__(kThreads) pw_score_ffma_kernel(const ModelDev 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Diffusion teacher (voila_diffusion_sample): one DDIM-ODE step = one call of the
+// denoiser v(c, a, x, tau_k) on [c ; onehot(a) ; x ; temb(tau_k)] and the v-prediction update.
+// ---------------------------------------------------------------------------------------------
+template <bool EMU>
+__global__ void __launch_bounds__(kThreads) diffusion_step_ffma_kernel(const ModelDev m, const DiffusionArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ int act_row[R], src_row[R];
+    const int S = m.S, A = m.A, D = a.D, KW = m.max_width;
+    const MlpDev &f = m.mlp[4 + a.which];
+    float *xa = smem, *xb = xa + KW * R, *v = xb + KW * R, *xs = v + D * R;  // xs: the fp32 state [D][R]
+    const int i0 = blockIdx.x * R;
+    if (threadIdx.x < R) {
+        const int i = i0 + threadIdx.x;
+        src_row[threadIdx.x] = i < a.N ? i : -1;
+        act_row[threadIdx.x] = i < a.N ? __ldg(a.actions + i) : 0;
+    }
+    __syncthreads();
+    load_rows<EMU>(a.cond, S, src_row, xa);
+    fill_onehot(xa, S, A, act_row);
+    if (a.first) {
+        const int nblk = (D + 3) >> 2;
+        for (int idx = threadIdx.x; idx < R * nblk; idx += kThreads) {
+            const int r = idx & (R - 1), blk = idx / R;
+            float z[4];
+            normals4<false>(a.seed, (uint32_t)(i0 + r), 0u, 0u, kStreamDiffusion, (uint32_t)blk, z);
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (4 * blk + i < D) xs[(4 * blk + i) * R + r] = z[i];
+        }
+    } else {
+        for (int idx = threadIdx.x; idx < D * R; idx += kThreads) {
+            const int r = idx / D, j = idx - r * D;
+            xs[j * R + r] = (i0 + r < a.N) ? a.x[(size_t)(i0 + r) * D + j] : 0.0f;
+        }
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < D * R; idx += kThreads)
+        xa[(S + A) * R + idx] = EMU ? bf16_round(xs[idx]) : xs[idx];
+    for (int idx = threadIdx.x; idx < kTemb * R; idx += kThreads) {
+        const float t = a.temb[idx / R];
+        xa[(S + A + D) * R + idx] = EMU ? bf16_round(t) : t;
+    }
+    __syncthreads();
+    const int K0 = S + A + D + kTemb;
+    mlp_chain<EMU>(f, xa, xb, v, K0, K0, -1);
+    for (int idx = threadIdx.x; idx < D * R; idx += kThreads) {
+        const int r = idx / D, j = idx - r * D;
+        if (i0 + r < a.N) {
+            const float x = xs[j * R + r], vv = v[j * R + r];
+            const float x0_hat = a.al * x - a.si * vv;   // v-prediction
+            const float eps_hat = a.si * x + a.al * vv;
+            a.x[(size_t)(i0 + r) * D + j] = a.al_n * x0_hat + a.si_n * eps_hat;  // DDIM, eta = 0
+        }
+    }
+}
+
 __global__ void weight_sum_kernel(const float *__restrict__ w, int n, double *out) {
     __shared__ double sh[256];
     double acc = 0.0;
@@ -569,8 +626,10 @@ size_t ffma_smem_bytes(const ModelDev &m) {
     const size_t rollout = (size_t)(2 * m.max_width + 2 * m.S + 2 * m.O + kWarps + 2) * R * sizeof(float);
     const size_t belief = (size_t)(2 * m.max_width + 2 * m.S + d) * R * sizeof(float);
     const size_t fwd = (size_t)(3 * m.max_width) * R * sizeof(float);
+    const size_t diffusion = (size_t)(2 * m.max_width + 2 * (m.S > m.O ? m.S : m.O)) * R * sizeof(float);
     size_t b = rollout > belief ? rollout : belief;
-    return b > fwd ? b : fwd;
+    b = b > fwd ? b : fwd;
+    return b > diffusion ? b : diffusion;
 }
 
 template <typename K>
@@ -595,6 +654,20 @@ cudaError_t launch_pw_score_ffma(const ModelDev &m, const PwArgs &a, bool bf16, 
     const int grid = (a.N + R - 1) / R;
     return bf16 ? pw_launch(pw_score_ffma_kernel<true>, grid, m, a, st)
                 : pw_launch(pw_score_ffma_kernel<false>, grid, m, a, st);
+}
+
+cudaError_t launch_diffusion_step_ffma(const ModelDev &m, const DiffusionArgs &a, bool bf16, cudaStream_t st) {
+    const size_t smem = ffma_smem_bytes(m);
+    const int grid = (a.N + R - 1) / R;
+    cudaError_t e;
+    if (bf16) {
+        if ((e = set_smem(diffusion_step_ffma_kernel<true>, smem)) != cudaSuccess) return e;
+        diffusion_step_ffma_kernel<true><<<grid, kThreads, smem, st>>>(m, a);
+    } else {
+        if ((e = set_smem(diffusion_step_ffma_kernel<false>, smem)) != cudaSuccess) return e;
+        diffusion_step_ffma_kernel<false><<<grid, kThreads, smem, st>>>(m, a);
+    }
+    return cudaGetLastError();
 }
 
 cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cudaStream_t st) {

@@ -224,6 +224,8 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
         return VOILA_ERR_INVALID_ARG;
     const int d = desc->lik_obs.dims[desc->lik_obs.n_layers];
     if (d != desc->lik_state.dims[desc->lik_state.n_layers]) return VOILA_ERR_INVALID_ARG;
+    if (desc->denoise_T.n_layers != 0 && !valid_mlp(desc->denoise_T, S + A + S + kTemb, S)) return VOILA_ERR_INVALID_ARG;
+    if (desc->denoise_Z.n_layers != 0 && !valid_mlp(desc->denoise_Z, S + A + O + kTemb, O)) return VOILA_ERR_INVALID_ARG;
     if (desc->reward.kind < VOILA_R_NEG_L2_GOAL || desc->reward.kind > VOILA_R_LINEAR || !desc->reward.param)
         return VOILA_ERR_INVALID_ARG;
     const voila_terminal *term = desc->terminal;
@@ -261,7 +263,8 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
     m.lambda = desc->lik_temperature;
     m.gamma = desc->discount;
     m.max_width = 1;
-    const voila_mlp *src[4] = {&desc->f_T, &desc->f_Z, &desc->lik_obs, &desc->lik_state};
+    const voila_mlp *src[6] = {&desc->f_T, &desc->f_Z, &desc->lik_obs, &desc->lik_state, &desc->denoise_T,
+                               &desc->denoise_Z};
     const bool bf16 = desc->prec == VOILA_PREC_BF16;
 
     auto upload = [&](const std::vector<float> &h, const float **dst) -> cudaError_t {
@@ -273,10 +276,11 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
         return cudaMemcpy(p, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice);
     };
     cudaError_t e = cudaSuccess;
-    for (int w = 0; w < 4 && e == cudaSuccess; ++w) {
+    for (int w = 0; w < 6 && e == cudaSuccess; ++w) {
         const voila_mlp &f = *src[w];
         MlpDev &g = m.mlp[w];
         g.n_layers = f.n_layers;
+        if (w >= 4 && f.n_layers == 0) continue;  // no such diffusion teacher
         g.act = f.act;
         for (int l = 0; l <= f.n_layers; ++l) {
             g.dims[l] = f.dims[l];
@@ -740,6 +744,36 @@ voila_status voila_porpp_backup_level(voila_ctx *ctx, const float *R, const floa
                                                     reinterpret_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->launches += 1;
+    return VOILA_OK;
+}
+
+voila_status voila_diffusion_sample(voila_ctx *ctx, int which, const void *cond, const int32_t *actions, int N,
+                                    int K, uint64_t seed, float *out, void *cuda_stream) {
+    if (!ctx || which < 0 || which > 1 || !cond || !actions || !out || N < 1 || K < 1 || K > 256)
+        return VOILA_ERR_INVALID_ARG;
+    if (misaligned(cond) || misaligned(out)) return VOILA_ERR_INVALID_ARG;
+    if (ctx->model.mlp[4 + which].n_layers < 1) return VOILA_ERR_UNSUPPORTED;
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const bool bf16 = ctx->prec == VOILA_PREC_BF16;
+    DiffusionArgs a{};
+    a.cond = cond; a.actions = actions; a.N = N; a.which = which;
+    a.D = which == 0 ? ctx->S : ctx->O;
+    a.seed = seed; a.x = out;
+    const double half_pi = 1.5707963267948966, pi = 3.141592653589793;
+    for (int k = 0; k < K; ++k) {  // one denoiser call per step (why the teacher is expensive)
+        const double tau = 1.0 - (double)k / (double)K, tau_n = 1.0 - (double)(k + 1) / (double)K;
+        for (int e = 0; e < kTemb / 2; ++e) {
+            a.temb[2 * e] = (float)std::sin(pi * (double)(1 << e) * tau);
+            a.temb[2 * e + 1] = (float)std::cos(pi * (double)(1 << e) * tau);
+        }
+        a.al = (float)std::cos(half_pi * tau); a.si = (float)std::sin(half_pi * tau);
+        a.al_n = (float)std::cos(half_pi * tau_n); a.si_n = (float)std::sin(half_pi * tau_n);
+        a.first = k == 0;
+        const cudaError_t e = launch_diffusion_step_ffma(ctx->model, a, bf16, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 1;
+    }
     return VOILA_OK;
 }
 

@@ -13,6 +13,7 @@ constexpr uint32_t kStreamBeliefT = 3u;
 constexpr uint32_t kStreamResample = 4u;
 constexpr uint32_t kStreamPwObs = 5u;     // progressive widening: noise of the sampled observation
 constexpr uint32_t kStreamPwAttach = 6u;  // progressive widening: word that picks an existing branch
+constexpr uint32_t kStreamDiffusion = 7u;  // diffusion teacher: the initial noise x_1 = omega
 
 // Philox4x32-10 (Salmon et al., SC'11): counter-based generator, one 128-bit block per call.
 __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {

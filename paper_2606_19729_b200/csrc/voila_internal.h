@@ -41,7 +41,7 @@ struct ModelDev {
     int S, O, A, Nz;
     int lik_action_cond;
     float lambda, gamma;
-    MlpDev mlp[4];  // 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower)
+    MlpDev mlp[6];  // 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower), 4 / 5 denoisers v_T / v_Z (n_layers 0: none)
     RewardDev reward;
     TerminalDev term;
     int max_width;  // widest activation vector over all four networks (incl. inputs)
@@ -97,6 +97,19 @@ struct PwArgs {
     void *particles_out;
     float *weights_out, *post_weights_out;
     int32_t *ancestors_out, *sim_branch_out, *opened_out, *seg_status_out;
+};
+
+// voila_diffusion_sample: one DDIM-ODE step (one denoiser call) over all samples.
+constexpr int kTemb = 8;  // width of the diffusion-time embedding (reading R31)
+struct DiffusionArgs {
+    const void *cond;        // [N][S]
+    const int32_t *actions;  // [N]
+    int N, which, D;         // D = S (transition teacher) | O (observation teacher)
+    int first;               // 1: x = omega (Philox stream 7) instead of the stored state
+    uint64_t seed;
+    float temb[kTemb];       // temb(tau_k)
+    float al, si, al_n, si_n;  // alpha, sigma at tau_k and at tau_{k+1}
+    float *x;                // [N][D] fp32 state, updated in place (the caller's output buffer)
 };
 
 // Bookkeeping block of the scan / resample kernels (device memory, zeroed per call by a kernel).

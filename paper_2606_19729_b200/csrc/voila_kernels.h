@@ -59,6 +59,9 @@ cudaError_t launch_pw_propose_score_tc2(void *tc2, const ModelDev &m, const PwAr
                                         const int32_t *sim_seg, cudaStream_t st, std::string *kernel_name);
 cudaError_t launch_pw_resample(const PwArgs &a, const unsigned long long *cdf, int row_bytes, cudaStream_t st);  // 1-2 launches
 
+// ---- mlp_ffma.cu : one DDIM-ODE step of the diffusion teacher's sampler (voila_diffusion_sample) ----
+cudaError_t launch_diffusion_step_ffma(const ModelDev &m, const DiffusionArgs &a, bool bf16, cudaStream_t st);
+
 // ---- porpp.cu : one level of the PORPP preference backup (Eq. 1) ----
 cudaError_t launch_porpp_backup_level(const float *R, const float *logpi0, const int32_t *child_off,
                                       const int32_t *child_idx, const float *child_w, const float *v_next,

@@ -27,7 +27,7 @@ EXPORTS = [
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read", "voila_pw_workspace_bytes", "voila_pw_reserve", "voila_pw_update",
-    "voila_porpp_backup",
+    "voila_porpp_backup", "voila_diffusion_sample",
 ]
 
 
@@ -62,7 +62,7 @@ class _ModelDesc(C.Structure):
                 ("noise_dim", C.c_int), ("f_T", _Mlp), ("f_Z", _Mlp), ("lik_obs", _Mlp),
                 ("lik_state", _Mlp), ("lik_action_cond", C.c_int), ("lik_temperature", C.c_float),
                 ("discount", C.c_float), ("reward", _Reward), ("prec", C.c_int),
-                ("terminal", C.POINTER(_Terminal))]
+                ("terminal", C.POINTER(_Terminal)), ("denoise_T", _Mlp), ("denoise_Z", _Mlp)]
 
 
 def lib_path() -> str:
@@ -134,6 +134,8 @@ def load_library():
     lib.voila_pw_update.restype = i32
     lib.voila_porpp_backup.argtypes = [vp, C.POINTER(_PorppLevel), i32, i32, vp, C.c_float, C.c_float, vp, vp]
     lib.voila_porpp_backup.restype = i32
+    lib.voila_diffusion_sample.argtypes = [vp, i32, vp, vp, i32, i32, u64, vp, vp]
+    lib.voila_diffusion_sample.restype = i32
     lib.voila_version.argtypes = []
     lib.voila_version.restype = i32
     _LIB = lib
@@ -206,6 +208,10 @@ class Voila:
                                 _fptr(t_rad), _fptr(t_rew), t_stop.ctypes.data_as(C.POINTER(C.c_int)))
             keep.extend([t_dims, t_cen, t_rad, t_rew, t_stop, tstruct])
             desc.terminal = C.pointer(tstruct)
+        for name in ("denoise_T", "denoise_Z"):
+            f = getattr(model, name, None)
+            if f is not None:
+                setattr(desc, name, _pack_mlp(f, keep))
         h = C.c_void_p()
         self._h = None
         self._check(self.lib.voila_create(C.byref(desc), self.device, C.byref(h)), "voila_create")
@@ -382,6 +388,19 @@ class Voila:
             _dptr(out["ancestors"]), _dptr(out["sim_branch"]), _dptr(out.get("opened")),
             _dptr(out.get("post_weights")), _dptr(out.get("proposals")), _dptr(out["seg_status"]),
             self._stream()), "voila_pw_update")
+        return out
+
+    def voila_diffusion_sample(self, which, cond, actions, K, seed):
+        """The diffusion teacher's DDIM-ODE sampler (include/voila.h): K denoiser calls per sample.
+        which = 0 transition teacher (-> [N][S]), 1 observation teacher (-> [N][O]); fp32 output."""
+        torch = self._torch
+        N = cond.shape[0]
+        assert cond.dtype == self.particle_dtype and cond.is_contiguous() and cond.shape[1] == self.S
+        assert actions.dtype == torch.int32 and actions.numel() == N
+        out = torch.empty((N, self.S if which == 0 else self.O), dtype=torch.float32, device=cond.device)
+        self._check(self.lib.voila_diffusion_sample(self._h, int(which), _dptr(cond), _dptr(actions), N, int(K),
+                                                    C.c_uint64(int(seed)), _dptr(out), self._stream()),
+                    "voila_diffusion_sample")
         return out
 
     def voila_resample_systematic(self, v, seed):
