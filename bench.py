@@ -400,6 +400,57 @@ def _leg_pw(vl, synth, dev, local, peaks, flush, calls=10):
     return leg
 
 
+def _leg_diffusion(vl, synth, dev, local, peaks, K=32, N=1 << 16):
+    """the diffusion teacher's sampler next to the distilled generator it is distilled into
+    (PAPER.md:202 reports 8.6e5 / 1.2e6 samples/s distilled vs 8.2e3 / 1.8e4 for the diffusion models at
+    batch 1024 on a laptop GPU, "up to 105x"): config-3 shapes, denoisers 4 x 512 SiLU, K = 32 DDIM-ODE
+    steps, against the f_T proposals of one belief update of the same batch (propose + score kernel)."""
+    import torch
+    cfg = synth.CONFIGS[3]
+    vT, vZ = synth.make_denoisers(cfg, [512, 512, 512, 512])
+    model = synth.make_model(cfg).replace(denoise_T=vT, denoise_Z=vZ)
+    rng = np.random.default_rng(20260619 + 88)
+    ctx = vl.Voila(model, device=local)
+    cond = ctx.to_particles(rng.standard_normal((N, cfg.S)).astype(np.float32))
+    act = torch.from_numpy(rng.integers(0, cfg.A, N).astype(np.int32)).to(dev)
+    out = {}
+    for which, name in ((0, "transition"), (1, "observation")):
+        for _ in range(2):
+            ctx.voila_diffusion_sample(which, cond, act, K, 1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        a.record()
+        for r in range(3):
+            ctx.voila_diffusion_sample(which, cond, act, K, 2 + r)
+        b.record()
+        torch.cuda.synchronize(dev)
+        ms = a.elapsed_time(b) / 3
+        f = vT if which == 0 else vZ
+        flop = 2 * sum(f.dims[l] * f.dims[l + 1] for l in range(len(f.W))) * K
+        out[name] = {"samples_per_s": N / (ms * 1e-3), "ms": ms, "denoiser_calls": K,
+                     "tflops": N * flop / (ms * 1e-3) / 1e12, "kernel": ctx.voila_last_belief_kernel() or "diffusion_step_ffma_kernel"}
+    # the distilled side: one f_T sample per particle inside the belief update's propose+score kernel
+    obs = torch.zeros(cfg.O, device=dev)
+    bufs = ctx.belief_update_buffers(cond, want_debug=False)
+    ctx.voila_set_profiling(True)
+    for _ in range(3):
+        ctx.voila_belief_update(cond, 1, obs, None, 5, want_debug=False, out=bufs)
+    torch.cuda.synchronize(dev)
+    ctx.voila_profile_read(1)
+    for _ in range(5):
+        ctx.voila_belief_update(cond, 1, obs, None, 6, want_debug=False, out=bufs)
+    torch.cuda.synchronize(dev)
+    kt = ctx.voila_profile_read(1)
+    ctx.voila_set_profiling(False)
+    dist = N / (float(np.mean(kt)) * 1e-3)
+    ctx.close()
+    return {"workload": f"{N} samples, config-3 shapes, denoisers 4x512, K={K}", "teacher": out,
+            "distilled_f_T_samples_per_s": dist, "distilled_note": "f_T proposal + state tower + score per sample "
+            "(the belief update's propose+score kernel): an upper bound on the cost of one f_T sample",
+            "ratio_transition": dist / out["transition"]["samples_per_s"],
+            "paper": "PAPER.md:202: 8.6e5 vs 8.2e3 (transition), 1.2e6 vs 1.8e4 (observation) samples/s, up to 105x, laptop RTX 3500 Ada"}
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     from paper_2606_19729_b200 import synth
@@ -625,6 +676,7 @@ def run_voila(args):
         extra["belief_update_cfg4"] = _leg_belief_cfg4(vl, synth, dev, local, peaks, flush)
         extra["rollout_cfg3"] = _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush)
         extra["progressive_widening"] = _leg_pw(vl, synth, dev, local, peaks, flush)
+        extra["diffusion_teacher"] = _leg_diffusion(vl, synth, dev, local, peaks)
 
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
     cpu_1t = _oracle_one_thread(cfg, model, inp)
