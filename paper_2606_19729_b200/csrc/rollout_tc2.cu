@@ -100,6 +100,11 @@ struct T2Params {
     const int32_t *pw_sim_seg;     // [N] child index g * M_max + b
     const float *pw_E;             // [children][d]
     int *pw_seg_max;               // [children] ordered-int maxima
+    // diffusion teacher (voila_diffusion_sample): one DDIM-ODE step per launch; the operand is
+    // [c ; x ; onehot(a)], the time embedding sits in the step's bias row (bu_action = step index)
+    float *diff_x;                 // [N][D] fp32 state, updated in place, or nullptr
+    int diff_D, diff_first;        // first: x = omega (Philox stream 7) instead of the stored state
+    float al, si, al_n, si_n;      // alpha, sigma at tau_k and tau_{k+1}
 };
 
 struct Smem2 {
@@ -760,14 +765,32 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             }
         }
         const int u0 = S >> 3;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (8 * u < Nz) {
-                const uint4 v = noise_unit8(p.seed, (uint32_t)i_idx, 0u, 0u, kStreamBeliefT, (uint32_t)u);
+        int u_next = u0;
+        if (p.diff_x) {
+            // diffusion teacher: the current x (bf16 operand copy of the fp32 state; omega at the first step)
+            for (int u = 0; u < (p.diff_D >> 3); ++u) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (p.diff_first) {
+                    v = noise_unit8(p.seed, (uint32_t)i_idx, 0u, 0u, kStreamDiffusion, (uint32_t)u);
+                } else if (valid) {
+                    const float4 *xp = reinterpret_cast<const float4 *>(p.diff_x + (size_t)i_idx * p.diff_D) + 2 * u;
+                    const float4 x0 = __ldg(xp), x1 = __ldg(xp + 1);
+                    v = make_uint4(pack_bf16x2(x0.x, x0.y), pack_bf16x2(x0.z, x0.w), pack_bf16x2(x1.x, x1.y),
+                                   pack_bf16x2(x1.z, x1.w));
+                }
                 st_shared_v4(a_unit_addr(a_slot, row, u0 + u), v.x, v.y, v.z, v.w);
             }
+            u_next = u0 + (p.diff_D >> 3);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (8 * u < Nz) {
+                    const uint4 v = noise_unit8(p.seed, (uint32_t)i_idx, 0u, 0u, kStreamBeliefT, (uint32_t)u);
+                    st_shared_v4(a_unit_addr(a_slot, row, u0 + u), v.x, v.y, v.z, v.w);
+                }
+            }
+            u_next = u0 + (Nz >> 3);
         }
-        int u_next = u0 + (Nz >> 3);
         if (p.pw_sim_action) {
             // per-row action: the one-hot block is part of the operand, columns [S + Nz, S + Nz + A)
             const int a_row = valid ? __ldg(p.pw_sim_action + i_idx) : -1;
@@ -858,6 +881,56 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 } else {
                     for (int u = S >> 3; u < g_units; ++u) st_shared_v4(a_unit_addr(a_slot, row, u), 0u, 0u, 0u, 0u);
                 }
+                fence_proxy_async_smem();
+                tc_fence_before();
+                es.arrive_event();
+                T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
+            } else if (l.epi == T2_EPI_DIFFUSE) {  // diffusion teacher: last (only) network of the unit
+                const int i_idx = row_index(step, slot);
+                const bool valid = i_idx < p.P;
+                const int D = p.diff_D;
+                es.wait_layer();
+                T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
+                if (half == 0) {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        if (16 * g < (int)l.n_pad) {
+                            uint32_t v[16];
+                            tmem_ld16(taddr + 16 * g, v);
+                            float4 b[4], x[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                                x[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                if (16 * g + 4 * i < D) {
+                                    if (p.diff_first) {
+                                        x[i] = normals_f4(p.seed, (uint32_t)i_idx, 0u, 0u, kStreamDiffusion,
+                                                          (uint32_t)(4 * g + i));
+                                    } else if (valid) {
+                                        x[i] = __ldg(reinterpret_cast<const float4 *>(p.diff_x + (size_t)i_idx * D) + 4 * g + i);
+                                    }
+                                }
+                            }
+                            tmem_ld_wait();
+                            // v-prediction and the DDIM step (eta = 0) per element
+                            auto upd = [&](float xx, uint32_t d, float bb) {
+                                const float vv = __uint_as_float(d) + bb;
+                                const float x0_hat = p.al * xx - p.si * vv, eps_hat = p.si * xx + p.al * vv;
+                                return p.al_n * x0_hat + p.si_n * eps_hat;
+                            };
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                if (valid && 16 * g + 4 * i < D) {
+                                    const float4 o = make_float4(upd(x[i].x, v[4 * i], b[i].x), upd(x[i].y, v[4 * i + 1], b[i].y),
+                                                                 upd(x[i].z, v[4 * i + 2], b[i].z), upd(x[i].w, v[4 * i + 3], b[i].w));
+                                    *(reinterpret_cast<float4 *>(p.diff_x + (size_t)i_idx * D) + 4 * g + i) = o;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot);
+                named_bar_sync(bar_id, 256);
                 fence_proxy_async_smem();
                 tc_fence_before();
                 es.arrive_event();
@@ -1415,7 +1488,7 @@ struct Builder2 {
             }
         } else {
             for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
-            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE)  // the next layer-1 input is written with this event
+            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE && epi != T2_EPI_DIFFUSE)  // the next layer-1 input is written with this event
                 for (int j = chunk_off; j < std::min(8, chunk_off + slot_chunks); ++j) a_ready[j] = evt;
             evt_set.push_back(0);
             ++evt;
@@ -1462,6 +1535,12 @@ struct T2Handle {
     // progressive widening: the belief program with the one-hot block in the operand (per-row actions)
     T2Program pw, pw_dual;
     bool has_pw = false, has_pw_dual = false;
+    // diffusion teachers (0 transition, 1 observation): one denoiser call per launch, [which][dual]
+    T2Program diff[2][2];
+    bool has_diff[2][2] = {{false, false}, {false, false}};
+    float *d_diff_b1[2] = {nullptr, nullptr}, *d_diff_w1t[2] = {nullptr, nullptr};  // layer-1 bias, time-embedding columns
+    int diff_n1[2] = {0, 0};
+    float diff_scale[2] = {1.0f, 1.0f};
     bool roll_x = false;    // rollout runs the 640-thread kernel (two sets of epilogue warps)
 };
 
@@ -1506,6 +1585,44 @@ void add_generator2_dense(Builder2 &pb, const voila_mlp &f, int S, int A, int Nz
             pb.add_layer(f.W[l], N, K, f.b[l], 1, last ? last_epi : T2_EPI_HIDDEN, f.act);
         }
     }
+}
+
+// Denoiser of a diffusion teacher: input order [c ; x ; onehot(a)] (K = S + D + A); the time-embedding
+// columns of layer 1 are folded into one bias row per DDIM step (the row is written before the step's
+// launch by diffusion_bias_kernel and picked like a per-action row).
+constexpr int kT2DiffMaxSteps = 256;
+void add_denoiser2(Builder2 &pb, const voila_mlp &f, int S, int A, int D) {
+    for (int l = 0; l < f.n_layers; ++l) {
+        const int K = f.dims[l], N = f.dims[l + 1];
+        const bool last = l == f.n_layers - 1;
+        if (l == 0) {
+            const int k0 = S + D + A;
+            std::vector<float> W((size_t)N * k0);
+            for (int j = 0; j < N; ++j) {
+                for (int k = 0; k < S; ++k) W[(size_t)j * k0 + k] = f.W[0][(size_t)j * K + k];
+                for (int k = 0; k < D; ++k) W[(size_t)j * k0 + S + k] = f.W[0][(size_t)j * K + S + A + k];
+                for (int a = 0; a < A; ++a) W[(size_t)j * k0 + S + D + a] = f.W[0][(size_t)j * K + S + a];
+            }
+            pb.add_layer(W.data(), N, k0, nullptr, kT2DiffMaxSteps, last ? T2_EPI_DIFFUSE : T2_EPI_HIDDEN, f.act);
+        } else {
+            pb.add_layer(f.W[l], N, K, f.b[l], 1, last ? T2_EPI_DIFFUSE : T2_EPI_HIDDEN, f.act);
+        }
+    }
+}
+
+// bias row of one DDIM step: scale * (b1[j] + sum_e bf16(W1[j][temb e]) * bf16(temb_e)), zero padding
+struct TembArg { float v[kTemb]; };
+__global__ void diffusion_bias_kernel(float *row, const float *__restrict__ b1, const float *__restrict__ w1t, int n,
+                                      int n_pad, float scale, TembArg t) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_pad) return;
+    float acc = 0.0f;
+    if (j < n) {
+        acc = b1[j];
+#pragma unroll
+        for (int e = 0; e < kTemb; ++e) acc = fmaf(w1t[j * kTemb + e], bf16_round(t.v[e]), acc);
+    }
+    row[j] = scale * acc;
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -1698,12 +1815,62 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             }
         }
     }
+    // diffusion teachers: one program per denoiser (one- and two-slot)
+    for (int which = 0; which < 2; ++which) {
+        const voila_mlp &f = which == 0 ? d->denoise_T : d->denoise_Z;
+        const int D = which == 0 ? S : d->obs_dim;
+        if (f.n_layers < 2 || f.n_layers > 8 || D % 8 != 0 || D > 64) continue;
+        bool fits = S + D + rup(A, 8) <= 512;
+        int widest = S + D + rup(A, 8);
+        for (int l = 1; l < f.n_layers; ++l) {
+            fits = fits && f.dims[l] % 64 == 0 && f.dims[l] <= 512;
+            widest = std::max(widest, f.dims[l]);
+        }
+        if (!fits) continue;
+        const int in_cols = S + D + rup(A, 8);
+        for (int dual = 0; dual <= ((widest <= 256 && rup(in_cols, 64) / 64 <= 4) ? 1 : 0); ++dual) {
+            Builder2 pb;
+            pb.policy = policy;
+            if (dual) pb.set_dual(4, 256);
+            add_denoiser2(pb, f, S, A, D);
+            T2Program &prog = h->diff[which][dual];
+            prog.hdr.g_in_chunks = 0;
+            prog.hdr.e_pad = 0;
+            prog.hdr.e_off = (int)pb.sbias_init.size();
+            const std::string m =
+                dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(in_cols, 64) / 64, sm_count, allocs, kT2ThreadsDual)
+                     : finish_program(pb, prog, belief_tc2_kernel, rup(in_cols, 64) / 64, sm_count, allocs);
+            h->has_diff[which][dual] = m.empty();
+        }
+        if (h->has_diff[which][0]) {
+            const int N1 = f.dims[1], K = f.dims[0];
+            std::vector<float> b1(f.b[0], f.b[0] + N1), w1t((size_t)N1 * kTemb);
+            for (int j = 0; j < N1; ++j)
+                for (int e = 0; e < kTemb; ++e) w1t[(size_t)j * kTemb + e] = h_bf16_round(f.W[0][(size_t)j * K + S + A + D + e]);
+            void *p1 = nullptr, *p2 = nullptr;
+            if (cudaMalloc(&p1, b1.size() * 4) == cudaSuccess && cudaMalloc(&p2, w1t.size() * 4) == cudaSuccess) {
+                allocs->push_back(p1);
+                allocs->push_back(p2);
+                cudaMemcpy(p1, b1.data(), b1.size() * 4, cudaMemcpyHostToDevice);
+                cudaMemcpy(p2, w1t.data(), w1t.size() * 4, cudaMemcpyHostToDevice);
+                h->d_diff_b1[which] = reinterpret_cast<float *>(p1);
+                h->d_diff_w1t[which] = reinterpret_cast<float *>(p2);
+                h->diff_n1[which] = N1;
+                h->diff_scale[which] = f.act == VOILA_ACT_SILU ? 0.5f : 1.0f;  // SiLU layers carry pre-halved biases
+            } else {
+                h->has_diff[which][0] = h->has_diff[which][1] = false;
+            }
+        }
+    }
     return h;
 }
 
 void tc2_destroy(void *tc) { delete reinterpret_cast<T2Handle *>(tc); }
 
 bool tc2_has_belief(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_belief; }
+bool tc2_has_diffusion(const void *tc, int which) {
+    return tc && reinterpret_cast<const T2Handle *>(tc)->has_diff[which][0];
+}
 bool tc2_has_pw(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_pw; }
 int tc2_pw_e_stride(const void *tc) { return reinterpret_cast<const T2Handle *>(tc)->pw.hdr.e_pad; }
 
@@ -1817,6 +1984,46 @@ cudaError_t launch_pw_propose_score_tc2(void *tc, const ModelDev &m, const PwArg
     if (kernel_name)
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, per-row actions>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, per-row actions>";
+    return cudaGetLastError();
+}
+
+// One DDIM-ODE step of a diffusion teacher on the CTA-pair tcgen05 program (2 launches: the step's
+// bias row with the time embedding folded in, then the denoiser + update over all samples).
+cudaError_t launch_diffusion_step_tc2(void *tc, const ModelDev &m, const DiffusionArgs &a, int k, cudaStream_t st,
+                                      std::string *kernel_name) {
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    const int w = a.which;
+    const bool dual = h->has_diff[w][1] && a.N > 2 * kT2Rows * h->diff[w][0].max_clusters;
+    const T2Program &g = h->diff[w][dual ? 1 : 0];
+    // layer 1 is the program's first layer record: its per-step bias rows start at offset 0 of the
+    // program's bias buffer; hidden widths are multiples of 64, so n_pad = N1
+    const int n_pad = h->diff_n1[w];
+    float *row = reinterpret_cast<float *>(g.d_bias) + (size_t)k * n_pad;
+    TembArg t;
+    for (int e = 0; e < kTemb; ++e) t.v[e] = a.temb[e];
+    diffusion_bias_kernel<<<(n_pad + 127) / 128, 128, 0, st>>>(row, h->d_diff_b1[w], h->d_diff_w1t[w], h->diff_n1[w], n_pad,
+                                                               h->diff_scale[w], t);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    T2Params p = base_params(g, m);
+    p.particles = reinterpret_cast<const uint16_t *>(a.cond);
+    p.weights = nullptr;
+    p.P = a.N; p.Q = 1; p.H = 1;
+    p.seed = a.seed;
+    const int unit_rows = 2 * kT2Rows * g.hdr.n_slots;
+    p.n_units = (a.N + unit_rows - 1) / unit_rows;
+    p.bu_action = k;  // the step's bias row
+    p.pw_sim_action = a.actions;
+    p.diff_x = a.x;
+    p.diff_D = a.D;
+    p.diff_first = a.first;
+    p.al = a.al; p.si = a.si; p.al_n = a.al_n; p.si_n = a.si_n;
+    const int clusters = std::min(g.max_clusters, p.n_units);
+    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (kernel_name)
+        *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, denoiser + DDIM step>"
+                            : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, denoiser + DDIM step>";
     return cudaGetLastError();
 }
 

@@ -45,7 +45,8 @@ enum T2Epi : int {
     T2_EPI_STATE = 2,     // rollout: s' = D + bias ; next operand = [s' ; w_Z]
     T2_EPI_OBS = 3,       // rollout: o = D + bias -> witness ; next operand = [s' ; w_T]
     T2_EPI_PROPOSAL = 4,  // belief: s' = D + bias -> proposals (HBM) ; next operand = [s']
-    T2_EPI_SCORE = 5      // belief: logit = <e, D + bias>/lambda + log w -> logits, running max
+    T2_EPI_SCORE = 5,     // belief: logit = <e, D + bias>/lambda + log w -> logits, running max
+    T2_EPI_DIFFUSE = 6    // diffusion teacher: v = D + bias ; x <- DDIM-ODE step(x, v) (fp32 state in HBM)
 };
 
 struct T2Layer {  // what the epilogue needs to know about a layer

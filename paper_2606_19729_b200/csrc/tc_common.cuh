@@ -90,6 +90,13 @@ static __device__ __noinline__ uint4 noise_unit8(uint64_t seed, uint32_t p, uint
     return make_uint4(pack_bf16x2(z[0], z[1]), pack_bf16x2(z[2], z[3]), pack_bf16x2(z[4], z[5]),
                       pack_bf16x2(z[6], z[7]));
 }
+// Four fp32 normals of one Philox block (same fast intrinsics as noise_unit8); not inlined either.
+static __device__ __noinline__ float4 normals_f4(uint64_t seed, uint32_t p, uint32_t q, uint32_t t, uint32_t stream,
+                                                 uint32_t blk) {
+    float z[4];
+    normals4<true>(seed, p, q, t, stream, blk, z);
+    return make_float4(z[0], z[1], z[2], z[3]);
+}
 __device__ __forceinline__ void gen_noise_call(uint32_t (&nz)[16], uint64_t seed, uint32_t p, uint32_t q,
                                                uint32_t t, uint32_t stream, int Nz) {
 #pragma unroll

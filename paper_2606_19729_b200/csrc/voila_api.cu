@@ -770,9 +770,16 @@ voila_status voila_diffusion_sample(voila_ctx *ctx, int which, const void *cond,
         a.al = (float)std::cos(half_pi * tau); a.si = (float)std::sin(half_pi * tau);
         a.al_n = (float)std::cos(half_pi * tau_n); a.si_n = (float)std::sin(half_pi * tau_n);
         a.first = k == 0;
-        const cudaError_t e = launch_diffusion_step_ffma(ctx->model, a, bf16, st);
+        cudaError_t e;
+        if (use_tc2(ctx) && tc2_has_diffusion(ctx->tc2, which)) {
+            e = launch_diffusion_step_tc2(ctx->tc2, ctx->model, a, k, st, &ctx->last_belief_kernel);
+            ctx->launches += 2;
+        } else {
+            e = launch_diffusion_step_ffma(ctx->model, a, bf16, st);
+            ctx->last_belief_kernel = bf16 ? "diffusion_step_ffma_kernel<bf16>" : "diffusion_step_ffma_kernel<fp32>";
+            ctx->launches += 1;
+        }
         if (e != cudaSuccess) return cuda_fail(ctx, e);
-        ctx->launches += 1;
     }
     return VOILA_OK;
 }

@@ -54,6 +54,9 @@ cudaError_t launch_pw_propose_ffma(const ModelDev &m, const PwArgs &a, bool bf16
 cudaError_t launch_pw_obs_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);
 cudaError_t launch_pw_score_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);
 cudaError_t launch_pw_weights(const PwArgs &a, cudaStream_t st);
+bool tc2_has_diffusion(const void *tc2, int which);  // the denoiser program of that teacher was built
+cudaError_t launch_diffusion_step_tc2(void *tc2, const ModelDev &m, const DiffusionArgs &a, int k, cudaStream_t st,
+                                      std::string *kernel_name);
 bool tc2_has_pw(const void *tc2);  // the per-row-action propose+score program was built
 cudaError_t launch_pw_propose_score_tc2(void *tc2, const ModelDev &m, const PwArgs &a, const int32_t *sim_action,
                                         const int32_t *sim_seg, cudaStream_t st, std::string *kernel_name);
