@@ -670,12 +670,20 @@ def run_voila(args):
 
     porpp = _porpp_leg(ctx, dev, peaks)
     extra = {}
-    if args.config == DEFAULT_CONFIG and not reduced and not args.no_legs:
-        # BASELINE.json's metric is "rollout steps/sec AND belief-update latency": the latency half is
-        # defined on config 4 (2^20 particles), the paper-shaped rollout on config 3
+    all_legs = ["belief_update_cfg4", "rollout_cfg3", "progressive_widening", "diffusion_teacher"]
+    if args.legs is not None:
+        legs = [x for x in args.legs.split(",") if x]
+    else:
+        legs = all_legs if (args.config == DEFAULT_CONFIG and not reduced and not args.no_legs) else []
+    # BASELINE.json's metric is "rollout steps/sec AND belief-update latency": the latency half is defined
+    # on config 4 (2^20 particles), the paper-shaped rollout on config 3; then the SURVEY 8(f) rows
+    if "belief_update_cfg4" in legs:
         extra["belief_update_cfg4"] = _leg_belief_cfg4(vl, synth, dev, local, peaks, flush)
+    if "rollout_cfg3" in legs:
         extra["rollout_cfg3"] = _leg_rollout_cfg3(vl, synth, dev, local, peaks, flush)
+    if "progressive_widening" in legs:
         extra["progressive_widening"] = _leg_pw(vl, synth, dev, local, peaks, flush)
+    if "diffusion_teacher" in legs:
         extra["diffusion_teacher"] = _leg_diffusion(vl, synth, dev, local, peaks)
 
     cpu_v, cores, desc, _ = _oracle_sample(cfg, model, inp, target_s=args.cpu_seconds)
@@ -710,6 +718,9 @@ def main():
     ap.add_argument("--impl", default="voila", choices=["voila", "reference"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "ffma", "tcgen05"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--legs", default=None,
+                    help="comma list of the extra legs to run whatever the config (profiling runs): "
+                         "belief_update_cfg4,rollout_cfg3,progressive_widening,diffusion_teacher")
     ap.add_argument("--no-legs", action="store_true",
                     help="skip the config-4 belief-update and config-3 rollout legs of the default line")
     # size overrides for profiling runs (ncu replays every launch ~40 times); the line then says
