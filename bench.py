@@ -602,9 +602,12 @@ def run_voila(args):
     h_st = torch.empty(1, dtype=torch.int32).pin_memory()
     e2e_steps = max(1, min(args.steps, 3))
 
+    h_best = torch.zeros(2, dtype=torch.int32).pin_memory()
+
     def e2e_step(k):
-        ctx.voila_rollout_values_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals)
-        a_exec = int(h_seqs[int(np.argmax(h_vals.numpy())), 0]) if cfg.index == 5 else inp.bu_action  # ties -> lowest q
+        # planning half through the C ABI: rollout + executed action (argmax on the device), host buffers
+        ctx.voila_plan_host(h_parts, h_seqs, None, seed0 + 2 * k, h_vals, h_best)
+        a_exec = int(h_best[1]) if cfg.index == 5 else inp.bu_action
         ctx.voila_belief_update_host(h_bu, a_exec, h_obs[k % h_obs.shape[0], :cfg.O], h_w,
                                      seed0 + 2 * k + 1, h_pout, None, h_anc, h_le, h_st)
 
@@ -619,10 +622,10 @@ def run_voila(args):
     e2e_s = time.perf_counter() - t0
     e2e_s = replicas.max_over_ranks(e2e_s, dist, dev)
     h2d = P * cfg.S * esize + Q * H * 4 + N * cfg.S * esize + cfg.O * 4 + (N * 4 if h_w is not None else 0)
-    d2h = Q * 4 + N * cfg.S * esize + N * 4 + 8
+    d2h = Q * 4 + 8 + N * cfg.S * esize + N * 4 + 8
     e2e = {"value": world * P * Q * H * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-           "api": "voila_rollout_values_host + voila_belief_update_host"}
+           "api": "voila_plan_host + voila_belief_update_host"}
     if rank != 0:
         return
 

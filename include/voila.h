@@ -33,6 +33,14 @@
  *   - Errors found on the host return a status and enqueue nothing.  Conditions only the device can
  *     see (all weights zero, non-finite scores) set *dev_status_out != 0.
  *   - There is no CPU fallback: without a usable sm_100 device voila_create fails.
+ *   - A ctx owns ONE workspace (voila_reserve): its calls must be issued on one stream at a time; two
+ *     calls of the same ctx running concurrently on different streams race on it.  Use one ctx per stream.
+ *   - If the rollout's weights sum to zero (or are not finite) values_out / obs_witness_out are NaN.
+ *   - particles_out must alias neither particles nor proposals_out.
+ *   - Tuning knobs read once by voila_create from the environment (A/B measurements only; the defaults are
+ *     what the tests and bench.py run): VOILA_T2_BLOCK_POLICY (0..4: accumulator block shapes of the
+ *     tcgen05 pair kernels), VOILA_T2_ROLLOUT_WARPS (8 | 16 epilogue warps of the rollout kernel),
+ *     VOILA_T2_STAGES (2..8 weight-ring stages), VOILA_T2_BELIEF_1SLOT (disable the two-slot programs).
  */
 #ifndef VOILA_H_
 #define VOILA_H_
@@ -156,7 +164,7 @@ int voila_tcgen05_supported(const voila_ctx *ctx);
  * s_{t+1} = f_T(s_t, a_{q,t}, w_T(p,q,t)),  o_{t+1} = f_Z(s_{t+1}, a_{q,t}, w_Z(p,q,t)),
  * wbar_p = weights[p] / sum weights   (O4).
  *   particles        dev [P][S]   fp32 | bf16 (see prec)
- *   action_seqs      dev [Q][H]   int32 in [0, A)   (values are not range-checked on the device)
+ *   action_seqs      dev [Q][H]   int32 in [0, A)   (an out-of-range entry is clamped into [0, A) by the kernels)
  *   weights          dev [P] fp32 >= 0, unnormalised; NULL = uniform
  *   seed             keys the Philox4x32-10 noise: counter (p, q, t, stream<<16 | block)
  *   values_out       dev [Q] fp32
@@ -340,6 +348,12 @@ voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, in
                                        const int32_t *action_seqs, int Q, int H,
                                        const float *weights, uint64_t seed, float *values_out,
                                        float *obs_witness_out, void *cuda_stream);
+/* The whole planning half through host buffers: the rollout, then the executed action (the first action
+ * of argmax_q V_q, voila_best_action) on the device; best_q_out / best_action_out host [1] int32 or NULL. */
+voila_status voila_plan_host(voila_ctx *ctx, const void *particles, int P, const int32_t *action_seqs, int Q,
+                             int H, const float *weights, uint64_t seed, float *values_out,
+                             float *obs_witness_out, int32_t *best_q_out, int32_t *best_action_out,
+                             void *cuda_stream);
 voila_status voila_belief_update_host(voila_ctx *ctx, const void *particles, int N, int32_t action,
                                       const float *observation, const float *weights,
                                       uint64_t seed, void *particles_out, float *weights_out,

@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
     float *xa = smem, *xb = xa + KW * R, *s = xb + KW * R, *sn = s + S * R, *wit = sn + S * R;
     float *obs = wit + O * R, *red = obs + O * R, *G = red + kWarps * R;
     float *alive = G + R;  // 1 while the row's episode runs (terminal regions, voila_terminal)
-    const int tile = blockIdx.x, q = blockIdx.y, p0 = tile * R;
+    const int tile = blockIdx.y, q = blockIdx.x, p0 = tile * R;  // q on x: no 65535 limit on the sequences
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     load_particles<EMU>(a.particles, S, a.P, p0, s);
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(kThreads) rollout_ffma_kernel(const ModelDev m
 
     float disc = 1.0f;
     for (int t = 0; t < a.H; ++t) {
-        const int act_t = __ldg(a.action_seqs + (size_t)q * a.H + t);
+        const int act_t = clamp_action(__ldg(a.action_seqs + (size_t)q * a.H + t), A);
         // reward on the CURRENT state (reading R7)
         const float rew = tile_reward(m.reward, S, s, act_t, red);
         if (warp == 0) {
@@ -677,7 +677,7 @@ cudaError_t launch_weight_sum(const float *weights, int n, double *wsum_out, cud
 
 cudaError_t launch_rollout_ffma(const ModelDev &m, const RolloutArgs &a, bool bf16, cudaStream_t st) {
     const size_t smem = ffma_smem_bytes(m);
-    dim3 grid(a.tiles, a.Q);
+    dim3 grid(a.Q, a.tiles);
     cudaError_t e;
     if (bf16) {
         if ((e = set_smem(rollout_ffma_kernel<true>, smem)) != cudaSuccess) return e;

@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
         auto step_reward = [&]() {  // non-quadratic reward kinds: R(s_t, a_t) from the state words
             if (half == 0 && p.reward_kind != VOILA_R_NEG_QUADRATIC) {
                 float r = reward_from_state(persist, S, p.reward_kind, p.reward_param);
-                if (p.action_cost) r += __ldg(p.action_cost + __ldg(p.seqs + (size_t)q * p.H + t));
+                if (p.action_cost) r += __ldg(p.action_cost + clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A));
                 G = fmaf(disc, r, G);
             }
         };
@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) rollout_tc_kernel(const TcRollo
             arrive_event();
         }
         for (int step = 0; step < total_steps; ++step) {
-            const int a_t = __ldg(p.seqs + (size_t)q * p.H + t);
+            const int a_t = clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A);
             for (int li = 0; li < n_layers; ++li) {
                 const TcLayer l = L[li];
                 const float *bias = p.bias + l.bias_off + (l.bias_per_action ? (size_t)a_t * l.n_pad : 0);

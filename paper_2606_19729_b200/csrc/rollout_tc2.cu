@@ -477,7 +477,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         auto step_reward = [&]() {  // non-quadratic reward kinds: R(s_t, a_t) from the state words
             if (half == 0 && p.reward_kind != VOILA_R_NEG_QUADRATIC) {
                 float r = reward_from_state(persist, S, p.reward_kind, p.reward_param);
-                if (p.action_cost) r += __ldg(p.action_cost + __ldg(p.seqs + (size_t)q * p.H + t));
+                if (p.action_cost) r += __ldg(p.action_cost + clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A));
                 pay(r);
             }
         };
@@ -488,7 +488,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         const int tid_e = (int)threadIdx.x - 128;
         float4 pa_reg[2] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
         auto refresh_issue = [&](int q_next, int t_next) {
-            const int a_next = __ldg(p.seqs + (size_t)q_next * p.H + t_next);
+            const int a_next = clamp_action(__ldg(p.seqs + (size_t)q_next * p.H + t_next), p.A);
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 const int li = p.hdr.pa_layer[i];
@@ -519,7 +519,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             arrive_event();
         }
         for (int step = 0; step < total_steps; ++step) {
-            const int a_t = __ldg(p.seqs + (size_t)q * p.H + t);
+            const int a_t = clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A);
 #ifdef VOILA_T2_TRACE
             es.tl_on = blockIdx.x == 0 && warp == 4 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
 #endif

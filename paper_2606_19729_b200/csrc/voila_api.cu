@@ -436,6 +436,7 @@ voila_status voila_rollout_values(voila_ctx *ctx, const void *particles, int P,
     a.final_states_out = final_states_out;
     const int tile_rows = use_tc(ctx) ? 128 : kTileRows;
     a.tiles = use_tc2(ctx) ? 2 * ((P + 255) / 256) : (P + tile_rows - 1) / tile_rows;
+    if (a.tiles > 65535) return VOILA_ERR_INVALID_ARG;  // grid.y of the CUDA-core kernel (P > 2^21 particles)
     double *wsum = reinterpret_cast<double *>(w + L.wsum);
 
     cudaError_t e = launch_weight_sum(weights, P, wsum, st);
@@ -499,7 +500,9 @@ voila_status voila_belief_update_ess(voila_ctx *ctx, const void *particles, int 
     if (!(ess_threshold > 0.0f)) return VOILA_ERR_INVALID_ARG;  // also rejects NaN
     if (misaligned(ess_out) || misaligned(resampled_out)) return VOILA_ERR_INVALID_ARG;
     if (action < 0 || action >= ctx->A) return VOILA_ERR_INVALID_ARG;
-    if (particles_out == particles || proposals_out == particles) return VOILA_ERR_INVALID_ARG;
+    if (particles_out == particles || proposals_out == particles || particles_out == proposals_out)
+        return VOILA_ERR_INVALID_ARG;  // the gather reads proposal rows while other CTAs write particles_out
+    if (((uintptr_t)log_evidence_out & 3u) || ((uintptr_t)dev_status_out & 3u)) return VOILA_ERR_INVALID_ARG;
     if (misaligned(particles) || misaligned(observation) || misaligned(weights) ||
         misaligned(particles_out) || misaligned(weights_out) || misaligned(ancestors_out) ||
         misaligned(post_weights_out) || misaligned(proposals_out))
@@ -837,6 +840,14 @@ voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, in
                                        const int32_t *action_seqs, int Q, int H, const float *weights,
                                        uint64_t seed, float *values_out, float *obs_witness_out,
                                        void *cuda_stream) {
+    return voila_plan_host(ctx, particles, P, action_seqs, Q, H, weights, seed, values_out, obs_witness_out,
+                           nullptr, nullptr, cuda_stream);
+}
+
+voila_status voila_plan_host(voila_ctx *ctx, const void *particles, int P, const int32_t *action_seqs, int Q,
+                             int H, const float *weights, uint64_t seed, float *values_out,
+                             float *obs_witness_out, int32_t *best_q_out, int32_t *best_action_out,
+                             void *cuda_stream) {
     if (!ctx || !particles || !action_seqs || !values_out || P < 1 || Q < 1 || H < 1)
         return VOILA_ERR_INVALID_ARG;
     if (!ctx->stage || P > ctx->res_P || Q > ctx->res_Q || H > ctx->res_H) return VOILA_ERR_WORKSPACE;
@@ -859,6 +870,16 @@ voila_status voila_rollout_values_host(voila_ctx *ctx, const void *particles, in
         reinterpret_cast<float *>(g + s.values),
         obs_witness_out ? reinterpret_cast<float *>(g + s.witness) : nullptr, nullptr, nullptr, cuda_stream);
     if (vs != VOILA_OK) return vs;
+    int32_t *best = reinterpret_cast<int32_t *>(g + s.scalars + 32);  // best q, best action
+    if (best_q_out || best_action_out) {
+        vs = voila_best_action(ctx, reinterpret_cast<const float *>(g + s.values),
+                               reinterpret_cast<const int32_t *>(g + s.actions), Q, H, best, best + 1, cuda_stream);
+        if (vs != VOILA_OK) return vs;
+        if (best_q_out) e = cudaMemcpyAsync(best_q_out, best, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && best_action_out)
+            e = cudaMemcpyAsync(best_action_out, best + 1, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+    }
     e = cudaMemcpyAsync(values_out, g + s.values, (size_t)Q * sizeof(float), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && obs_witness_out)
         e = cudaMemcpyAsync(obs_witness_out, g + s.witness, (size_t)Q * ctx->O * sizeof(float),

@@ -92,6 +92,10 @@ __device__ __forceinline__ float ordered_to_float(int i) {
     return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff);
 }
 
+// An action index as the kernels use it: clamped into [0, A), so that an out-of-range entry of
+// action_seqs can never index past the per-action tables (voila.h: such entries are clamped).
+__device__ __forceinline__ int clamp_action(int a, int A) { return a < 0 ? 0 : (a >= A ? A - 1 : a); }
+
 __device__ __forceinline__ float act_apply(float x, int act) {
     if (act == 1) return x > 0.0f ? x : 0.0f;
     if (act == 2) return x / (1.0f + expf(-x));

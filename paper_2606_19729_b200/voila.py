@@ -27,7 +27,7 @@ EXPORTS = [
     "voila_belief_update_host", "voila_launch_count", "voila_last_rollout_kernel", "voila_last_belief_kernel",
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read", "voila_pw_workspace_bytes", "voila_pw_reserve", "voila_pw_update",
-    "voila_porpp_backup", "voila_diffusion_sample",
+    "voila_porpp_backup", "voila_diffusion_sample", "voila_plan_host",
 ]
 
 
@@ -108,6 +108,8 @@ def load_library():
     lib.voila_porpp_backup_level.restype = i32
     lib.voila_rollout_values_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp]
     lib.voila_rollout_values_host.restype = i32
+    lib.voila_plan_host.argtypes = [vp, vp, i32, vp, i32, i32, vp, u64, vp, vp, vp, vp, vp]
+    lib.voila_plan_host.restype = i32
     lib.voila_belief_update_host.argtypes = [vp, vp, i32, C.c_int32, vp, vp, u64, vp, vp, vp, vp, vp,
                                              vp]
     lib.voila_belief_update_host.restype = i32
@@ -478,6 +480,17 @@ class Voila:
             self._h, _hptr(particles), P, _hptr(action_seqs), Q, H, _hptr(weights),
             C.c_uint64(int(seed)), _hptr(values_out), _hptr(witness_out), self._stream()),
             "voila_rollout_values_host")
+        return values_out
+
+    def voila_plan_host(self, particles, action_seqs, weights, seed, values_out, best_out, witness_out=None):
+        """Rollout + executed action through host buffers; best_out: host int32 [2] = (q*, first action)."""
+        P, Q, H = particles.shape[0], action_seqs.shape[0], action_seqs.shape[1]
+        self._ensure(P=P, Q=Q, H=H)
+        bq = _hptr(best_out)
+        ba = C.c_void_p(bq.value + 4)
+        self._check(self.lib.voila_plan_host(
+            self._h, _hptr(particles), P, _hptr(action_seqs), Q, H, _hptr(weights), C.c_uint64(int(seed)),
+            _hptr(values_out), _hptr(witness_out), bq, ba, self._stream()), "voila_plan_host")
         return values_out
 
     def voila_belief_update_host(self, particles, action, observation, weights, seed, particles_out,

@@ -34,9 +34,23 @@ def value_err(v, ref):
     return float(np.max(np.abs(v - ref) / den))
 
 
+def elem_err(x, ref):
+    """max_i |x_i - ref_i| / max(|ref_i|, rms(ref)): element-wise, so that a wrong SMALL component cannot
+    hide under a large one (the norm ratios above can); the rms floor keeps zero crossings meaningful."""
+    x = np.asarray(x, np.float64)
+    ref = np.asarray(ref, np.float64)
+    rms = float(np.sqrt(np.mean(ref ** 2)))
+    den = np.maximum(np.abs(ref), rms if rms > 0 else 1.0)
+    return float(np.max(np.abs(x - ref) / den))
+
+
+ELEM_FACTOR = 4.0  # element-wise bound = 4 x the north-star tolerance (a per-element error may exceed the norm ratio)
+
+
 def assert_close(x, ref, tol, what=""):
-    e2, ei = rel_l2(x, ref), rel_inf(x, ref)
+    e2, ei, ee = rel_l2(x, ref), rel_inf(x, ref), elem_err(x, ref)
     assert e2 <= tol and ei <= tol, f"{what}: rel_l2={e2:.3e} rel_inf={ei:.3e} > {tol:.1e}"
+    assert ee <= ELEM_FACTOR * tol, f"{what}: element-wise {ee:.3e} > {ELEM_FACTOR * tol:.1e}"
 
 
 def t2n(t):

@@ -18,14 +18,25 @@ def torch_cuda():
     return torch
 
 
-def _sample_pairs(P, Q, n, rng):
+def _sample_pairs(P, Q, n, rng, n_clusters=74):
+    """Corners, then pairs spread over the work units of every CTA pair: unit = q * ceil(P/256) + block,
+    units go round-robin over the CTA pairs, so the first and the last unit of each pair are hit."""
     pairs = {(0, 0), (P - 1, Q - 1), (P - 1, 0), (0, Q - 1), (P // 2 + 1, Q // 2 - 1)}
+    bpq = (P + 255) // 256
+    n_units = bpq * Q
+    for c in range(min(n_clusters, n_units)):
+        last = c + ((n_units - 1 - c) // n_clusters) * n_clusters
+        for unit in (c, last):
+            q, blk = divmod(unit, bpq)
+            p = min(P - 1, blk * 256 + int(rng.integers(256)))
+            if len(pairs) < n:
+                pairs.add((p, q))
     while len(pairs) < n:
         pairs.add((int(rng.integers(P)), int(rng.integers(Q))))
     return sorted(pairs)
 
 
-@pytest.mark.parametrize("cfg_idx,n_pairs", [(1, 64), (2, 48), (3, 32), (5, 24)])
+@pytest.mark.parametrize("cfg_idx,n_pairs", [(1, 64), (2, 96), (3, 160), (5, 256)])
 def test_rollout_full_size_sampled(torch_cuda, oracle, cfg_idx, n_pairs):
     import paper_2606_19729_b200 as vl
     torch = torch_cuda
