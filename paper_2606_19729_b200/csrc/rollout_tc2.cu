@@ -1107,10 +1107,19 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
 #endif
             (void)tr_empty; (void)tr_start;
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer: leader CTA only.  The whole warp walks the tile program (waits are
-        // warp-uniform); one elected lane issues the MMAs and commits. =====
+    } else if (warp == 1 || (warp == 3 && p.hdr.n_issuers == 2)) {
+        // ===== MMA issuer(s): leader CTA only.  The whole warp walks the tile program (waits are
+        // warp-uniform); one elected lane issues the MMAs and commits.  With two issuers (warps 1 and
+        // 3, on different schedulers) every tile belongs to one of them: the slots of a two-slot
+        // program, else the accumulator blocks by parity.  Each walks the whole program, keeps the ring
+        // position and the chunk-free sequence for the tiles it skips, and issues its own in program
+        // order: a tile only ever depends on earlier program items, so the earliest unfinished item is
+        // always at the head of its owner's queue (no deadlock), and one slot no longer waits behind
+        // the other's tiles.  The issuer loop is ~150 instructions per 512-cycle tile on a scheduler it
+        // shares with four epilogue warps (ncu: the tensor queue is never full); two warps halve that. =====
         if (rank == 0) {
+            const bool two = p.hdr.n_issuers == 2;
+            const uint32_t owner = warp == 3 ? 1u : 0u;
             uint32_t stage = 0, phase = 0;
             uint32_t tl_n = 0;
             (void)tl_n;
@@ -1124,10 +1133,18 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
+                    if (two && ((T[i].misc >> 7) & 1u) != owner) {  // the other issuer's tile: books only
+                        free_seq += (T[i].misc >> 6) & 1u;
+                        if (++stage == (uint32_t)n_stages) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
+                        continue;
+                    }
                     const uint4 r0 = *reinterpret_cast<const uint4 *>(T + i);
                     const uint4 r1 = *(reinterpret_cast<const uint4 *>(T + i) + 1);
 #ifdef VOILA_T2_TRACE
-                    const bool tl_on = cluster_id == 0 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+                    const bool tl_on = cluster_id == 0 && warp == 1 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
 #endif
                     // events needed from epilogue set 0 and set 1 (-100000: nothing to wait for)
                     const int n0 = base + (int)r1.x, n1 = base + (int)r1.y;
@@ -1202,7 +1219,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                 blk_base += p.hdr.blocks_per_step;
             }
 #ifdef VOILA_T2_TRACE
-            if (cluster_id == 0 && elect_one_sync()) {
+            if (cluster_id == 0 && warp == 1 && elect_one_sync()) {
                 g_t2_trace[4] = tr_evt;
                 g_t2_trace[5] = tr_full;
                 g_t2_trace[6] = clock64() - tr_start;
@@ -1409,6 +1426,7 @@ struct Builder2 {
                 t.kc0 = (uint8_t)(chunk_off + kc0);
                 t.nk = (uint8_t)nk;
                 t.rows8 = (uint8_t)(half / 8);
+                t.pad = (uint8_t)slot;  // two-slot programs: the slot (= the MMA issuer warp that owns the tile)
                 int need = blk_need;
                 for (int c = 0; c < nk; ++c) need = std::max(need, a_ready[chunk_off + kc0 + c]);
                 t.need = (int16_t)need;
@@ -1657,6 +1675,8 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     int cols = 32;
     while (cols < max_n) cols *= 2;
     g.hdr.tmem_cols = cols;
+    g.hdr.n_issuers = 2;
+    if (const char *e = getenv("VOILA_T2_ISSUERS")) g.hdr.n_issuers = atoi(e) == 1 ? 1 : 2;  // A/B knob
     g.hdr.n_stages = 8;
     if (const char *e = getenv("VOILA_T2_STAGES")) g.hdr.n_stages = std::max(2, std::min(8, atoi(e)));
     while (g.hdr.n_stages > 2 && smem2_map(g.hdr).total + 1024 > kMaxDynSmem2) --g.hdr.n_stages;
@@ -1675,7 +1695,8 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         d.need_s0 = s0;
         d.need_s1 = need2 != need ? s1 : -100000;
         d.chunk_b16 = ((uint32_t)t.rows8 * 1024u) >> 4;
-        d.misc = (uint32_t)t.nk | ((uint32_t)(t.flags & 7u) << 4) | ((uint32_t)t.blk << 8) |
+        const uint32_t owner = pb.dual ? (uint32_t)t.pad : ((uint32_t)t.blk & 1u);
+        d.misc = (uint32_t)t.nk | ((uint32_t)(t.flags & 7u) << 4) | (owner << 7) | ((uint32_t)t.blk << 8) |
                  ((uint32_t)((int)t.nk * (int)t.rows8 * 8) << 16);
         dev_tiles.push_back(d);
     }

@@ -87,7 +87,7 @@ struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block 
     // the latest earlier event of the OTHER set (= need when there is one set only).
     int16_t need2;
     uint8_t need_set;  // 0 | 1: the set that publishes event `need`
-    uint8_t pad;
+    uint8_t pad;       // host scratch: the tile's slot in a two-slot program
 };
 static_assert(sizeof(T2Tile) == 20, "T2Tile is copied to shared memory as 32-bit words");
 
@@ -103,7 +103,9 @@ struct T2TileDev {
     int32_t need_s0;    // event of epilogue set 0 to wait for (relative to the step), -100000: none
     int32_t need_s1;    // event of epilogue set 1 to wait for, -100000: none
     uint32_t chunk_b16; // weight bytes of one K chunk in the stage / 16 (descriptor units)
-    uint32_t misc;      // nk | flags << 4 | blk << 8 | rows << 16   (rows = weight rows per CTA in the stage)
+    uint32_t misc;      // nk | flags << 4 | owner << 7 | blk << 8 | rows << 16   (rows = weight rows per CTA in
+                        // the stage; owner = the issuer warp the tile belongs to: its slot in a two-slot
+                        // program, else the parity of its accumulator block)
 };
 static_assert(sizeof(T2TileDev) == 32, "T2TileDev is read with two 16-byte loads");
 
@@ -117,6 +119,7 @@ struct T2Header {
     int slot_chunks;      // operand chunks per slot
     int g_in_chunks;      // belief program: operand chunks of the state tower's input
     int e_off, e_pad;     // belief program: f(o) in the shared-memory table (float offset, padded length)
+    int n_issuers;        // 1 | 2 MMA issuer warps (warp 1, warp 3): a tile belongs to issuer (misc >> 7) & 1
 };
 
 }  // namespace voila
