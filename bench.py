@@ -647,9 +647,12 @@ def run_voila(args):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": achieved / peak, "traffic": None,
                 "peak_kind": "fp32 FFMA: SMs x 128 lanes x 2 flop x max SM clock (CUDA-core kernel)"}
-    # roof["traffic"] (DRAM bytes per launch) is only ever a value measured by ncu on a launch of the
-    # SAME size; none is committed for the full-size launch, so the key stays null (the Q=37 capture,
-    # profiles/r01f_rollout_tc2x_cfg5.md, read 4.4 MB: inputs once, the horizon loop never touches HBM)
+    # roof["traffic"]: DRAM bytes of ONE launch (dram__bytes_read.sum + dram__bytes_write.sum) from the
+    # committed `ncu --set full` capture of this kernel at THIS size (full-size CFG5); null for any other
+    # size or kernel (inputs are read once, per-(q, tile) partial sums written; the horizon loop never touches HBM)
+    if cfg.index == 5 and not reduced and "rollout_tc2x" in ctx.voila_last_rollout_kernel():
+        roof["traffic"] = 5400576 + 25332992
+        roof["traffic_from"] = "profiles/r02b_rollout_tc2x_cfg5_fullsize.md (ncu --set full, the full-size launch)"
     roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
                  "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
                  "share_of_step": k_ms / ms_per_step})

@@ -30,7 +30,7 @@ __global__ void bu_init_kernel(ScanBuffers sb, int tiles) {
     if (i == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.done_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(kObsThreads) bu_init_obs_kernel(ScanBuffers sb
     if (tid == 0) {
         ScanState z;
         z.total_q = 0; z.offset_u = 0; z.sum_v = 0.0; z.sum_w = 0.0;
-        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
+        z.max_logit = 0.0f; z.status = 0; z.tile_counter = 0; z.done_counter = 0; z.resample = 1; z.ess = 0.0; z.inv_sum_v = 0.0;
         *sb.state = z;
         *sb.max_ordered = (int)0x80000000;
     }
@@ -134,19 +134,94 @@ __device__ __forceinline__ u64 quantise_weight(float v) {
     return __float2ull_rz(v * 4294967296.0f);  // power-of-two scaling is exact
 }
 
+// W = C_{N-1}, comb offset U, log evidence, status, the ESS decision: run by ONE CTA of T threads once
+// every scan tile is published (the last scan CTA, or bu_finalize_kernel).  Fixed-order double sums.
+template <int T>
+__device__ __forceinline__ void finalize_block(const ScanBuffers &sb, int N, int tiles, const FinalizeArgs &f,
+                                               double *sh /* [T] shared */) {
+    const int tid = threadIdx.x;
+    // prior-weight partials (one per 32 particles: 32768 at N = 2^20): 8 independent loads per round
+    // (the loop is latency-bound); fixed order, so the sum is bit-reproducible
+    double acc = 0.0;
+    if (f.has_prior) {
+        int i = tid;
+        for (; i + 7 * T < f.n_wsum_parts; i += 8 * T) {
+            double t[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) t[u] = __ldcg(sb.part_wsum + i + u * T);
+            acc += ((t[0] + t[1]) + (t[2] + t[3])) + ((t[4] + t[5]) + (t[6] + t[7]));
+        }
+        for (; i < f.n_wsum_parts; i += T) acc += __ldcg(sb.part_wsum + i);
+    }
+    sh[tid] = acc;
+    __syncthreads();
+    for (int o = T / 2; o > 0; o >>= 1) {
+        if (tid < o) sh[tid] += sh[tid + o];
+        __syncthreads();
+    }
+    const double sum_wp = sh[0];
+    __syncthreads();
+    // sum v (threads [0, T/2)) and sum v^2 (threads [T/2, T)) of the scan tiles: two trees at once
+    constexpr int Hh = T / 2;
+    acc = 0.0;
+    for (int i = tid & (Hh - 1); i < tiles; i += Hh) acc += __ldcg(sb.tile_sumv + (tid < Hh ? 0 : tiles) + i);
+    sh[tid] = acc;
+    __syncthreads();
+    for (int o = Hh / 2; o > 0; o >>= 1) {
+        if ((tid & (Hh - 1)) < o) sh[tid] += sh[tid + o];
+        __syncthreads();
+    }
+    const double sum_v = sh[0], sum_v2 = sh[Hh];
+    if (tid == 0) {
+        const double sum_w = f.has_prior ? sum_wp : (double)N;
+        const u64 W = ld_u64_volatile(&sb.state->total_q);
+        float m = 0.0f;
+        int status = 0;
+        if (f.from_logits) {
+            m = ordered_to_float(*reinterpret_cast<volatile int *>(sb.max_ordered));
+            if (!(fabsf(m) < INFINITY)) status = 1;
+        }
+        if (W == 0ull) status = 1;
+        const uint4 x = noise_words(f.seed, 0u, 0u, 0u, kStreamResample, 0u);
+        const u64 x0 = (u64)x.x;
+        // U = (x0 * W) >> 32 from the 96-bit product
+        const u64 lo = x0 * W, hi = __umul64hi(x0, W);
+        sb.state->offset_u = (hi << 32) | (lo >> 32);
+        sb.state->sum_v = sum_v;
+        sb.state->inv_sum_v = sum_v > 0.0 ? 1.0 / sum_v : 0.0;
+        sb.state->sum_w = sum_w;
+        sb.state->max_logit = m;
+        sb.state->status = status;
+        // adaptive resampling (SURVEY 8f f3): resample iff ESS < ess_threshold * N (+inf: always)
+        const double ess = (status == 0 && sum_v2 > 0.0) ? sum_v * sum_v / sum_v2 : 0.0;
+        const int resample = status == 0 && (isinf(f.ess_threshold) || ess < (double)f.ess_threshold * (double)N);
+        sb.state->ess = ess;
+        sb.state->resample = resample;
+        if (f.ess_out) *f.ess_out = (float)ess;
+        if (f.resampled_out) *f.resampled_out = resample;
+        if (f.dev_status_out) *f.dev_status_out = status;
+        if (f.log_evidence_out)
+            *f.log_evidence_out = status ? -INFINITY : (float)((double)m + log(sum_v) - log(sum_w));
+    }
+}
+
 template <bool FROM_LOGITS>
 __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers sb,
                                                                    const float *__restrict__ in, int N,
-                                                                   float *post_weights_out) {
+                                                                   float *post_weights_out, const FinalizeArgs fin) {
     constexpr int kWarpsS = kScanThreads / 32;
+    __shared__ double fin_sh[kScanThreads];
+    __shared__ int tile_s, last_s;
     __shared__ u64 warp_tot[kWarpsS];
     __shared__ u64 look_tot[kWarpsS];
     __shared__ int look_first[kWarpsS];
     __shared__ double dsum[kWarpsS], dsum2[kWarpsS];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // Tile = CTA index: a look-back only waits for lower-numbered CTAs, which the hardware
-    // dispatches first (the same assumption CUB's single-pass scan makes).
-    const int tile = (int)blockIdx.x;
+    // Tile = ticket taken at start: a look-back only waits for tiles whose CTA has already started,
+    // whatever order the hardware dispatches the CTAs in.
+    if (tid == 0) tile_s = (int)atomicAdd(&sb.state->tile_counter, 1u);
+    __syncthreads();
+    const int tile = tile_s;
     const int base = tile * kScanTile + tid * kItems;
 
     float m = 0.0f;
@@ -278,79 +353,23 @@ __global__ void __launch_bounds__(kScanThreads) weight_scan_kernel(ScanBuffers s
                 if (post_weights_out) post_weights_out[base + i] = x[i];
             }
     }
+    // the last CTA to get here finalises (W, U, evidence, status, ESS): one launch less per update
+    if (fin.enabled) {
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) last_s = atomicAdd(&sb.state->done_counter, 1u) == gridDim.x - 1u;
+        __syncthreads();
+        if (last_s) {
+            __threadfence();
+            finalize_block<kScanThreads>(sb, N, (int)gridDim.x, fin, fin_sh);
+        }
+    }
 }
 
 constexpr int kFinThreads = 1024;
-
-__global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb, int N, int tiles, int n_wsum_parts,
-                                                                  int has_prior, int from_logits, uint64_t seed,
-                                                                  float ess_threshold, float *log_evidence_out,
-                                                                  int32_t *dev_status_out, float *ess_out,
-                                                                  int32_t *resampled_out) {
+__global__ void __launch_bounds__(kFinThreads) bu_finalize_kernel(ScanBuffers sb, int N, int tiles, FinalizeArgs fin) {
     __shared__ double sh[kFinThreads];
-    const int tid = threadIdx.x;
-    // prior-weight partials (one per 32 particles: 32768 at N = 2^20): all 1024 threads, 8 independent
-    // loads per round (the loop is latency-bound); fixed order, so the sum is bit-reproducible
-    double acc = 0.0;
-    if (has_prior) {
-        int i = tid;
-        for (; i + 7 * kFinThreads < n_wsum_parts; i += 8 * kFinThreads) {
-            double t[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) t[u] = sb.part_wsum[i + u * kFinThreads];
-            acc += ((t[0] + t[1]) + (t[2] + t[3])) + ((t[4] + t[5]) + (t[6] + t[7]));
-        }
-        for (; i < n_wsum_parts; i += kFinThreads) acc += sb.part_wsum[i];
-    }
-    sh[tid] = acc;
-    __syncthreads();
-    for (int o = kFinThreads / 2; o > 0; o >>= 1) {
-        if (tid < o) sh[tid] += sh[tid + o];
-        __syncthreads();
-    }
-    const double sum_wp = sh[0];
-    __syncthreads();
-    // sum v (threads [0, 512)) and sum v^2 (threads [512, 1024)) of the scan tiles: two trees at once
-    acc = 0.0;
-    for (int i = tid & 511; i < tiles; i += 512) acc += sb.tile_sumv[(tid < 512 ? 0 : tiles) + i];
-    sh[tid] = acc;
-    __syncthreads();
-    for (int o = 256; o > 0; o >>= 1) {
-        if ((tid & 511) < o) sh[tid] += sh[tid + o];
-        __syncthreads();
-    }
-    const double sum_v = sh[0], sum_v2 = sh[512];
-    if (tid == 0) {
-        const double sum_w = has_prior ? sum_wp : (double)N;
-        const u64 W = sb.state->total_q;
-        float m = 0.0f;
-        int status = 0;
-        if (from_logits) {
-            m = ordered_to_float(*sb.max_ordered);
-            if (!(fabsf(m) < INFINITY)) status = 1;
-        }
-        if (W == 0ull) status = 1;
-        const uint4 x = noise_words(seed, 0u, 0u, 0u, kStreamResample, 0u);
-        const u64 x0 = (u64)x.x;
-        // U = (x0 * W) >> 32 from the 96-bit product
-        const u64 lo = x0 * W, hi = __umul64hi(x0, W);
-        sb.state->offset_u = (hi << 32) | (lo >> 32);
-        sb.state->sum_v = sum_v;
-        sb.state->inv_sum_v = sum_v > 0.0 ? 1.0 / sum_v : 0.0;
-        sb.state->sum_w = sum_w;
-        sb.state->max_logit = m;
-        sb.state->status = status;
-        // adaptive resampling (SURVEY 8f f3): resample iff ESS < ess_threshold * N (+inf: always)
-        const double ess = (status == 0 && sum_v2 > 0.0) ? sum_v * sum_v / sum_v2 : 0.0;
-        const int resample = status == 0 && (isinf(ess_threshold) || ess < (double)ess_threshold * (double)N);
-        sb.state->ess = ess;
-        sb.state->resample = resample;
-        if (ess_out) *ess_out = (float)ess;
-        if (resampled_out) *resampled_out = resample;
-        if (dev_status_out) *dev_status_out = status;
-        if (log_evidence_out)
-            *log_evidence_out = status ? -INFINITY : (float)((double)m + log(sum_v) - log(sum_w));
-    }
+    finalize_block<kFinThreads>(sb, N, tiles, fin, sh);
 }
 
 // N*C > k*W + U as 128-bit integers.
@@ -509,10 +528,12 @@ cudaError_t launch_bu_init_obs(const ScanBuffers &sb, int N, const MlpDev &f, co
 }
 
 cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bool from_logits,
-                               float *post_weights_out, cudaStream_t st) {
+                               float *post_weights_out, cudaStream_t st, const FinalizeArgs *fin) {
     const int tiles = scan_tiles(N);
-    if (from_logits) weight_scan_kernel<true><<<tiles, kScanThreads, 0, st>>>(sb, in, N, post_weights_out);
-    else weight_scan_kernel<false><<<tiles, kScanThreads, 0, st>>>(sb, in, N, post_weights_out);
+    FinalizeArgs f{};
+    if (fin) f = *fin;
+    if (from_logits) weight_scan_kernel<true><<<tiles, kScanThreads, 0, st>>>(sb, in, N, post_weights_out, f);
+    else weight_scan_kernel<false><<<tiles, kScanThreads, 0, st>>>(sb, in, N, post_weights_out, f);
     return cudaGetLastError();
 }
 
@@ -520,10 +541,16 @@ cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, b
                                uint64_t seed, float *log_evidence_out, int32_t *dev_status_out,
                                cudaStream_t st, float ess_threshold, float *ess_out, int32_t *resampled_out) {
     // n_wsum_parts < 0 marks the stage-level resampler (weights given directly, no logits)
-    const int from_logits = n_wsum_parts >= 0;
-    bu_finalize_kernel<<<1, kFinThreads, 0, st>>>(sb, N, scan_tiles(N), n_wsum_parts < 0 ? 0 : n_wsum_parts,
-                                          has_prior ? 1 : 0, from_logits, seed, ess_threshold, log_evidence_out,
-                                          dev_status_out, ess_out, resampled_out);
+    FinalizeArgs f{};
+    f.enabled = 1;
+    f.from_logits = n_wsum_parts >= 0;
+    f.n_wsum_parts = n_wsum_parts < 0 ? 0 : n_wsum_parts;
+    f.has_prior = has_prior ? 1 : 0;
+    f.seed = seed;
+    f.ess_threshold = ess_threshold;
+    f.log_evidence_out = log_evidence_out; f.ess_out = ess_out;
+    f.dev_status_out = dev_status_out; f.resampled_out = resampled_out;
+    bu_finalize_kernel<<<1, kFinThreads, 0, st>>>(sb, N, scan_tiles(N), f);
     return cudaGetLastError();
 }
 

@@ -564,14 +564,21 @@ voila_status voila_belief_update_ess(voila_ctx *ctx, const void *particles, int 
         ctx->last_belief_kernel = bf16 ? "bu_propose_score_ffma_kernel<bf16>" : "bu_propose_score_ffma_kernel<fp32>";
     }
     {
+        // scan; its last CTA finalises (W, comb offset, evidence, status, ESS decision)
+        FinalizeArgs fin{};
+        fin.enabled = 1;
+        fin.n_wsum_parts = n_parts;
+        fin.has_prior = weights != nullptr;
+        fin.from_logits = 1;
+        fin.seed = seed;
+        fin.ess_threshold = ess_threshold;
+        fin.log_evidence_out = log_evidence_out; fin.ess_out = ess_out;
+        fin.dev_status_out = dev_status_out; fin.resampled_out = resampled_out;
         ProfScope prof(ctx, VOILA_K_SCAN, st);
-        e = launch_weight_scan(sb, a.logits, N, true, post_weights_out, st);
+        e = launch_weight_scan(sb, a.logits, N, true, post_weights_out, st, &fin);
     }
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    e = launch_bu_finalize(sb, N, n_parts, weights != nullptr, seed, log_evidence_out, dev_status_out, st,
-                           ess_threshold, ess_out, resampled_out);
-    if (e != cudaSuccess) return cuda_fail(ctx, e);
-    ctx->launches += 2;
+    ctx->launches += 1;
     return run_resample(ctx, sb, N, a.proposals, particles_out, weights_out, ancestors_out, st, a.logits, true);
 }
 
@@ -586,11 +593,16 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
     const Layout L = make_layout(ctx, ctx->res_P, ctx->res_Q, ctx->res_N);
     const ScanBuffers sb = scan_buffers(ctx, L);
     cudaError_t e = launch_bu_init(sb, N, st);
-    if (e == cudaSuccess) e = launch_weight_scan(sb, v, N, false, nullptr, st);
-    if (e == cudaSuccess)
-        e = launch_bu_finalize(sb, N, -1, false, seed, nullptr, dev_status_out, st, INFINITY, nullptr, nullptr);
+    if (e == cudaSuccess) {
+        FinalizeArgs fin{};
+        fin.enabled = 1;
+        fin.seed = seed;
+        fin.ess_threshold = INFINITY;
+        fin.dev_status_out = dev_status_out;
+        e = launch_weight_scan(sb, v, N, false, nullptr, st, &fin);
+    }
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    ctx->launches += 3;
+    ctx->launches += 2;
     return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st, v, false);
 }
 

@@ -120,7 +120,8 @@ struct ScanState {
     double sum_w;
     float max_logit;
     int status;
-    unsigned int tile_counter;
+    unsigned int tile_counter;   // ticket: scan CTAs take their tile index in start order (look-back never waits on a later start)
+    unsigned int done_counter;   // scan CTAs that have published everything: the last one finalises
     int resample;        // 1: resample (always, unless adaptive resampling found ESS >= threshold * N)
     double ess;          // effective sample size (sum v)^2 / sum v^2 of the posterior weights
     double inv_sum_v;    // 1 / sum v (normalised weights without resampling)

@@ -35,9 +35,18 @@ cudaError_t launch_bu_init(const ScanBuffers &sb, int N, cudaStream_t st);
 bool obs_tower_fits(const MlpDev &f);
 cudaError_t launch_bu_init_obs(const ScanBuffers &sb, int N, const MlpDev &f, const float *obs, float *e_out,
                                bool bf16, cudaStream_t st);
+// What the scan's last CTA does once every tile is published (the former bu_finalize launch): W, the
+// comb offset U, log evidence, status, the ESS decision.  enabled = 0: scan only (progressive widening).
+struct FinalizeArgs {
+    int enabled, n_wsum_parts, has_prior, from_logits;
+    uint64_t seed;
+    float ess_threshold;
+    float *log_evidence_out, *ess_out;
+    int32_t *dev_status_out, *resampled_out;
+};
 // from_logits: v_i = exp(L_i - max) (belief update) ; else v_i = in[i] (stage-level resampler)
 cudaError_t launch_weight_scan(const ScanBuffers &sb, const float *in, int N, bool from_logits,
-                               float *post_weights_out, cudaStream_t st);
+                               float *post_weights_out, cudaStream_t st, const FinalizeArgs *fin = nullptr);
 // ess_threshold: resample iff ESS < ess_threshold * N (INFINITY: always); ess_out / resampled_out may be null
 cudaError_t launch_bu_finalize(const ScanBuffers &sb, int N, int n_wsum_parts, bool has_prior,
                                uint64_t seed, float *log_evidence_out, int32_t *dev_status_out,
