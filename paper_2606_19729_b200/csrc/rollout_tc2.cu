@@ -169,6 +169,8 @@ __device__ __forceinline__ float4 ld_shared_f4(uint32_t addr) {
 template <int ACT>
 __device__ __forceinline__ void hidden_store16(const uint32_t (&v)[16], uint32_t bias_u32, uint32_t row_addr,
                                                uint32_t sw0, uint32_t sw1) {
+    // (loading the 16 biases ahead of the TMEM wait was tried: more live registers, spills in the
+    // 16-warp rollout kernel, CFG5 1140 -> 1073 TFLOP/s)
     uint32_t o[8];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -829,6 +831,15 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             const float *bias = sbias + l.sbias_off;
             const uint32_t a_slot = a_u32 + (uint32_t)l.chunk_off * kT2ChunkBytes;
             const uint32_t taddr = lane_taddr + (uint32_t)l.col_off;
+            if (my_slot >= 0 && p.hdr.split_hidden && l.epi == T2_EPI_HIDDEN) {
+                // both sets share the layer: this set takes the chunks of its parity (four epilogue
+                // warps per scheduler on every layer instead of two: a set alone is latency-bound)
+                EpiConst ecs = ec;
+                ecs.st_base += (uint32_t)l.chunk_off * kT2ChunkBytes;
+                ecs.taddr0 += (uint32_t)l.col_off;
+                epi_hidden_layer_par(es, l, (int)l.sbias_off, ecs, my_slot);
+                continue;
+            }
             if (my_slot >= 0 && slot != my_slot) {  // the other set's record: sequence numbers only
                 const bool hid = l.epi == T2_EPI_HIDDEN;
                 es.ev += hid ? (int)(l.n_pad >> 6) : 1;
@@ -1508,7 +1519,7 @@ struct Builder2 {
             for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
             if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE && epi != T2_EPI_DIFFUSE)  // the next layer-1 input is written with this event
                 for (int j = chunk_off; j < std::min(8, chunk_off + slot_chunks); ++j) a_ready[j] = evt;
-            evt_set.push_back(0);
+            evt_set.push_back((uint8_t)((dual && par_split) ? slot : 0));
             ++evt;
         }
         return li;
@@ -1516,20 +1527,16 @@ struct Builder2 {
 
     // After the last layer: the second wait of every tile (see T2Tile::need2).
     void finish_needs() {
-        int last_of_set[2] = {-100000, -100000};  // latest event of each set in a step
-        for (int e = 0; e < evt; ++e) last_of_set[evt_set[e]] = e;
+        // events repeat with period `evt` (one step); a negative index names an event of the previous step
+        auto set_of = [&](int e) { return (int)evt_set[((e % evt) + evt) % evt]; };
         for (T2Tile &t : tiles) {
             const int need = t.need;
-            // negative needs name events of the previous step; -1 is its last event (set 0), and
-            // the dual-slot programs' -2 / -1 are handled by their own in-order slots
-            const int set = need >= 0 ? evt_set[need] : 0;
+            const int set = par_split ? set_of(need) : 0;
             t.need_set = (uint8_t)set;
             int other = -100000;
-            if (par_split) {
-                for (int e = std::min(need, evt) - 1; e >= 0 && other < -1000; --e)
-                    if (evt_set[e] != set) other = e;
-                if (other < -1000 && last_of_set[1 - set] > -1000) other = last_of_set[1 - set] - evt;  // previous step
-            }
+            if (par_split)
+                for (int e = need - 1; e >= need - evt && other < -1000; --e)
+                    if (set_of(e) != set) other = e;
             t.need2 = (int16_t)(other > -1000 ? other : need);
         }
     }
@@ -1675,8 +1682,9 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     int cols = 32;
     while (cols < max_n) cols *= 2;
     g.hdr.tmem_cols = cols;
-    g.hdr.n_issuers = 2;
-    if (const char *e = getenv("VOILA_T2_ISSUERS")) g.hdr.n_issuers = atoi(e) == 1 ? 1 : 2;  // A/B knob
+    g.hdr.split_hidden = (pb.dual && pb.par_split) ? 1 : 0;
+    g.hdr.n_issuers = 1;  // a second issuer warp (warp 3) measured no gain: the epilogue chain sets the pace
+    if (const char *e = getenv("VOILA_T2_ISSUERS")) g.hdr.n_issuers = atoi(e) == 2 ? 2 : 1;  // A/B knob
     g.hdr.n_stages = 8;
     if (const char *e = getenv("VOILA_T2_STAGES")) g.hdr.n_stages = std::max(2, std::min(8, atoi(e)));
     while (g.hdr.n_stages > 2 && smem2_map(g.hdr).total + 1024 > kMaxDynSmem2) --g.hdr.n_stages;
@@ -1809,7 +1817,10 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             for (int dual = 0; dual <= (dual_ok ? 1 : 0); ++dual) {
                 Builder2 pb;
                 pb.policy = policy;
-                if (dual) pb.set_dual(4, 256);
+                if (dual) {
+                    pb.set_dual(4, 256);
+                    pb.par_split = getenv("VOILA_T2_DUAL_SPLIT") != nullptr;  // measured slower (CFG4 676 vs 645 us): off
+                }
                 if (pw) add_generator2_dense(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
                 else add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_PROPOSAL);
                 const voila_mlp &g = d->lik_state;
@@ -1852,7 +1863,10 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         for (int dual = 0; dual <= ((widest <= 256 && rup(in_cols, 64) / 64 <= 4) ? 1 : 0); ++dual) {
             Builder2 pb;
             pb.policy = policy;
-            if (dual) pb.set_dual(4, 256);
+            if (dual) {
+                    pb.set_dual(4, 256);
+                    pb.par_split = getenv("VOILA_T2_DUAL_SPLIT") != nullptr;  // measured slower (CFG4 676 vs 645 us): off
+                }
             add_denoiser2(pb, f, S, A, D);
             T2Program &prog = h->diff[which][dual];
             prog.hdr.g_in_chunks = 0;

@@ -119,6 +119,9 @@ struct T2Header {
     int slot_chunks;      // operand chunks per slot
     int g_in_chunks;      // belief program: operand chunks of the state tower's input
     int e_off, e_pad;     // belief program: f(o) in the shared-memory table (float offset, padded length)
+    int split_hidden;     // two-slot programs: 1 = both sets of epilogue warps share EVERY hidden layer of both
+                          // slots (even / odd chunks), a slot's other layers go to the set of its number;
+                          // 0 = one set per slot
     int n_issuers;        // 1 | 2 MMA issuer warps (warp 1, warp 3): a tile belongs to issuer (misc >> 7) & 1
 };
 
