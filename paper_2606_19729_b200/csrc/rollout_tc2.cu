@@ -79,7 +79,8 @@ struct T2Params {
     float *returns_out;
     float *final_states_out;
     int tiles_per_q, blocks_per_q, n_units;
-    int S, O, A, Nz;
+    int S, O, A, Nz;  // S, Nz: as the operand sees them (padded to multiples of 8); O, A: public
+    int S_io;         // public state width: rows of particles / proposals / final states
     float gamma;
     int reward_kind;
     const float *reward_param;
@@ -411,8 +412,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
                     uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if (8 * u < S && valid)
-                        v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)p_idx * S) + u);
+                    if (8 * u < S && valid) v = load_row_unit(p.particles + (size_t)p_idx * p.S_io, p.S_io, u);
                     persist[4 * u] = v.x; persist[4 * u + 1] = v.y;
                     persist[4 * u + 2] = v.z; persist[4 * u + 3] = v.w;
                 }
@@ -478,7 +478,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         };
         auto step_reward = [&]() {  // non-quadratic reward kinds: R(s_t, a_t) from the state words
             if (half == 0 && p.reward_kind != VOILA_R_NEG_QUADRATIC) {
-                float r = reward_from_state(persist, S, p.reward_kind, p.reward_param);
+                float r = reward_from_state(persist, p.S_io, p.reward_kind, p.reward_param);
                 if (p.action_cost) r += __ldg(p.action_cost + clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A));
                 pay(r);
             }
@@ -637,12 +637,12 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                             if (lane == 0) red_g[qd] = v;
                             if (valid && p.returns_out) p.returns_out[(size_t)q * p.P + p_idx] = G;
                             if (valid && p.final_states_out) {
-                                float *fs = p.final_states_out + ((size_t)q * p.P + p_idx) * S;
+                                float *fs = p.final_states_out + ((size_t)q * p.P + p_idx) * p.S_io;
 #pragma unroll
                                 for (int c2 = 0; c2 < 32; ++c2)
-                                    if (2 * c2 < S) {
+                                    if (2 * c2 < p.S_io) {
                                         fs[2 * c2] = bf16lo(persist[c2]);
-                                        fs[2 * c2 + 1] = bf16hi(persist[c2]);
+                                        if (2 * c2 + 1 < p.S_io) fs[2 * c2 + 1] = bf16hi(persist[c2]);
                                     }
                             }
                         } else if (p.part_witness) {
@@ -762,7 +762,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
         for (int u = 0; u < 8; ++u) {
             if (8 * u < S) {
                 uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                if (valid) v = __ldg(reinterpret_cast<const uint4 *>(p.particles + (size_t)i_idx * S) + u);
+                if (valid) v = load_row_unit(p.particles + (size_t)i_idx * p.S_io, p.S_io, u);
                 st_shared_v4(a_unit_addr(a_slot, row, u), v.x, v.y, v.z, v.w);
             }
         }
@@ -798,9 +798,13 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             const int a_row = valid ? __ldg(p.pw_sim_action + i_idx) : -1;
             const int n_u = (p.A + 7) >> 3;
             for (int u = 0; u < n_u; ++u) {
-                uint32_t wv[4] = {0u, 0u, 0u, 0u};
-                if (a_row >= 0 && (a_row >> 3) == u) wv[(a_row & 7) >> 1] = (a_row & 1) ? 0x3F800000u : 0x00003F80u;
-                st_shared_v4(a_unit_addr(a_slot, row, u_next + u), wv[0], wv[1], wv[2], wv[3]);
+                // bf16 1.0 at column a_row of the block (selects, no dynamically indexed array: that went to local memory)
+                const bool here = a_row >= 0 && (a_row >> 3) == u;
+                const int wsel = (a_row & 7) >> 1;
+                const uint32_t one = (a_row & 1) ? 0x3F800000u : 0x00003F80u;
+                st_shared_v4(a_unit_addr(a_slot, row, u_next + u), (here && wsel == 0) ? one : 0u,
+                             (here && wsel == 1) ? one : 0u, (here && wsel == 2) ? one : 0u,
+                             (here && wsel == 3) ? one : 0u);
             }
             u_next += n_u;
         }
@@ -883,8 +887,8 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                                     st_shared_v4(a_unit_addr(a_slot, row, u), o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2],
                                                  o[4 * h2 + 3]);
                                     if (valid)
-                                        *(reinterpret_cast<uint4 *>(p.bu_proposals + (size_t)i_idx * S) + u) =
-                                            make_uint4(o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2], o[4 * h2 + 3]);
+                                        store_row_unit(p.bu_proposals + (size_t)i_idx * p.S_io, p.S_io, u,
+                                                       make_uint4(o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2], o[4 * h2 + 3]));
                                 }
                             }
                         }
@@ -1390,7 +1394,7 @@ struct Builder2 {
     int add_one(const float *W, int n0, int k0, const float *b, int bias_rows, int epi, int act, int same_as) {
         T2Layer l{};
         const bool hidden = epi == T2_EPI_HIDDEN;
-        const int n_pad = hidden ? n0 : rup(n0, 16);
+        const int n_pad = hidden ? rup(n0, 64) : rup(n0, 16);  // padded neurons: zero weights, zero bias -> act(0) = 0
         const int kc_n = rup(k0, 64) / 64;
         l.bias_off = (uint32_t)bias.size();
         l.n_pad = (uint16_t)n_pad;
@@ -1567,20 +1571,24 @@ struct T2Handle {
     int diff_n1[2] = {0, 0};
     float diff_scale[2] = {1.0f, 1.0f};
     bool roll_x = false;    // rollout runs the 640-thread kernel (two sets of epilogue warps)
+    int Sp = 0, Nzp = 0;    // operand widths of the state and the noise (public widths rounded up to 8)
 };
 
 // Layer 1 of a generator sees the "algorithmic" input [s ; w] (K = S + Nz): the one-hot block is
 // folded into a per-action bias row b1 + W1[:, S + a] (R21).
+// S, Nz are the PUBLIC widths; in the operand the state occupies rup(S, 8) columns and the noise
+// rup(Nz, 8) (paper-shaped states of 39 / 45 coordinates: the pad columns carry zero weights).
 void add_generator2(Builder2 &pb, const voila_mlp &f, int S, int A, int Nz, int last_epi) {
+    const int Sp = rup(S, 8), Nzp = rup(Nz, 8);
     for (int l = 0; l < f.n_layers; ++l) {
         const int K = f.dims[l], N = f.dims[l + 1];
         const bool last = l == f.n_layers - 1;
         if (l == 0) {
-            const int k0 = S + Nz;
-            std::vector<float> W((size_t)N * k0), b((size_t)A * N);
+            const int k0 = Sp + Nzp;
+            std::vector<float> W((size_t)N * k0, 0.0f), b((size_t)A * N);
             for (int j = 0; j < N; ++j) {
                 for (int k = 0; k < S; ++k) W[(size_t)j * k0 + k] = f.W[0][(size_t)j * K + k];
-                for (int k = 0; k < Nz; ++k) W[(size_t)j * k0 + S + k] = f.W[0][(size_t)j * K + S + A + k];
+                for (int k = 0; k < Nz; ++k) W[(size_t)j * k0 + Sp + k] = f.W[0][(size_t)j * K + S + A + k];
                 for (int a = 0; a < A; ++a)
                     b[(size_t)a * N + j] = f.b[0][j] + h_bf16_round(f.W[0][(size_t)j * K + S + a]);
             }
@@ -1753,7 +1761,24 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
 
 }  // namespace
 
-bool tc2_supported(const voila_model_desc *d, std::string *why) { return tc_supported(d, why); }
+// The CTA-pair programs pad what the MMA shapes want (state / noise columns to multiples of 8, hidden
+// widths to multiples of 64) when the weights are packed; the public buffers keep their widths.
+bool tc2_supported(const voila_model_desc *d, std::string *why) {
+    auto fail = [&](const char *m) {
+        if (why) *why = m;
+        return false;
+    };
+    if (d->prec != VOILA_PREC_BF16) return fail("tcgen05 path is the bf16 mode");
+    if (d->state_dim < 1 || d->state_dim > 64) return fail("state_dim must be at most 64");
+    if (d->obs_dim < 1 || d->obs_dim > 64) return fail("obs_dim must be at most 64");
+    if (d->noise_dim < 1 || d->noise_dim > 32) return fail("noise_dim must be 1 .. 32");
+    for (const voila_mlp *f : {&d->f_T, &d->f_Z}) {
+        if (f->n_layers < 2) return fail("generator needs at least one hidden layer");
+        for (int l = 1; l < f->n_layers; ++l)
+            if (f->dims[l] > 512) return fail("hidden widths must be at most 512");
+    }
+    return true;
+}
 
 namespace {
 // The state tower g fits the belief program when its hidden widths are MMA-block shaped and the
@@ -1763,16 +1788,20 @@ bool tower_fits_tc2(const voila_model_desc *d) {
     if (g.n_layers < 2 || g.n_layers > 6) return false;
     if (g.dims[0] != d->state_dim + (d->lik_action_cond ? d->n_actions : 0)) return false;
     for (int l = 1; l < g.n_layers; ++l)
-        if (g.dims[l] % 64 != 0 || g.dims[l] > 512) return false;
+        if (g.dims[l] > 512) return false;
     return g.dims[g.n_layers] >= 1 && g.dims[g.n_layers] <= 128;
 }
 }  // namespace
 
 void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *allocs, std::string *err) {
     const int S = d->state_dim, A = d->n_actions, Nz = d->noise_dim;
+    const int Sp = rup(S, 8), Nzp = rup(Nz, 8);  // operand widths of the state and the noise
+    const bool aligned = Sp == S && Nzp == Nz;   // the per-row-action / denoiser programs want aligned widths
     int policy = 0;
     if (const char *e = getenv("VOILA_T2_BLOCK_POLICY")) policy = atoi(e);  // tuning knob (0, 1, 2)
     T2Handle *h = new T2Handle();
+    h->Sp = Sp;
+    h->Nzp = Nzp;
     {
         Builder2 pb;
         pb.policy = policy;
@@ -1789,9 +1818,9 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
         // 16 epilogue warps (two sets sharing every hidden layer) unless the 8-warp kernel is asked for
         const std::string m =
-            h->roll_x ? finish_program(pb, h->roll, rollout_tc2x_kernel, rup(S + Nz, 64) / 64, sm_count, allocs,
+            h->roll_x ? finish_program(pb, h->roll, rollout_tc2x_kernel, rup(Sp + Nzp, 64) / 64, sm_count, allocs,
                                        kT2ThreadsDual)
-                      : finish_program(pb, h->roll, rollout_tc2_kernel, rup(S + Nz, 64) / 64, sm_count, allocs);
+                      : finish_program(pb, h->roll, rollout_tc2_kernel, rup(Sp + Nzp, 64) / 64, sm_count, allocs);
         if (!m.empty()) {
             if (err) *err = m;
             delete h;
@@ -1804,15 +1833,15 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         // units in flight per CTA pair (4 operand chunks and 256 TMEM columns each), so that the
         // epilogue of one unit overlaps the MMAs of the other; used when there is more than one
         // unit per CTA pair (large N), while small N keeps the one-slot program (lower latency).
-        int widest = S + Nz;
-        for (int l = 1; l <= d->f_T.n_layers; ++l) widest = std::max(widest, d->f_T.dims[l]);
-        for (int l = 0; l <= d->lik_state.n_layers; ++l) widest = std::max(widest, l == 0 ? S : d->lik_state.dims[l]);
+        int widest = Sp + Nzp;
+        for (int l = 1; l <= d->f_T.n_layers; ++l) widest = std::max(widest, rup(d->f_T.dims[l], 64));
+        for (int l = 0; l <= d->lik_state.n_layers; ++l) widest = std::max(widest, l == 0 ? Sp : rup(d->lik_state.dims[l], 64));
         const bool want_dual = widest <= 256 && !getenv("VOILA_T2_BELIEF_1SLOT");
         // pw = 1: the progressive-widening form (one-hot block in the operand; its layer-1 K is
         // S + Nz + A); only without an action-conditioned state tower
         for (int pw = 0; pw <= (d->lik_action_cond ? 0 : 1); ++pw) {
-            const int in_cols = S + Nz + (pw ? rup(A, 8) : 0);
-            if (pw && (A % 8 != 0 || in_cols > 512)) continue;
+            const int in_cols = Sp + Nzp + (pw ? rup(A, 8) : 0);
+            if (pw && (!aligned || A % 8 != 0 || in_cols > 512)) continue;
             const bool dual_ok = want_dual && rup(in_cols, 64) / 64 <= 4;
             for (int dual = 0; dual <= (dual_ok ? 1 : 0); ++dual) {
                 Builder2 pb;
@@ -1833,7 +1862,7 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
                 }
                 T2Program &prog = pw ? (dual ? h->pw_dual : h->pw) : (dual ? h->belief_dual : h->belief);
                 const int dd = g.dims[g.n_layers];
-                prog.hdr.g_in_chunks = rup(S, 64) / 64;
+                prog.hdr.g_in_chunks = rup(Sp, 64) / 64;
                 prog.hdr.e_pad = rup(dd, 16);
                 prog.hdr.e_off = (int)pb.sbias_init.size();
                 pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
@@ -1851,7 +1880,7 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     for (int which = 0; which < 2; ++which) {
         const voila_mlp &f = which == 0 ? d->denoise_T : d->denoise_Z;
         const int D = which == 0 ? S : d->obs_dim;
-        if (f.n_layers < 2 || f.n_layers > 8 || D % 8 != 0 || D > 64) continue;
+        if (f.n_layers < 2 || f.n_layers > 8 || D % 8 != 0 || D > 64 || !aligned) continue;
         bool fits = S + D + rup(A, 8) <= 512;
         int widest = S + D + rup(A, 8);
         for (int l = 1; l < f.n_layers; ++l) {
@@ -1917,7 +1946,8 @@ T2Params base_params(const T2Program &g, const ModelDev &m) {
     p.layers = reinterpret_cast<const T2Layer *>(g.d_layers);
     p.tiles = reinterpret_cast<const T2TileDev *>(g.d_tiles);
     p.hdr = g.hdr;
-    p.S = m.S; p.O = m.O; p.A = m.A; p.Nz = m.Nz;
+    p.S = rup(m.S, 8); p.O = m.O; p.A = m.A; p.Nz = rup(m.Nz, 8);
+    p.S_io = m.S;
     p.gamma = m.gamma;
     p.reward_kind = m.reward.kind;
     p.reward_param = m.reward.param;

@@ -108,21 +108,51 @@ __device__ __forceinline__ void gen_noise_call(uint32_t (&nz)[16], uint64_t seed
     }
 }
 
+// One 8-column unit (16 bytes) of a public bf16 row of S_io columns: rows whose length is a multiple
+// of 8 are 16-byte aligned and move as one vector; other lengths (paper-shaped states, S = 39 / 45) go
+// element by element with the tail zero-filled / masked.
+__device__ __forceinline__ uint4 load_row_unit(const uint16_t *__restrict__ row, int S_io, int u) {
+    if ((S_io & 7) == 0) return __ldg(reinterpret_cast<const uint4 *>(row) + u);
+    uint32_t w[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int c = 8 * u + 2 * e;
+        const uint32_t lo = c < S_io ? (uint32_t)__ldg(row + c) : 0u;
+        const uint32_t hi = c + 1 < S_io ? (uint32_t)__ldg(row + c + 1) : 0u;
+        w[e] = lo | (hi << 16);
+    }
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
+__device__ __forceinline__ void store_row_unit(uint16_t *row, int S_io, int u, uint4 v) {
+    if ((S_io & 7) == 0) {
+        *(reinterpret_cast<uint4 *>(row) + u) = v;
+        return;
+    }
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int c = 8 * u + 2 * e;
+        if (c < S_io) row[c] = (uint16_t)(w[e] & 0xffffu);
+        if (c + 1 < S_io) row[c + 1] = (uint16_t)(w[e] >> 16);
+    }
+}
+
 // R(s, a) from the bf16 state for the non-quadratic reward kinds (R14).
 __device__ __forceinline__ float reward_from_state(const uint32_t *st, int S, int kind,
                                                    const float *__restrict__ param) {
     float acc = 0.0f;
 #pragma unroll
     for (int c2 = 0; c2 < 32; ++c2) {
-        if (2 * c2 < S) {
+        if (2 * c2 < S) {  // S: the PUBLIC state width (an odd S leaves the last pair half used)
+            const bool two = 2 * c2 + 1 < S;
             const float s0 = bf16lo(st[c2]), s1 = bf16hi(st[c2]);
-            const float p0 = __ldg(param + 2 * c2), p1 = __ldg(param + 2 * c2 + 1);
+            const float p0 = __ldg(param + 2 * c2), p1 = two ? __ldg(param + 2 * c2 + 1) : 0.0f;
             if (kind == VOILA_R_NEG_L2_GOAL) {
                 acc = fmaf(s0 - p0, s0 - p0, acc);
-                acc = fmaf(s1 - p1, s1 - p1, acc);
+                if (two) acc = fmaf(s1 - p1, s1 - p1, acc);
             } else {
                 acc = fmaf(p0, s0, acc);
-                acc = fmaf(p1, s1, acc);
+                if (two) acc = fmaf(p1, s1, acc);
             }
         }
     }

@@ -334,11 +334,11 @@ voila_status voila_create(const voila_model_desc *desc, int device, voila_ctx **
     }
     if (bf16) {
         std::string why;
-        if (tc_supported(desc, &why) && term_fits_tc) {
+        if (tc2_supported(desc, &why) && term_fits_tc) {
             // A program that does not fit (tables, shared memory, tensor map) leaves its handle null and
             // AUTO runs the CUDA-core kernels, as voila.h promises; the reason stays readable.
             std::string err;
-            if (m.term.n == 0) {  // the single-CTA variant has no terminal-region epilogue
+            if (m.term.n == 0 && tc_supported(desc, &why)) {  // the single-CTA variant: aligned dims, no terminal regions
                 ctx->tc = tc_create(desc, ctx->sm_count, &ctx->dev_allocs, &err);
                 if (!ctx->tc) ctx->last_cuda_error = "single-CTA tcgen05 program not built: " + err;
             }
