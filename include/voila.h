@@ -41,8 +41,7 @@
  *     what the tests and bench.py run): VOILA_T2_BLOCK_POLICY (0..4: accumulator block shapes of the
  *     tcgen05 pair kernels), VOILA_T2_ROLLOUT_WARPS (8 | 16 epilogue warps of the rollout kernel),
  *     VOILA_T2_STAGES (2..8 weight-ring stages), VOILA_T2_BELIEF_1SLOT (disable the two-slot programs),
- *     VOILA_T2_ISSUERS (1 | 2 MMA issuer warps), VOILA_T2_DUAL_SPLIT (both epilogue sets share every hidden
- *     layer of a two-slot program).
+ *     VOILA_T2_DUAL_SPLIT (both epilogue sets share every hidden layer of a two-slot program).
  */
 #ifndef VOILA_H_
 #define VOILA_H_

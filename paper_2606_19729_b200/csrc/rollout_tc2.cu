@@ -367,6 +367,9 @@ __device__ __forceinline__ void t2_helper_epilogue(const T2Params &p, const T2La
 // Epilogue role (warps 4-11 of BOTH CTAs): each warp owns 32 rows (TMEM lane quadrant warp % 4) and,
 // in hidden layers, one 32-column half of every 64-column chunk.  Events are published on the
 // LEADER's mbarriers (remote arrive from the peer CTA).
+// MODE: 1 = the model has terminal regions (voila_terminal); 0 compiles the alive-flag logic out (it cost
+// the plain rollout 2.4 % when it was a runtime test).
+template <int MODE>
 __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                             uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
                                             uint8_t *alive_s, float *sbias, int warp, int lane, uint32_t rank,
@@ -447,7 +450,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         // one ends the episode here (r_step is not paid, the state freezes, nothing accrues later).
         // The row's alive flag of step t goes to shared memory for the warp that holds its witness.
         auto pay = [&](float r_step) {
-            if (p.term.n == 0) {
+            if (MODE == 0) {
                 G = fmaf(disc, r_step, G);
                 return;
             }
@@ -584,8 +587,8 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                     const uint32_t n1 = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z,
                                                                     __uint_as_float(v[4 * i + 3]) + b[i].w);
                                     // a row whose episode has ended keeps its state
-                                    persist[8 * g + 2 * i] = alive ? n0 : persist[8 * g + 2 * i];
-                                    persist[8 * g + 2 * i + 1] = alive ? n1 : persist[8 * g + 2 * i + 1];
+                                    persist[8 * g + 2 * i] = (MODE == 0 || alive) ? n0 : persist[8 * g + 2 * i];
+                                    persist[8 * g + 2 * i + 1] = (MODE == 0 || alive) ? n1 : persist[8 * g + 2 * i + 1];
                                 }
                             }
                         }
@@ -603,7 +606,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 1) {
                         // no observation for a row whose episode ended at or before step t
-                        const float disc_w = (p.term.n == 0 || alive_s[(t & 1) * kT2Rows + row] != 0) ? disc : 0.0f;
+                        const float disc_w = (MODE == 0 || alive_s[(t & 1) * kT2Rows + row] != 0) ? disc : 0.0f;
 #pragma unroll
                         for (int g = 0; g < 4; ++g) {
                             if (16 * g < (int)l.n_pad) {
@@ -711,6 +714,10 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
 // buffer -> HBM: no per-row register state, so a TWO-SLOT program (hdr.n_slots == 2: narrow models)
 // keeps two units in flight, each layer record naming its slot; the epilogue of one unit then
 // overlaps the MMAs of the other.
+// MODE: 0 the belief update, 1 progressive widening (per-row action / embedding / child maximum),
+// 2 diffusion teacher (one denoiser call + DDIM step).  Compile-time: as runtime tests these branches
+// cost the plain belief update 8 % (CFG4 propose+score 611 -> 660 us).
+template <int MODE>
 __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer *L, uint32_t a_u32, uint32_t tmem_base,
                                                uint64_t *evt, uint64_t *layer_done, float *sbias, int warp, int lane,
                                                uint32_t rank, int cluster_id, int n_clusters, int n_my_units,
@@ -768,7 +775,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
         }
         const int u0 = S >> 3;
         int u_next = u0;
-        if (p.diff_x) {
+        if (MODE == 2) {
             // diffusion teacher: the current x (bf16 operand copy of the fp32 state; omega at the first step)
             for (int u = 0; u < (p.diff_D >> 3); ++u) {
                 uint4 v = make_uint4(0u, 0u, 0u, 0u);
@@ -793,7 +800,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             }
             u_next = u0 + (Nz >> 3);
         }
-        if (p.pw_sim_action) {
+        if (MODE >= 1) {
             // per-row action: the one-hot block is part of the operand, columns [S + Nz, S + Nz + A)
             const int a_row = valid ? __ldg(p.pw_sim_action + i_idx) : -1;
             const int n_u = (p.A + 7) >> 3;
@@ -856,7 +863,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 ecs.st_base += (uint32_t)l.chunk_off * kT2ChunkBytes;
                 ecs.taddr0 += (uint32_t)l.col_off;
                 epi_hidden_layer(es, l, (int)l.sbias_off, ecs);
-            } else if (l.epi == T2_EPI_PROPOSAL) {
+            } else if (MODE < 2 && l.epi == T2_EPI_PROPOSAL) {
                 const int i_idx = row_index(step, slot);
                 const bool valid = i_idx < p.P;
                 es.wait_layer();
@@ -900,7 +907,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 tc_fence_before();
                 es.arrive_event();
                 T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
-            } else if (l.epi == T2_EPI_DIFFUSE) {  // diffusion teacher: last (only) network of the unit
+            } else if (MODE == 2) {  // T2_EPI_DIFFUSE: diffusion teacher, last (only) network of the unit
                 const int i_idx = row_index(step, slot);
                 const bool valid = i_idx < p.P;
                 const int D = p.diff_D;
@@ -961,7 +968,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 // progressive widening: the row's own embedding (rows of e_pad floats, zero-padded)
                 const float *e_row = nullptr;
                 int seg = 0;
-                if (p.pw_sim_seg && half == 0) {
+                if (MODE == 1 && half == 0) {
                     seg = valid ? __ldg(p.pw_sim_seg + i_idx) : 0;
                     e_row = p.pw_E + (size_t)seg * (size_t)p.hdr.e_pad;
                 }
@@ -978,8 +985,8 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 #pragma unroll
                             for (int i = 0; i < 4; ++i) {
                                 b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
-                                e4[i] = e_row ? __ldg(reinterpret_cast<const float4 *>(e_row + 16 * g) + i)
-                                              : *(reinterpret_cast<const float4 *>(e_s + 16 * g) + i);
+                                e4[i] = MODE == 1 ? __ldg(reinterpret_cast<const float4 *>(e_row + 16 * g) + i)
+                                                  : *(reinterpret_cast<const float4 *>(e_s + 16 * g) + i);
                             }
                             tmem_ld_wait();
 #pragma unroll
@@ -994,7 +1001,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                     const float Lg = lw + ell * p.inv_lambda;
                     int ord = float_to_ordered(valid ? Lg : -INFINITY);
                     if (valid) p.bu_logits[i_idx] = Lg;
-                    if (p.pw_seg_max) {  // the maximum of the row's own child belief; no evidence sums
+                    if (MODE == 1) {  // the maximum of the row's own child belief; no evidence sums
                         if (valid) atomicMax(p.pw_seg_max + seg, ord);
                         ord = (int)0x80000000;
                     }
@@ -1004,7 +1011,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
                     const int i0 = i_idx - lane;  // first particle of this warp's 32 rows
-                    if (lane == 0 && i0 < p.P && !p.pw_seg_max) {
+                    if (MODE == 0 && lane == 0 && i0 < p.P) {
                         atomicMax(p.bu_max_ordered, ord);
                         p.bu_part_wsum[i0 >> 5] = ws;
                     }
@@ -1026,7 +1033,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
 // warpgroups after `setmaxnreg` (their total must fit the launch allocation).
 // R_HELP: registers of the second set of epilogue warps (warps 12-19 of a 640-thread kernel);
 // > 0: raised to R_HELP, < 0: lowered to -R_HELP.
-template <bool BELIEF, int NTHREADS, int R_LOW, int R_HIGH, int R_HELP = 0>
+template <bool BELIEF, int NTHREADS, int R_LOW, int R_HIGH, int R_HELP, int MODE>
 __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &wmap) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw_u32 = smem_u32(smem_raw);
@@ -1122,19 +1129,13 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
 #endif
             (void)tr_empty; (void)tr_start;
         }
-    } else if (warp == 1 || (warp == 3 && p.hdr.n_issuers == 2)) {
-        // ===== MMA issuer(s): leader CTA only.  The whole warp walks the tile program (waits are
-        // warp-uniform); one elected lane issues the MMAs and commits.  With two issuers (warps 1 and
-        // 3, on different schedulers) every tile belongs to one of them: the slots of a two-slot
-        // program, else the accumulator blocks by parity.  Each walks the whole program, keeps the ring
-        // position and the chunk-free sequence for the tiles it skips, and issues its own in program
-        // order: a tile only ever depends on earlier program items, so the earliest unfinished item is
-        // always at the head of its owner's queue (no deadlock), and one slot no longer waits behind
-        // the other's tiles.  The issuer loop is ~150 instructions per 512-cycle tile on a scheduler it
-        // shares with four epilogue warps (ncu: the tensor queue is never full); two warps halve that. =====
+    } else if (warp == 1) {
+        // ===== MMA issuer: leader CTA only.  The whole warp walks the tile program (waits are
+        // warp-uniform); one elected lane issues the MMAs and commits.  (A second issuer warp taking the
+        // tiles of the other slot / of the odd accumulator blocks was built and measured: no gain, and
+        // its per-tile ownership test alone cost the one-issuer kernel 3 % -- every instruction of this
+        // loop is on the critical path.) =====
         if (rank == 0) {
-            const bool two = p.hdr.n_issuers == 2;
-            const uint32_t owner = warp == 3 ? 1u : 0u;
             uint32_t stage = 0, phase = 0;
             uint32_t tl_n = 0;
             (void)tl_n;
@@ -1146,20 +1147,19 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             uint64_t *cfree = layer_done + kT2AccRing;
             long long tr_evt = 0, tr_full = 0, tr_mma = 0, tr_commit = 0;
             const long long tr_start = clock64();
+            // the next tile's record is fetched while the current tile waits / issues (its shared-memory
+            // latency is otherwise at the head of every tile's dependent chain)
+            uint4 r0n = *reinterpret_cast<const uint4 *>(T), r1n = *(reinterpret_cast<const uint4 *>(T) + 1);
             for (int step = 0; step < total_steps; ++step) {
                 for (int i = 0; i < n_tiles; ++i) {
-                    if (two && ((T[i].misc >> 7) & 1u) != owner) {  // the other issuer's tile: books only
-                        free_seq += (T[i].misc >> 6) & 1u;
-                        if (++stage == (uint32_t)n_stages) {
-                            stage = 0;
-                            phase ^= 1u;
-                        }
-                        continue;
+                    const uint4 r0 = r0n, r1 = r1n;
+                    {
+                        const int ni = i + 1 < n_tiles ? i + 1 : 0;
+                        r0n = *reinterpret_cast<const uint4 *>(T + ni);
+                        r1n = *(reinterpret_cast<const uint4 *>(T + ni) + 1);
                     }
-                    const uint4 r0 = *reinterpret_cast<const uint4 *>(T + i);
-                    const uint4 r1 = *(reinterpret_cast<const uint4 *>(T + i) + 1);
 #ifdef VOILA_T2_TRACE
-                    const bool tl_on = cluster_id == 0 && warp == 1 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+                    const bool tl_on = cluster_id == 0 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
 #endif
                     // events needed from epilogue set 0 and set 1 (-100000: nothing to wait for)
                     const int n0 = base + (int)r1.x, n1 = base + (int)r1.y;
@@ -1234,7 +1234,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                 blk_base += p.hdr.blocks_per_step;
             }
 #ifdef VOILA_T2_TRACE
-            if (cluster_id == 0 && warp == 1 && elect_one_sync()) {
+            if (cluster_id == 0 && elect_one_sync()) {
                 g_t2_trace[4] = tr_evt;
                 g_t2_trace[5] = tr_full;
                 g_t2_trace[6] = clock64() - tr_start;
@@ -1248,17 +1248,17 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     } else if (NTHREADS == kT2Threads || warp < 12) {
         setmaxnreg_inc<R_HIGH>();
         if (BELIEF)
-            t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
+            t2_bu_epilogue<BELIEF ? MODE : 0>(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
                            n_my_units, NTHREADS == kT2Threads ? -1 : 0);
         else
-            t2_epilogue(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, alive_s, sbias, warp, lane, rank,
+            t2_epilogue<BELIEF ? 0 : MODE>(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, alive_s, sbias, warp, lane, rank,
                         cluster_id, n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads);
     } else {
         // second set of epilogue warps (640-thread kernels)
         if (R_HELP > 0) setmaxnreg_inc<(R_HELP > 0 ? R_HELP : 24)>();
         else setmaxnreg_dec<(R_HELP < 0 ? -R_HELP : 24)>();
         if (BELIEF)
-            t2_bu_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
+            t2_bu_epilogue<BELIEF ? MODE : 0>(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
                            n_my_units, 1);
         else
             t2_helper_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, total_steps);
@@ -1270,26 +1270,31 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     if (warp == 2) tmem_dealloc_2cta(tmem_base, (uint32_t)p.hdr.tmem_cols);
 }
 
+// MODE: rollout kernels 0 | 1 (terminal regions); belief-style kernels 0 | 1 | 2 (see t2_bu_epilogue).
+template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     rollout_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<false, kT2Threads, 56, 224>(p, wmap);
+    tc2_body<false, kT2Threads, 56, 224, 0, MODE>(p, wmap);
 }
+template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2Threads, 1)
     belief_tc2_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<true, kT2Threads, 56, 224>(p, wmap);
+    tc2_body<true, kT2Threads, 56, 224, 0, MODE>(p, wmap);
 }
 // Two-slot belief program with one set of eight epilogue warps PER SLOT (20 warps): the two units'
 // epilogues run concurrently, four epilogue warps per scheduler hide each other's latencies.
 constexpr int kT2ThreadsDual = 640;
+template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
     belief_tc2_dual_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<true, kT2ThreadsDual, 40, 104, 104>(p, wmap);
+    tc2_body<true, kT2ThreadsDual, 40, 104, 104, MODE>(p, wmap);
 }
 // Rollout with a second set of epilogue warps that takes the odd chunks of every hidden layer: the
 // layer's epilogue (TMEM read, activation, pack, store) runs on 16 warps, four per scheduler.
+template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
     rollout_tc2x_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
-    tc2_body<false, kT2ThreadsDual, 32, 168, -56>(p, wmap);
+    tc2_body<false, kT2ThreadsDual, 32, 168, -56, MODE>(p, wmap);
 }
 
 }  // namespace
@@ -1691,8 +1696,6 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
     while (cols < max_n) cols *= 2;
     g.hdr.tmem_cols = cols;
     g.hdr.split_hidden = (pb.dual && pb.par_split) ? 1 : 0;
-    g.hdr.n_issuers = 1;  // a second issuer warp (warp 3) measured no gain: the epilogue chain sets the pace
-    if (const char *e = getenv("VOILA_T2_ISSUERS")) g.hdr.n_issuers = atoi(e) == 2 ? 2 : 1;  // A/B knob
     g.hdr.n_stages = 8;
     if (const char *e = getenv("VOILA_T2_STAGES")) g.hdr.n_stages = std::max(2, std::min(8, atoi(e)));
     while (g.hdr.n_stages > 2 && smem2_map(g.hdr).total + 1024 > kMaxDynSmem2) --g.hdr.n_stages;
@@ -1711,8 +1714,7 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         d.need_s0 = s0;
         d.need_s1 = need2 != need ? s1 : -100000;
         d.chunk_b16 = ((uint32_t)t.rows8 * 1024u) >> 4;
-        const uint32_t owner = pb.dual ? (uint32_t)t.pad : ((uint32_t)t.blk & 1u);
-        d.misc = (uint32_t)t.nk | ((uint32_t)(t.flags & 7u) << 4) | (owner << 7) | ((uint32_t)t.blk << 8) |
+        d.misc = (uint32_t)t.nk | ((uint32_t)(t.flags & 7u) << 4) | ((uint32_t)t.blk << 8) |
                  ((uint32_t)((int)t.nk * (int)t.rows8 * 8) << 16);
         dev_tiles.push_back(d);
     }
@@ -1797,6 +1799,7 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
     const int S = d->state_dim, A = d->n_actions, Nz = d->noise_dim;
     const int Sp = rup(S, 8), Nzp = rup(Nz, 8);  // operand widths of the state and the noise
     const bool aligned = Sp == S && Nzp == Nz;   // the per-row-action / denoiser programs want aligned widths
+    const bool term = d->terminal && d->terminal->n_regions > 0;  // the rollout kernel instance with the alive-flag logic
     int policy = 0;
     if (const char *e = getenv("VOILA_T2_BLOCK_POLICY")) policy = atoi(e);  // tuning knob (0, 1, 2)
     T2Handle *h = new T2Handle();
@@ -1818,9 +1821,10 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
         add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
         // 16 epilogue warps (two sets sharing every hidden layer) unless the 8-warp kernel is asked for
         const std::string m =
-            h->roll_x ? finish_program(pb, h->roll, rollout_tc2x_kernel, rup(Sp + Nzp, 64) / 64, sm_count, allocs,
-                                       kT2ThreadsDual)
-                      : finish_program(pb, h->roll, rollout_tc2_kernel, rup(Sp + Nzp, 64) / 64, sm_count, allocs);
+            h->roll_x ? (term ? finish_program(pb, h->roll, rollout_tc2x_kernel<1>, rup(Sp + Nzp, 64) / 64, sm_count, allocs, kT2ThreadsDual)
+                              : finish_program(pb, h->roll, rollout_tc2x_kernel<0>, rup(Sp + Nzp, 64) / 64, sm_count, allocs, kT2ThreadsDual))
+                      : (term ? finish_program(pb, h->roll, rollout_tc2_kernel<1>, rup(Sp + Nzp, 64) / 64, sm_count, allocs)
+                              : finish_program(pb, h->roll, rollout_tc2_kernel<0>, rup(Sp + Nzp, 64) / 64, sm_count, allocs));
         if (!m.empty()) {
             if (err) *err = m;
             delete h;
@@ -1867,9 +1871,10 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
                 prog.hdr.e_off = (int)pb.sbias_init.size();
                 pb.sbias_init.resize(pb.sbias_init.size() + (size_t)prog.hdr.e_pad, 0.0f);
                 const std::string m =
-                    dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(in_cols, 64) / 64, sm_count, allocs,
-                                          kT2ThreadsDual)
-                         : finish_program(pb, prog, belief_tc2_kernel, rup(in_cols, 64) / 64, sm_count, allocs);
+                    dual ? (pw ? finish_program(pb, prog, belief_tc2_dual_kernel<1>, rup(in_cols, 64) / 64, sm_count, allocs, kT2ThreadsDual)
+                               : finish_program(pb, prog, belief_tc2_dual_kernel<0>, rup(in_cols, 64) / 64, sm_count, allocs, kT2ThreadsDual))
+                         : (pw ? finish_program(pb, prog, belief_tc2_kernel<1>, rup(in_cols, 64) / 64, sm_count, allocs)
+                               : finish_program(pb, prog, belief_tc2_kernel<0>, rup(in_cols, 64) / 64, sm_count, allocs));
                 // without a one-slot program the CUDA-core kernels serve the call
                 bool &flag = pw ? (dual ? h->has_pw_dual : h->has_pw) : (dual ? h->has_belief_dual : h->has_belief);
                 flag = m.empty();
@@ -1902,8 +1907,8 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             prog.hdr.e_pad = 0;
             prog.hdr.e_off = (int)pb.sbias_init.size();
             const std::string m =
-                dual ? finish_program(pb, prog, belief_tc2_dual_kernel, rup(in_cols, 64) / 64, sm_count, allocs, kT2ThreadsDual)
-                     : finish_program(pb, prog, belief_tc2_kernel, rup(in_cols, 64) / 64, sm_count, allocs);
+                dual ? finish_program(pb, prog, belief_tc2_dual_kernel<2>, rup(in_cols, 64) / 64, sm_count, allocs, kT2ThreadsDual)
+                     : finish_program(pb, prog, belief_tc2_kernel<2>, rup(in_cols, 64) / 64, sm_count, allocs);
             h->has_diff[which][dual] = m.empty();
         }
         if (h->has_diff[which][0]) {
@@ -1975,8 +1980,14 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     p.tiles_per_q = a.tiles;  // = 2 * blocks_per_q (see rollout_tile_count)
     p.n_units = p.blocks_per_q * a.Q;
     const int clusters = std::min(g.max_clusters, p.n_units);
-    if (h->roll_x) rollout_tc2x_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
-    else rollout_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    const bool term = m.term.n > 0;
+    if (h->roll_x) {
+        if (term) rollout_tc2x_kernel<1><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+        else rollout_tc2x_kernel<0><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    } else {
+        if (term) rollout_tc2_kernel<1><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+        else rollout_tc2_kernel<0><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    }
     if (kernel_name)
         *kernel_name = h->roll_x ? "rollout_tc2x_kernel<tcgen05 cta_group::2 bf16, 16 epilogue warps>"
                                  : "rollout_tc2_kernel<tcgen05 cta_group::2 bf16>";
@@ -2008,8 +2019,8 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
     p.inv_lambda = 1.0f / m.lambda;
     p.d = m.mlp[3].dims[m.mlp[3].n_layers];
     const int clusters = std::min(g.max_clusters, p.n_units);
-    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
-    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (dual) belief_tc2_dual_kernel<0><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<0><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (kernel_name)
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
@@ -2044,8 +2055,8 @@ cudaError_t launch_pw_propose_score_tc2(void *tc, const ModelDev &m, const PwArg
     p.pw_E = a.E;
     p.pw_seg_max = a.seg_max;
     const int clusters = std::min(g.max_clusters, p.n_units);
-    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
-    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (dual) belief_tc2_dual_kernel<1><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<1><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (kernel_name)
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, per-row actions>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, per-row actions>";
@@ -2084,8 +2095,8 @@ cudaError_t launch_diffusion_step_tc2(void *tc, const ModelDev &m, const Diffusi
     p.diff_first = a.first;
     p.al = a.al; p.si = a.si; p.al_n = a.al_n; p.si_n = a.si_n;
     const int clusters = std::min(g.max_clusters, p.n_units);
-    if (dual) belief_tc2_dual_kernel<<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
-    else belief_tc2_kernel<<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    if (dual) belief_tc2_dual_kernel<2><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+    else belief_tc2_kernel<2><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
     if (kernel_name)
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, denoiser + DDIM step>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, denoiser + DDIM step>";

@@ -103,9 +103,7 @@ struct T2TileDev {
     int32_t need_s0;    // event of epilogue set 0 to wait for (relative to the step), -100000: none
     int32_t need_s1;    // event of epilogue set 1 to wait for, -100000: none
     uint32_t chunk_b16; // weight bytes of one K chunk in the stage / 16 (descriptor units)
-    uint32_t misc;      // nk | flags << 4 | owner << 7 | blk << 8 | rows << 16   (rows = weight rows per CTA in
-                        // the stage; owner = the issuer warp the tile belongs to: its slot in a two-slot
-                        // program, else the parity of its accumulator block)
+    uint32_t misc;      // nk | flags << 4 | blk << 8 | rows << 16   (rows = weight rows per CTA in the stage)
 };
 static_assert(sizeof(T2TileDev) == 32, "T2TileDev is read with two 16-byte loads");
 
@@ -122,7 +120,6 @@ struct T2Header {
     int split_hidden;     // two-slot programs: 1 = both sets of epilogue warps share EVERY hidden layer of both
                           // slots (even / odd chunks), a slot's other layers go to the set of its number;
                           // 0 = one set per slot
-    int n_issuers;        // 1 | 2 MMA issuer warps (warp 1, warp 3): a tile belongs to issuer (misc >> 7) & 1
 };
 
 }  // namespace voila
