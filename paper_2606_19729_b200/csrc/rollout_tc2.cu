@@ -355,7 +355,9 @@ __device__ __forceinline__ void t2_helper_epilogue(const T2Params &p, const T2La
             const T2Layer l = L[li];
             es.tl_layer = (uint32_t)li;
             if (l.epi == T2_EPI_HIDDEN) {
-                epi_hidden_layer_par(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ec, 1);
+                EpiConst ecs = ec;
+                ecs.taddr0 += (uint32_t)l.col_off;  // accumulators ping-pong between the TMEM halves (narrow models)
+                epi_hidden_layer_par(es, l, (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0), ecs, 1);
             } else {
                 ++es.ev;
                 ++es.ld_seq;
@@ -534,8 +536,10 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
                     const int boff = (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
-                    if (shared_hidden) epi_hidden_layer_par(es, l, boff, ec, 0);
-                    else epi_hidden_layer(es, l, boff, ec);
+                    EpiConst ecs = ec;
+                    ecs.taddr0 += (uint32_t)l.col_off;  // accumulators ping-pong between the TMEM halves (narrow models)
+                    if (shared_hidden) epi_hidden_layer_par(es, l, boff, ecs, 0);
+                    else epi_hidden_layer(es, l, boff, ecs);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
                     T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
@@ -545,7 +549,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         for (int g = 0; g < 4; ++g) {
                             if (16 * g < (int)l.n_pad) {
                                 uint32_t v[16];
-                                tmem_ld16(lane_taddr + 16 * g, v);
+                                tmem_ld16(lane_taddr + (uint32_t)l.col_off + 16 * g, v);
                                 tmem_ld_wait();
 #pragma unroll
                                 for (int c = 0; c < 16; c += 2) {
@@ -575,7 +579,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         for (int g = 0; g < 4; ++g) {
                             if (16 * g < (int)l.n_pad) {
                                 uint32_t v[16];
-                                tmem_ld16(lane_taddr + 16 * g, v);
+                                tmem_ld16(lane_taddr + (uint32_t)l.col_off + 16 * g, v);
                                 float4 b[4];
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
@@ -611,7 +615,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                         for (int g = 0; g < 4; ++g) {
                             if (16 * g < (int)l.n_pad) {
                                 uint32_t v[16];
-                                tmem_ld16(lane_taddr + 16 * g, v);
+                                tmem_ld16(lane_taddr + (uint32_t)l.col_off + 16 * g, v);
                                 float4 b[4];
 #pragma unroll
                                 for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
@@ -1370,6 +1374,7 @@ struct Builder2 {
 
     // Two-slot mode: every layer is added once per slot (slot 1 shares slot 0's biases and weight
     // tiles; its operand chunks / TMEM columns are disjoint, so its dependencies are tracked apart).
+    bool pingpong = false;         // see add_layer
     bool par_split = false;        // two sets of epilogue warps share every hidden layer (even / odd chunks)
     std::vector<uint8_t> evt_set;  // set that publishes event e of the step
     bool dual = false;
@@ -1387,6 +1392,10 @@ struct Builder2 {
     // W: [n0][k0] row-major fp32 ("algorithmic" column order); bias_rows x n0 biases.
     void add_layer(const float *W, int n0, int k0, const float *b, int bias_rows, int epi, int act) {
         if (!dual) {
+            // narrow single-slot programs: consecutive layers accumulate in alternate halves of TMEM, so a
+            // layer's tiles wait only for the operand chunks they read (not for the previous layer's
+            // accumulator to be drained) and start chunk by chunk while that epilogue is still running
+            if (pingpong) col_off = (int)(layers.size() & 1) * 256;
             add_one(W, n0, k0, b, bias_rows, epi, act, -1);
             return;
         }
@@ -1815,6 +1824,12 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             h->roll_x = e ? atoi(e) == 16 : true;
         }
         pb.par_split = h->roll_x;
+        {
+            int w = 0;
+            for (const voila_mlp *f : {&d->f_T, &d->f_Z})
+                for (int l = 1; l <= f->n_layers; ++l) w = std::max(w, rup(f->dims[l], 64));
+            pb.pingpong = w <= 256 && !getenv("VOILA_T2_NO_PINGPONG");
+        }
         if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
             pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
         add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
