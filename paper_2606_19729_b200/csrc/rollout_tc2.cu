@@ -106,6 +106,15 @@ struct T2Params {
     float *diff_x;                 // [N][D] fp32 state, updated in place, or nullptr
     int diff_D, diff_first;        // first: x = omega (Philox stream 7) instead of the stored state
     float al, si, al_n, si_n;      // alpha, sigma at tau_k and tau_{k+1}
+    // progressive widening, the small passes over the (action node, branch) slots (row = slot g * M_max + m):
+    // MODE 3: slots opened in this call: s' = f_T(s_src, a_g, w_T(src)), o = f_Z(s', a_g, w_Z(src)) -> branch_obs
+    // MODE 4: every stored branch (m < branch_count[g]): e = f(obs) -> embedding table
+    const int32_t *slot_src;       // [slots] simulation that opened the slot, or -1
+    const int32_t *slot_action;    // [G] action of the node
+    const int32_t *slot_count;     // [G] branches stored per node (MODE 4)
+    float *slot_obs;               // [slots][O] fp32
+    float *slot_emb;               // [slots][d] fp32
+    int slot_M;                    // M_max
 };
 
 struct Smem2 {
@@ -768,6 +777,43 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
     auto load_input = [&](int unit_local, int slot, uint32_t a_slot) {
         if (half != 0) return;
         const int i_idx = row_index(unit_local, slot);
+        if (MODE == 4) {  // [bf16(obs)] of a stored branch
+            const bool ok = i_idx < p.P && (i_idx % p.slot_M) < __ldg(p.slot_count + i_idx / p.slot_M);
+            for (int u = 0; u < in_units; ++u) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (ok && 8 * u < p.O) {
+                    const float4 *xp = reinterpret_cast<const float4 *>(p.slot_obs + (size_t)i_idx * p.O) + 2 * u;
+                    const float4 x0 = __ldg(xp), x1 = __ldg(xp + 1);
+                    v = make_uint4(pack_bf16x2(x0.x, x0.y), pack_bf16x2(x0.z, x0.w), pack_bf16x2(x1.x, x1.y),
+                                   pack_bf16x2(x1.z, x1.w));
+                }
+                st_shared_v4(a_unit_addr(a_slot, row, u), v.x, v.y, v.z, v.w);
+            }
+            return;
+        }
+        if (MODE == 3) {  // [s_src ; w_T(src) ; onehot(a_g)] of the simulation that opened the slot
+            const int src = i_idx < p.P ? __ldg(p.slot_src + i_idx) : -1;
+            const int a_row = src >= 0 ? __ldg(p.slot_action + i_idx / p.slot_M) : -1;
+            int un = 0;
+            for (int u = 0; u < (S >> 3); ++u, ++un) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (src >= 0) v = load_row_unit(p.particles + (size_t)src * p.S_io, p.S_io, u);
+                st_shared_v4(a_unit_addr(a_slot, row, un), v.x, v.y, v.z, v.w);
+            }
+            for (int u = 0; u < (Nz >> 3); ++u, ++un) {
+                const uint4 v = noise_unit8(p.seed, (uint32_t)(src >= 0 ? src : 0), 0u, 0u, kStreamBeliefT, (uint32_t)u);
+                st_shared_v4(a_unit_addr(a_slot, row, un), v.x, v.y, v.z, v.w);
+            }
+            for (int u = 0; u < ((p.A + 7) >> 3); ++u, ++un) {
+                const bool here = a_row >= 0 && (a_row >> 3) == u;
+                const int wsel = (a_row & 7) >> 1;
+                const uint32_t one = (a_row & 1) ? 0x3F800000u : 0x00003F80u;
+                st_shared_v4(a_unit_addr(a_slot, row, un), (here && wsel == 0) ? one : 0u, (here && wsel == 1) ? one : 0u,
+                             (here && wsel == 2) ? one : 0u, (here && wsel == 3) ? one : 0u);
+            }
+            for (; un < in_units; ++un) st_shared_v4(a_unit_addr(a_slot, row, un), 0u, 0u, 0u, 0u);
+            return;
+        }
         const bool valid = i_idx < p.P;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
@@ -911,6 +957,86 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 tc_fence_before();
                 es.arrive_event();
                 T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
+            } else if (MODE == 3 && l.epi == T2_EPI_CHAIN) {
+                // opened branches: s' -> bf16 -> the state units of f_Z's input; the other half of the warps
+                // writes w_Z(src) (stream 5), the one-hot block and the zero padding
+                const int i_idx = row_index(step, slot);
+                const int src = i_idx < p.P ? __ldg(p.slot_src + i_idx) : -1;
+                es.wait_layer();
+                if (half == 0) {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        if (16 * g < (int)l.n_pad) {
+                            uint32_t v[16], o[8];
+                            tmem_ld16(taddr + 16 * g, v);
+                            float4 b[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                o[2 * i] = pack_bf16x2(__uint_as_float(v[4 * i]) + b[i].x, __uint_as_float(v[4 * i + 1]) + b[i].y);
+                                o[2 * i + 1] = pack_bf16x2(__uint_as_float(v[4 * i + 2]) + b[i].z, __uint_as_float(v[4 * i + 3]) + b[i].w);
+                            }
+#pragma unroll
+                            for (int h2 = 0; h2 < 2; ++h2) {
+                                const int u = 2 * g + h2;
+                                if (8 * u < S)
+                                    st_shared_v4(a_unit_addr(a_slot, row, u), o[4 * h2], o[4 * h2 + 1], o[4 * h2 + 2], o[4 * h2 + 3]);
+                            }
+                        }
+                    }
+                } else {
+                    const int a_row = src >= 0 ? __ldg(p.slot_action + i_idx / p.slot_M) : -1;
+                    int un = S >> 3;
+                    for (int u = 0; u < (Nz >> 3); ++u, ++un) {
+                        const uint4 v = noise_unit8(p.seed, (uint32_t)(src >= 0 ? src : 0), 0u, 0u, kStreamPwObs, (uint32_t)u);
+                        st_shared_v4(a_unit_addr(a_slot, row, un), v.x, v.y, v.z, v.w);
+                    }
+                    for (int u = 0; u < ((p.A + 7) >> 3); ++u, ++un) {
+                        const bool here = a_row >= 0 && (a_row >> 3) == u;
+                        const int wsel = (a_row & 7) >> 1;
+                        const uint32_t one = (a_row & 1) ? 0x3F800000u : 0x00003F80u;
+                        st_shared_v4(a_unit_addr(a_slot, row, un), (here && wsel == 0) ? one : 0u, (here && wsel == 1) ? one : 0u,
+                                     (here && wsel == 2) ? one : 0u, (here && wsel == 3) ? one : 0u);
+                    }
+                    for (; un < in_units; ++un) st_shared_v4(a_unit_addr(a_slot, row, un), 0u, 0u, 0u, 0u);
+                }
+                fence_proxy_async_smem();
+                tc_fence_before();
+                es.arrive_event();
+            } else if (MODE >= 3) {  // T2_EPI_OBS_STORE (MODE 3) | T2_EPI_EMB_STORE (MODE 4): last layer of the unit
+                const int i_idx = row_index(step, slot);
+                bool ok = i_idx < p.P;
+                if (MODE == 3) ok = ok && __ldg(p.slot_src + i_idx) >= 0;
+                else ok = ok && (i_idx % p.slot_M) < __ldg(p.slot_count + i_idx / p.slot_M);
+                const int width = MODE == 3 ? p.O : p.d;
+                float *dst = (MODE == 3 ? p.slot_obs : p.slot_emb) + (size_t)i_idx * width;
+                es.wait_layer();
+                if (half == 0) {
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        if (16 * g < (int)l.n_pad) {
+                            uint32_t v[16];
+                            tmem_ld16(taddr + 16 * g, v);
+                            float4 b[4];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) b[i] = *(reinterpret_cast<const float4 *>(bias + 16 * g) + i);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 4; ++i)
+                                if (ok && 16 * g + 4 * i < width)
+                                    *(reinterpret_cast<float4 *>(dst) + 4 * g + i) =
+                                        make_float4(__uint_as_float(v[4 * i]) + b[i].x, __uint_as_float(v[4 * i + 1]) + b[i].y,
+                                                    __uint_as_float(v[4 * i + 2]) + b[i].z, __uint_as_float(v[4 * i + 3]) + b[i].w);
+                        }
+                    }
+                }
+                if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot);
+                named_bar_sync(bar_id, 256);
+                fence_proxy_async_smem();
+                tc_fence_before();
+                es.arrive_event();
             } else if (MODE == 2) {  // T2_EPI_DIFFUSE: diffusion teacher, last (only) network of the unit
                 const int i_idx = row_index(step, slot);
                 const bool valid = i_idx < p.P;
@@ -1535,7 +1661,8 @@ struct Builder2 {
             }
         } else {
             for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
-            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE && epi != T2_EPI_DIFFUSE)  // the next layer-1 input is written with this event
+            if (epi != T2_EPI_REWARD && epi != T2_EPI_SCORE && epi != T2_EPI_DIFFUSE && epi != T2_EPI_OBS_STORE &&
+                epi != T2_EPI_EMB_STORE)  // the next layer-1 input is written with this event
                 for (int j = chunk_off; j < std::min(8, chunk_off + slot_chunks); ++j) a_ready[j] = evt;
             evt_set.push_back((uint8_t)((dual && par_split) ? slot : 0));
             ++evt;
@@ -1578,6 +1705,8 @@ struct T2Handle {
     // progressive widening: the belief program with the one-hot block in the operand (per-row actions)
     T2Program pw, pw_dual;
     bool has_pw = false, has_pw_dual = false;
+    T2Program pw_open, pw_emb;  // the small passes over the (action node, branch) slots (see T2Params)
+    bool has_pw_slots = false;
     // diffusion teachers (0 transition, 1 observation): one denoiser call per launch, [which][dual]
     T2Program diff[2][2];
     bool has_diff[2][2] = {{false, false}, {false, false}};
@@ -1896,6 +2025,31 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             }
         }
     }
+    // progressive widening, the slot passes: (f_T -> f_Z) over the opened slots, tower f over the stored ones
+    if (h->has_pw && d->obs_dim % 8 == 0 && d->lik_obs.dims[d->lik_obs.n_layers] % 16 == 0 &&
+        d->lik_obs.dims[d->lik_obs.n_layers] <= 128) {
+        bool ok = true;
+        for (int l = 1; l < d->lik_obs.n_layers; ++l) ok = ok && d->lik_obs.dims[l] <= 512;
+        std::string m1 = "x", m2 = "x";
+        if (ok) {
+            const int in_cols = Sp + Nzp + rup(A, 8);
+            Builder2 pb;
+            pb.policy = policy;
+            add_generator2_dense(pb, d->f_T, S, A, Nz, T2_EPI_CHAIN);
+            add_generator2_dense(pb, d->f_Z, S, A, Nz, T2_EPI_OBS_STORE);
+            h->pw_open.hdr.e_off = (int)pb.sbias_init.size();
+            m1 = finish_program(pb, h->pw_open, belief_tc2_kernel<3>, rup(in_cols, 64) / 64, sm_count, allocs);
+            Builder2 pe;
+            pe.policy = policy;
+            const voila_mlp &f = d->lik_obs;
+            for (int l = 0; l < f.n_layers; ++l)
+                pe.add_layer(f.W[l], f.dims[l + 1], f.dims[l], f.b[l], 1,
+                             l == f.n_layers - 1 ? T2_EPI_EMB_STORE : T2_EPI_HIDDEN, f.act);
+            h->pw_emb.hdr.e_off = (int)pe.sbias_init.size();
+            m2 = finish_program(pe, h->pw_emb, belief_tc2_kernel<4>, rup(d->obs_dim, 64) / 64, sm_count, allocs);
+        }
+        h->has_pw_slots = m1.empty() && m2.empty();
+    }
     // diffusion teachers: one program per denoiser (one- and two-slot)
     for (int which = 0; which < 2; ++which) {
         const voila_mlp &f = which == 0 ? d->denoise_T : d->denoise_Z;
@@ -1955,6 +2109,7 @@ bool tc2_has_belief(const void *tc) { return tc && reinterpret_cast<const T2Hand
 bool tc2_has_diffusion(const void *tc, int which) {
     return tc && reinterpret_cast<const T2Handle *>(tc)->has_diff[which][0];
 }
+bool tc2_has_pw_slots(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_pw_slots; }
 bool tc2_has_pw(const void *tc) { return tc && reinterpret_cast<const T2Handle *>(tc)->has_pw; }
 int tc2_pw_e_stride(const void *tc) { return reinterpret_cast<const T2Handle *>(tc)->pw.hdr.e_pad; }
 
@@ -2076,6 +2231,34 @@ cudaError_t launch_pw_propose_score_tc2(void *tc, const ModelDev &m, const PwArg
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight, per-row actions>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16, per-row actions>";
     return cudaGetLastError();
+}
+
+// Progressive widening, the two small passes over the (action node, branch) slots on the tensor cores:
+// sampled observations of the slots opened in this call, then the tower f over every stored branch.
+cudaError_t launch_pw_slots_tc2(void *tc, const ModelDev &m, const PwArgs &a, cudaStream_t st) {
+    const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
+    const int slots = a.G * a.M_max;
+    for (int pass = 0; pass < 2; ++pass) {
+        const T2Program &g = pass == 0 ? h->pw_open : h->pw_emb;
+        T2Params p = base_params(g, m);
+        p.particles = reinterpret_cast<const uint16_t *>(a.particles);
+        p.P = slots; p.Q = 1; p.H = 1;
+        p.seed = a.seed;
+        p.n_units = (slots + 2 * kT2Rows - 1) / (2 * kT2Rows);
+        p.d = m.mlp[3].dims[m.mlp[3].n_layers];
+        p.slot_src = a.new_src;
+        p.slot_action = a.group_action;
+        p.slot_count = a.branch_count;
+        p.slot_obs = a.branch_obs;
+        p.slot_emb = a.E;
+        p.slot_M = a.M_max;
+        const int clusters = std::min(g.max_clusters, p.n_units);
+        if (pass == 0) belief_tc2_kernel<3><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+        else belief_tc2_kernel<4><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // One DDIM-ODE step of a diffusion teacher on the CTA-pair tcgen05 program (2 launches: the step's

@@ -46,7 +46,10 @@ enum T2Epi : int {
     T2_EPI_OBS = 3,       // rollout: o = D + bias -> witness ; next operand = [s' ; w_T]
     T2_EPI_PROPOSAL = 4,  // belief: s' = D + bias -> proposals (HBM) ; next operand = [s']
     T2_EPI_SCORE = 5,     // belief: logit = <e, D + bias>/lambda + log w -> logits, running max
-    T2_EPI_DIFFUSE = 6    // diffusion teacher: v = D + bias ; x <- DDIM-ODE step(x, v) (fp32 state in HBM)
+    T2_EPI_DIFFUSE = 6,   // diffusion teacher: v = D + bias ; x <- DDIM-ODE step(x, v) (fp32 state in HBM)
+    T2_EPI_CHAIN = 7,     // progressive widening, opened branches: s' = D + bias ; next operand = [s' ; w_Z ; onehot(a)]
+    T2_EPI_OBS_STORE = 8, // ... o = D + bias -> the branch's stored observation (fp32, HBM)
+    T2_EPI_EMB_STORE = 9  // tower f over stored observations: e = D + bias -> embedding table (fp32, HBM)
 };
 
 struct T2Layer {  // what the epilogue needs to know about a layer

@@ -724,9 +724,14 @@ voila_status voila_pw_update(voila_ctx *ctx, const void *particles, int N, const
     a.obs_from_particles = tc_path ? 1 : 0;
     cudaError_t e = launch_pw_widen(a, st);                                  // branches, children, sorted order
     if (e == cudaSuccess && !tc_path) e = launch_pw_propose_ffma(ctx->model, a, bf16, st);  // s' of every simulation
-    if (e == cudaSuccess) e = launch_pw_obs_ffma(ctx->model, a, bf16, st);      // o of the opened branches
-    if (e == cudaSuccess)                                                     // e = f(o) of every stored branch: one batch
-        e = launch_mlp_forward_ffma(ctx->model, 2, branch_obs, G * M_max, a.E, bf16, st);
+    if (tc_path && tc2_has_pw_slots(ctx->tc2)) {
+        // o of the opened branches, then e = f(o) of every stored branch: two small tcgen05 passes over the slots
+        if (e == cudaSuccess) e = launch_pw_slots_tc2(ctx->tc2, ctx->model, a, st);
+    } else {
+        if (e == cudaSuccess) e = launch_pw_obs_ffma(ctx->model, a, bf16, st);      // o of the opened branches
+        if (e == cudaSuccess)                                                     // e = f(o) of every stored branch: one batch
+            e = launch_mlp_forward_ffma(ctx->model, 2, branch_obs, G * M_max, a.E, bf16, st);
+    }
     if (e == cudaSuccess) {                                                   // L_i, child maxima
         ProfScope prof(ctx, VOILA_K_PROPOSE, st);
         if (tc_path) {

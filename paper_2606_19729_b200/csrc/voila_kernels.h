@@ -67,6 +67,8 @@ bool tc2_has_diffusion(const void *tc2, int which);  // the denoiser program of 
 cudaError_t launch_diffusion_step_tc2(void *tc2, const ModelDev &m, const DiffusionArgs &a, int k, cudaStream_t st,
                                       std::string *kernel_name);
 bool tc2_has_pw(const void *tc2);  // the per-row-action propose+score program was built
+bool tc2_has_pw_slots(const void *tc2);  // ... and the two slot passes (opened branches, tower f)
+cudaError_t launch_pw_slots_tc2(void *tc2, const ModelDev &m, const PwArgs &a, cudaStream_t st);
 cudaError_t launch_pw_propose_score_tc2(void *tc2, const ModelDev &m, const PwArgs &a, const int32_t *sim_action,
                                         const int32_t *sim_seg, cudaStream_t st, std::string *kernel_name);
 cudaError_t launch_pw_resample(const PwArgs &a, const unsigned long long *cdf, int row_bytes, cudaStream_t st);  // 1-2 launches
