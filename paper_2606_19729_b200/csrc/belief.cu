@@ -48,6 +48,9 @@ __global__ void __launch_bounds__(kObsThreads) bu_init_obs_kernel(ScanBuffers sb
     __shared__ float xs[2][kObsMaxWidth];
     __shared__ float part[kObsThreads];
     const int tid = threadIdx.x;
+    // programmatic dependent launch: the propose+score kernel may start now (its proposal layers need
+    // nothing from here); it waits (griddepcontrol.wait) before it reads e or touches the running maximum
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int i = tid; i < tiles; i += kObsThreads) sb.tile_flag[i] = kFlagEmpty;
     if (tid == 0) {
         ScanState z;

@@ -764,8 +764,10 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 for (int c = tid_e; c < (int)L[li].n_pad; c += 256)
                     sbias[L[li].sbias_off + c] = __ldg(p.bias + L[li].bias_off + (size_t)p.bu_action * L[li].n_pad + c);
         }
-        for (int c = tid_e; c < p.hdr.e_pad; c += 256)
-            sbias[p.hdr.e_off + c] = (p.bu_e && c < p.d) ? __ldg(p.bu_e + c) : 0.0f;
+        // (MODE 0: e = f(o) comes from the kernel launched just before this one; it is copied at the
+        //  first SCORE epilogue, after griddepcontrol.wait: programmatic dependent launch)
+        if (MODE != 0)
+            for (int c = tid_e; c < p.hdr.e_pad; c += 256) sbias[p.hdr.e_off + c] = 0.0f;
     }
 
     // particle index of this thread's row in (unit, slot)
@@ -1101,6 +1103,15 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                 if (MODE == 1 && half == 0) {
                     seg = valid ? __ldg(p.pw_sim_seg + i_idx) : 0;
                     e_row = p.pw_E + (size_t)seg * (size_t)p.hdr.e_pad;
+                }
+                if (MODE == 0 && step == 0) {
+                    // everything the previous kernel produced (e, the reset running maximum) is needed from
+                    // here on only: wait for it now, park e in shared memory
+                    asm volatile("griddepcontrol.wait;" ::: "memory");
+                    const int tid_e = ((int)threadIdx.x - 128) & 255;
+                    for (int c = tid_e; c < p.hdr.e_pad; c += 256)
+                        sbias[p.hdr.e_off + c] = c < p.d ? p.bu_e[c] : 0.0f;
+                    named_bar_sync(bar_id, 256);
                 }
                 es.wait_layer();
                 T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
@@ -2189,8 +2200,20 @@ cudaError_t launch_bu_propose_score_tc2(void *tc, const ModelDev &m, const Belie
     p.inv_lambda = 1.0f / m.lambda;
     p.d = m.mlp[3].dims[m.mlp[3].n_layers];
     const int clusters = std::min(g.max_clusters, p.n_units);
-    if (dual) belief_tc2_dual_kernel<0><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
-    else belief_tc2_kernel<0><<<2 * clusters, kT2Threads, g.smem_bytes, st>>>(p, g.wmap);
+    // programmatic dependent launch: may start while the observation-tower kernel in front of it still runs
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(2 * clusters));
+    cfg.blockDim = dim3((unsigned)(dual ? kT2ThreadsDual : kT2Threads));
+    cfg.dynamicSmemBytes = g.smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const cudaError_t le = dual ? cudaLaunchKernelEx(&cfg, belief_tc2_dual_kernel<0>, p, g.wmap)
+                                : cudaLaunchKernelEx(&cfg, belief_tc2_kernel<0>, p, g.wmap);
+    if (le != cudaSuccess) return le;
     if (kernel_name)
         *kernel_name = dual ? "belief_tc2_dual_kernel<tcgen05 cta_group::2 bf16, two units in flight>"
                             : "belief_tc2_kernel<tcgen05 cta_group::2 bf16>";
