@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from paper_2606_19729_b200 import synth
-from tests.parity_util import TOL_BF16_STATE, TOL_BF16_VALUE, TOL_FP32, rel_inf, t2n
+from tests.parity_util import TOL_BF16_STATE, TOL_BF16_VALUE, TOL_FP32, rel_inf, rel_l2, t2n
 
 pytestmark = pytest.mark.gpu
 
@@ -136,3 +136,78 @@ def test_belief_update_ragged_million(torch_cuda, oracle):
     o = om.belief_update(synth.bf16_round_np(inp.bu_particles[:M]), 2, inp.observation,
                          None if inp.bu_weights is None else inp.bu_weights[:M], 7)
     assert rel_inf(g["proposals"][:M], o["proposals"]) <= TOL_BF16_STATE
+
+
+def test_progressive_widening_bench_size(torch_cuda, oracle):
+    """The progressive-widening leg of bench.py (2^18 simulations, 2048 ragged action nodes, M_max = 16,
+    config-3 model, two-slot tcgen05 program): every integer output against the oracle, ancestors bit-exact
+    given the GPU's own weights child by child, proposals on a sample of rows."""
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    cfg = synth.CONFIGS[3]
+    model = synth.make_model(cfg)
+    N, G, M = 1 << 18, 2048, 16
+    rng = np.random.default_rng(20260619 + 77)
+    parts = rng.standard_normal((N, cfg.S)).astype(np.float32)
+    cuts = np.concatenate([[0], np.sort(rng.integers(0, N + 1, G - 1)), [N]]).astype(np.int32)
+    acts = rng.integers(0, cfg.A, G).astype(np.int32)
+    bc0 = rng.integers(0, M // 2 + 1, G).astype(np.int32)
+    vc0 = (bc0 * 8).astype(np.int32)
+    bo0 = rng.standard_normal((G, M, cfg.O)).astype(np.float32)
+    ctx = vl.Voila(model, device=0)
+    t = lambda a: torch.from_numpy(a.copy()).cuda()
+    t_vc, t_bc, t_bo = t(vc0), t(bc0), t(bo0)
+    out = ctx.voila_pw_update(ctx.to_particles(parts), t(cuts), t(acts), t_vc, t_bc, t_bo, 1.5, 0.5, None, 9000)
+    torch.cuda.synchronize()
+    assert "belief_tc2_dual_kernel" in ctx.voila_last_belief_kernel()
+    g = {k: (t2n(v) if v.dtype.is_floating_point else v.cpu().numpy()) for k, v in out.items()}
+    ctx.close()
+    ref = oracle.OracleModel(model, emulate_bf16=True).pw_update(synth.bf16_round_np(parts), cuts, acts, vc0, bc0, bo0,
+                                                                  1.5, 0.5, None, 9000)
+    for k in ("sim_branch", "opened", "seg_status"):
+        assert np.array_equal(g[k], ref[k]), k
+    assert np.array_equal(t_bc.cpu().numpy(), ref["branch_count"]) and np.array_equal(t_vc.cpu().numpy(), ref["visit_count"])
+    rows = rng.choice(N, 4096, replace=False)
+    assert rel_inf(g["proposals"][rows], ref["proposals"][rows]) <= TOL_BF16_STATE
+    opened = np.flatnonzero(ref["opened"])[:512]
+    gb, rb = t_bo.cpu().numpy(), ref["branch_obs"]
+    for i in opened:
+        gi = int(np.searchsorted(cuts, i, side="right") - 1)
+        b = int(ref["sim_branch"][i])
+        assert np.abs(gb[gi, b] - rb[gi, b]).max() <= 2 * TOL_BF16_STATE * max(1.0, float(np.abs(rb[gi, b]).max()))
+    # children: resampled among their own members, bit-exact given the GPU's weights (a sample of nodes)
+    seg = np.repeat(np.arange(G), np.diff(cuts)) * M + ref["sim_branch"]
+    for gi in rng.choice(G, 64, replace=False):
+        idx = np.arange(cuts[gi], cuts[gi + 1])
+        for b in range(ref["branch_count"][gi]):
+            mem = idx[ref["sim_branch"][idx] == b]
+            if mem.size == 0:
+                continue
+            v = g["post_weights"][mem]
+            x0 = oracle.philox4x32_10([gi * M + b, 0, 0, 4 << 16], [9000, 0])[0]
+            a_loc, st = oracle.resample_systematic_x0(v, int(x0))
+            assert st == 0 and np.array_equal(g["ancestors"][mem], mem[a_loc])
+    assert np.array_equal(seg[g["ancestors"]], seg)  # every draw stays inside its child, for ALL simulations
+    assert np.array_equal(g["particles"], g["proposals"][g["ancestors"]])
+
+
+def test_diffusion_teacher_bench_size_sampled(torch_cuda, oracle):
+    """The diffusion-teacher leg of bench.py (2^16 samples, 4 x 512 denoiser, K = 32): the first 1024 samples
+    against the oracle (the noise is keyed by the absolute sample index, so a prefix reproduces them)."""
+    import paper_2606_19729_b200 as vl
+    torch = torch_cuda
+    cfg = synth.CONFIGS[3]
+    vT, vZ = synth.make_denoisers(cfg, [512, 512, 512, 512])
+    model = synth.make_model(cfg).replace(denoise_T=vT, denoise_Z=vZ)
+    N, K, n_ref = 1 << 16, 32, 1024
+    rng = np.random.default_rng(20260619 + 88)
+    cond = rng.standard_normal((N, cfg.S)).astype(np.float32)
+    act = rng.integers(0, cfg.A, N).astype(np.int32)
+    ctx = vl.Voila(model, device=0)
+    out = t2n(ctx.voila_diffusion_sample(0, ctx.to_particles(cond), torch.from_numpy(act).cuda(), K, 2))
+    torch.cuda.synchronize()
+    assert "belief_tc2_kernel" in ctx.voila_last_belief_kernel()
+    ctx.close()
+    ref = oracle.OracleModel(model, emulate_bf16=True).diffusion_sample(0, synth.bf16_round_np(cond[:n_ref]), act[:n_ref], K, 2)
+    assert np.all(np.isfinite(out))
+    assert rel_l2(out[:n_ref], ref) <= TOL_BF16_STATE and rel_inf(out[:n_ref], ref) <= TOL_BF16_STATE
