@@ -136,6 +136,41 @@ def test_belief_update_degenerate_weights(torch_cuda):
     assert np.isneginf(g["log_evidence"][0])
 
 
+@pytest.mark.parametrize("prec", [synth.PREC_FP32, synth.PREC_BF16])
+@pytest.mark.parametrize("bad", ["nan_state", "inf_weight"])
+def test_belief_update_nonfinite_score(torch_cuda, oracle, prec, bad):
+    """Reading R20: a non-finite L_i (a NaN carried from one particle's state through f_T and g, or
+    +inf from an infinite prior weight) gives device status 1 on the GPU and a non-zero status in the
+    oracle, and the documented degenerate outputs: ancestors = identity, particles_out = proposals,
+    weights 1/N, log-evidence -inf.  On the tensor-core path the NaN stays in its own accumulator row."""
+    cfg = synth.CONFIGS[2]
+    model = synth.make_model(cfg)
+    N = 1000
+    inp = synth.make_inputs(cfg, N=N, P=8, Q=1, H=1)
+    w = np.full(N, 1.0 / N, np.float32)
+    parts = inp.bu_particles.copy()
+    if bad == "nan_state":
+        parts[617, 3] = np.nan
+    else:
+        w[617] = np.inf
+    g = _gpu_bu(torch_cuda, model, parts, 1, inp.observation, w, 5, prec)
+    om = oracle.OracleModel(model)
+    o = om.belief_update(synth.bf16_round_np(parts) if prec == synth.PREC_BF16 else parts, 1, inp.observation, w, 5)
+    assert o["status"] != 0
+    assert int(g["status"][0]) == 1
+    assert np.array_equal(g["ancestors"], np.arange(N)) and np.array_equal(o["ancestors"], np.arange(N))
+    assert np.array_equal(g["particles"], g["proposals"], equal_nan=True)
+    if bad == "nan_state":   # the NaN poisons its own row only
+        assert np.all(np.isnan(g["proposals"][617])) or np.isnan(g["proposals"][617]).any()
+        assert np.isfinite(np.delete(g["proposals"], 617, axis=0)).all()
+    assert np.all(g["weights"] == np.float32(1.0) / np.float32(N))
+    assert np.isneginf(g["log_evidence"][0]) and np.isneginf(o["log_evidence"])
+    # a NaN prior WEIGHT is not > 0: a zero weight on both sides, the update stays regular
+    w[617] = np.nan
+    g = _gpu_bu(torch_cuda, model, inp.bu_particles, 1, inp.observation, w, 5, prec)
+    assert int(g["status"][0]) == 0 and not np.any(g["ancestors"] == 617)
+
+
 @pytest.fixture(scope="module")
 def resample_ctx(torch_cuda):
     import paper_2606_19729_b200 as vl

@@ -5,6 +5,7 @@ likelihood (SURVEY 8c pin 5), scipy.special.logsumexp (library), invariances the
 (only relative weights matter), and a step-by-step recomposition from the separately
 pinned pieces (MLP forward, noise, resampler).
 """
+import pytest
 import numpy as np
 import scipy.special
 
@@ -155,3 +156,32 @@ def test_all_zero_prior_weights_pass_through(oracle):
     assert out["status"] == -2
     assert np.array_equal(out["ancestors"], np.arange(cfg.N))
     assert np.array_equal(out["particles"], out["proposals"])
+
+
+@pytest.mark.parametrize("bad", ["nan_state", "inf_weight"])
+def test_nonfinite_score_is_flagged(oracle, bad):
+    """Reading R20: any non-finite L_i (a NaN that a particle's state carried through
+    f_T and g, or +inf from an infinite prior weight) makes the update degenerate: non-zero status,
+    identity ancestors, particles_out = proposals, weights 1/N, log-evidence -inf; it never leaks
+    into the resampler.  (A NaN prior WEIGHT is not > 0 and counts as a zero weight.)"""
+    cfg = synth.CONFIGS[2]
+    om = oracle.OracleModel(synth.make_model(cfg))
+    N = 300
+    inp = synth.make_inputs(cfg, N=N)
+    w = np.full(N, 1.0 / N, np.float32)
+    parts = inp.bu_particles.copy()
+    if bad == "nan_state":
+        parts[17, 3] = np.nan
+    else:
+        w[17] = np.inf
+    out = om.belief_update(parts, 2, inp.observation, w, 11)
+    assert out["status"] != 0
+    assert (np.isnan(out["logits"][17]) if bad == "nan_state" else np.isposinf(out["logits"][17]))
+    assert np.array_equal(out["ancestors"], np.arange(N))
+    assert np.array_equal(out["particles"], out["proposals"], equal_nan=True)
+    assert np.all(out["weights"] == np.float32(1.0) / np.float32(N))
+    assert np.isneginf(out["log_evidence"])
+    # a NaN prior weight is a zero weight: the update stays regular and never picks that particle
+    w[17] = np.nan
+    out = om.belief_update(inp.bu_particles, 2, inp.observation, w, 11)
+    assert out["status"] == 0 and not np.any(out["ancestors"] == 17)
