@@ -120,6 +120,7 @@ struct T2Params {
 struct Smem2 {
     uint32_t a, ring, layers, tiles, bars, misc, sbias, total;
 };
+constexpr uint32_t kT2SlotMisc = 4 * 8 + 4 * 64 * 4 + 256;  // red_g[4] doubles, red_w[4][64] floats, alive[2][128] bytes
 __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     Smem2 m;
     m.a = 0;
@@ -128,7 +129,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
     m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2TileDev) + 15u) & ~15u);
     m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing + kT2FreeRing) * 8;
-    m.sbias = m.misc + 16 + 4 * 8 + 4 * 64 * 4 + 256;  // + per-row alive flags, two step parities
+    m.sbias = m.misc + 16 + 2 * kT2SlotMisc;  // per slot: reduction scratch + per-row alive flags (two step parities)
     m.total = m.sbias + (((uint32_t)h.sbias_floats * 4u + 15u) & ~15u);
     return m;
 }
@@ -385,13 +386,25 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                             uint64_t *evt, uint64_t *layer_done, double *red_g, float *red_w,
                                             uint8_t *alive_s, float *sbias, int warp, int lane, uint32_t rank,
                                             int cluster_id, int n_clusters, int n_my_units, int total_steps,
-                                            bool shared_hidden) {
+                                            bool shared_hidden, int my_slot) {
     // shared_hidden: a second set of epilogue warps takes the odd chunks of the hidden layers
+    // my_slot < 0: one unit in flight.  my_slot = 0 | 1: TWO-SLOT program (hdr.n_slots == 2, models
+    // whose layers are all <= 256 wide): this set of eight warps owns the rows of one slot (own operand
+    // chunks, TMEM columns, reduction scratch, named barrier) and only keeps the books (event,
+    // accumulator-block and chunk-free sequence numbers) for the other slot's layer records, so one
+    // unit's epilogue overlaps the other unit's MMAs.  Both slots of a work unit belong to the same
+    // sequence q (two adjacent 256-particle blocks): they share the action-dependent bias rows.
     const int n_layers = p.hdr.n_layers;
     const uint32_t evt_cl = mapa_u32(smem_u32(evt), 0u);
+    const int n_slots = my_slot < 0 ? 1 : 2, slot_i = my_slot > 0 ? 1 : 0;
+    const uint32_t bar_id = 1u + (uint32_t)slot_i;
+    a_u32 += (uint32_t)(slot_i * p.hdr.slot_chunks) * kT2ChunkBytes;
+    red_g += 4 * slot_i;
+    red_w += 4 * 64 * slot_i;
+    alive_s += 2 * kT2Rows * slot_i;
     {
         // ===== epilogue warps =====
-        const int ew = warp - 4, qd = warp & 3, half = ew >> 2;
+        const int ew = (warp - 4) & 7, qd = warp & 3, half = ew >> 2;
         const int row = qd * 32 + lane;
         const uint32_t lane_taddr = tmem_base + ((uint32_t)(qd * 32) << 16);
         const int S = p.S, O = p.O, Nz = p.Nz;
@@ -414,7 +427,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         auto load_unit = [&]() {
             const int unit = cluster_id + unit_i * n_clusters;
             q = unit / p.blocks_per_q;
-            blk = (unit - q * p.blocks_per_q) * 2 + (int)rank;  // 128-row tile index within the sequence
+            blk = ((unit - q * p.blocks_per_q) * n_slots + slot_i) * 2 + (int)rank;  // 128-row tile index within the sequence
             p_idx = blk * kT2Rows + row;
             valid = p_idx < p.P;
             w_row = valid ? (p.weights ? __ldg(p.weights + p_idx) : 1.0f) : 0.0f;
@@ -501,7 +514,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         // Bias rows that depend on the action (one-hot block folded into the bias, R21):
         // the rows of the NEXT step are fetched mid-step into registers and parked in the other
         // half of a two-row slot of the shared-memory bias table at the end of the step.
-        const int tid_e = (int)threadIdx.x - 128;
+        const int tid_e = ((int)threadIdx.x - 128) & 255;  // (two-slot: both sets park the same rows)
         float4 pa_reg[2] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
         auto refresh_issue = [&](int q_next, int t_next) {
             const int a_next = clamp_action(__ldg(p.seqs + (size_t)q_next * p.H + t_next), p.A);
@@ -524,15 +537,17 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         };
 
         if (n_my_units > 0) {
+            if (slot_i == 1) ++es.ev;  // slot 0's initial event (hdr.init_events = one per slot)
             load_unit();
             refresh_issue(q, 0);
             if (half == 0) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, 0u, kStreamRolloutT, Nz);
             write_input(0, 0);
             step_reward();
             refresh_store(0);
-            named_bar_sync(1, 256);
+            named_bar_sync(bar_id, 256);
             fence_proxy_async_smem();
             arrive_event();
+            if (my_slot == 0) ++es.ev;  // slot 1's initial event
         }
         for (int step = 0; step < total_steps; ++step) {
             const int a_t = clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A);
@@ -542,6 +557,13 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
             for (int li = 0; li < n_layers; ++li) {
                 const T2Layer l = L[li];
                 es.tl_layer = (uint32_t)li;
+                if (my_slot >= 0 && (int)l.slot != my_slot) {  // the other set's record: sequence numbers only
+                    const bool hid = l.epi == T2_EPI_HIDDEN;
+                    es.ev += hid ? (int)(l.n_pad >> 6) : 1;
+                    es.ld_seq += hid ? (uint32_t)__popc((unsigned)l.blk_mask) : 1u;
+                    if (hid && l.wait_chunks > 0) es.free_seq += ((uint32_t)l.wait_chunks + l.free_nk - 1u) / l.free_nk;
+                    continue;
+                }
                 const float *bias = sbias + l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
                 if (l.epi == T2_EPI_HIDDEN) {
                     const int boff = (int)l.sbias_off + (l.bias_per_action ? (step & 1) * (int)l.n_pad : 0);
@@ -672,16 +694,17 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                                 }
                             }
                         }
-                        named_bar_sync(1, 256);
-                        if (ew == 0 && lane == 0)
+                        named_bar_sync(bar_id, 256);
+                        // (two-slot: the second slot of a sequence's last pair may lie past the last tile)
+                        if (ew == 0 && lane == 0 && blk < p.tiles_per_q)
                             p.part_value[(size_t)q * p.tiles_per_q + blk] = (red_g[0] + red_g[1]) + (red_g[2] + red_g[3]);
-                        if (ew == 4 && p.part_witness) {
+                        if (ew == 4 && p.part_witness && blk < p.tiles_per_q) {
                             for (int c = lane; c < O; c += 32)
                                 p.part_witness[((size_t)q * p.tiles_per_q + blk) * O + c] =
                                     ((double)red_w[c] + (double)red_w[64 + c]) +
                                     ((double)red_w[128 + c] + (double)red_w[192 + c]);
                         }
-                        named_bar_sync(1, 256);
+                        named_bar_sync(bar_id, 256);
                         ++unit_i;
                         if (unit_i < n_my_units) {
                             load_unit();
@@ -695,7 +718,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     refresh_store((step + 1) & 1);
                     {
                         T2_TRACE_T0();
-                        named_bar_sync(1, 256);
+                        named_bar_sync(bar_id, 256);
                         T2_TRACE_ADD(es.tr_bar);
                     }
                     fence_proxy_async_smem();
@@ -1187,9 +1210,9 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
     uint64_t *evt = empty + 8;
     uint64_t *layer_done = evt + kT2EvtRing;
     uint32_t *tmem_ptr = reinterpret_cast<uint32_t *>(smem + map.misc);
-    double *red_g = reinterpret_cast<double *>(smem + map.misc + 16);
-    float *red_w = reinterpret_cast<float *>(smem + map.misc + 16 + 4 * 8);
-    uint8_t *alive_s = smem + map.misc + 16 + 4 * 8 + 4 * 64 * 4;
+    double *red_g = reinterpret_cast<double *>(smem + map.misc + 16);                 // [2 slots][4]
+    float *red_w = reinterpret_cast<float *>(smem + map.misc + 16 + 2 * 4 * 8);       // [2 slots][4][64]
+    uint8_t *alive_s = smem + map.misc + 16 + 2 * 4 * 8 + 2 * 4 * 64 * 4;             // [2 slots][2][128]
     float *sbias = reinterpret_cast<float *>(smem + map.sbias);
     const uint32_t a_u32 = smem_u32(smem + map.a), ring_u32 = smem_u32(smem + map.ring);
 
@@ -1393,7 +1416,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                            n_my_units, NTHREADS == kT2Threads ? -1 : 0);
         else
             t2_epilogue<BELIEF ? 0 : MODE>(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, alive_s, sbias, warp, lane, rank,
-                        cluster_id, n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads);
+                        cluster_id, n_clusters, n_my_units, total_steps, NTHREADS != kT2Threads && R_HELP < 0,
+                        (NTHREADS != kT2Threads && R_HELP > 0) ? 0 : -1);
     } else {
         // second set of epilogue warps (640-thread kernels)
         if (R_HELP > 0) setmaxnreg_inc<(R_HELP > 0 ? R_HELP : 24)>();
@@ -1401,6 +1425,9 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         if (BELIEF)
             t2_bu_epilogue<BELIEF ? MODE : 0>(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, rank, cluster_id, n_clusters,
                            n_my_units, 1);
+        else if (R_HELP > 0)  // two-slot rollout: the second slot's own set of stateful epilogue warps
+            t2_epilogue<BELIEF ? 0 : MODE>(p, L, a_u32, tmem_base, evt, layer_done, red_g, red_w, alive_s, sbias, warp, lane, rank,
+                        cluster_id, n_clusters, n_my_units, total_steps, false, 1);
         else
             t2_helper_epilogue(p, L, a_u32, tmem_base, evt, layer_done, sbias, warp, lane, total_steps);
     }
@@ -1436,6 +1463,14 @@ template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
     rollout_tc2x_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
     tc2_body<false, kT2ThreadsDual, 32, 168, -56, MODE>(p, wmap);
+}
+// Two-slot rollout (generators whose layers are all <= 256 wide): two 256-particle blocks of one
+// sequence in flight per CTA pair, each with its own set of eight stateful epilogue warps (state /
+// witness in registers), so that one block's epilogue overlaps the other block's MMAs.
+template <int MODE>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kT2ThreadsDual, 1)
+    rollout_tc2d_kernel(const T2Params p, const __grid_constant__ CUtensorMap wmap) {
+    tc2_body<false, kT2ThreadsDual, 32, 112, 112, MODE>(p, wmap);
 }
 
 }  // namespace
@@ -1725,6 +1760,8 @@ struct T2Handle {
     int diff_n1[2] = {0, 0};
     float diff_scale[2] = {1.0f, 1.0f};
     bool roll_x = false;    // rollout runs the 640-thread kernel (two sets of epilogue warps)
+    T2Program roll_dual;    // rollout with two 256-particle blocks in flight per CTA pair (layers <= 256 wide)
+    bool has_roll_dual = false;
     int Sp = 0, Nzp = 0;    // operand widths of the state and the noise (public widths rounded up to 8)
 };
 
@@ -1986,6 +2023,26 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             return nullptr;
         }
     }
+    {
+        // Two-slot rollout program (narrow generators): 4 operand chunks and 256 TMEM columns per slot,
+        // shared weight tiles, the tile program alternating the slots layer by layer.
+        int w = Sp + Nzp;
+        for (const voila_mlp *f : {&d->f_T, &d->f_Z})
+            for (int l = 1; l <= f->n_layers; ++l) w = std::max(w, rup(f->dims[l], l == f->n_layers ? 16 : 64));
+        if (w <= 256 && !getenv("VOILA_T2_ROLLOUT_1SLOT")) {
+            Builder2 pb;
+            pb.policy = policy;
+            pb.set_dual(4, 256);
+            if (d->reward.kind == VOILA_R_NEG_QUADRATIC)
+                pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);
+            add_generator2(pb, d->f_T, S, A, Nz, T2_EPI_STATE);
+            add_generator2(pb, d->f_Z, S, A, Nz, T2_EPI_OBS);
+            const std::string m =
+                term ? finish_program(pb, h->roll_dual, rollout_tc2d_kernel<1>, rup(Sp + Nzp, 64) / 64, sm_count, allocs, kT2ThreadsDual)
+                     : finish_program(pb, h->roll_dual, rollout_tc2d_kernel<0>, rup(Sp + Nzp, 64) / 64, sm_count, allocs, kT2ThreadsDual);
+            h->has_roll_dual = m.empty();  // (the one-slot program serves if this one does not fit)
+        }
+    }
     if (tower_fits_tc2(d)) {
         // belief-update program: proposal s' = f_T(s, a, w), then the state tower g(s') and the score.
         // Narrow models (every layer <= 256 wide, every K <= 256) get a second, TWO-SLOT build: two
@@ -2146,7 +2203,11 @@ T2Params base_params(const T2Program &g, const ModelDev &m) {
 cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a, cudaStream_t st,
                                std::string *kernel_name, int *n_launches) {
     const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
-    const T2Program &g = h->roll;
+    // two blocks in flight per CTA pair: when a sequence has an even number of 256-particle blocks (no
+    // idle slot) and every CTA pair gets more than one pair of blocks
+    const int blocks = (a.P + 2 * kT2Rows - 1) / (2 * kT2Rows);
+    const bool dual = h->has_roll_dual && blocks % 2 == 0 && (blocks / 2) * a.Q > h->roll_dual.max_clusters;
+    const T2Program &g = dual ? h->roll_dual : h->roll;
     T2Params p = base_params(g, m);
     p.particles = reinterpret_cast<const uint16_t *>(a.particles);
     p.seqs = a.action_seqs;
@@ -2157,11 +2218,18 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     p.part_witness = a.part_witness;
     p.returns_out = a.returns_out;
     p.final_states_out = a.final_states_out;
-    p.blocks_per_q = (a.P + 2 * kT2Rows - 1) / (2 * kT2Rows);
-    p.tiles_per_q = a.tiles;  // = 2 * blocks_per_q (see rollout_tile_count)
+    p.blocks_per_q = dual ? blocks / 2 : blocks;  // work units of a CTA pair per sequence
+    p.tiles_per_q = a.tiles;  // = 2 * blocks (see rollout_tile_count)
     p.n_units = p.blocks_per_q * a.Q;
     const int clusters = std::min(g.max_clusters, p.n_units);
     const bool term = m.term.n > 0;
+    if (dual) {
+        if (term) rollout_tc2d_kernel<1><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+        else rollout_tc2d_kernel<0><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
+        if (kernel_name) *kernel_name = "rollout_tc2d_kernel<tcgen05 cta_group::2 bf16, two blocks in flight>";
+        if (n_launches) *n_launches = 1;
+        return cudaGetLastError();
+    }
     if (h->roll_x) {
         if (term) rollout_tc2x_kernel<1><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);
         else rollout_tc2x_kernel<0><<<2 * clusters, kT2ThreadsDual, g.smem_bytes, st>>>(p, g.wmap);

@@ -155,6 +155,33 @@ def test_bf16_mode_within_north_star(torch_cuda, oracle, kernel_name, cfg_idx, P
     assert rel_l2(g["returns"], e["returns"]) <= 5e-3
 
 
+@pytest.mark.parametrize("cfg_idx,P,Q,H,weighted", [(2, 300, 80, 6, False), (3, 1000, 40, 4, True),
+                                                    (3, 512, 75, 3, False)])
+def test_bf16_two_slot_rollout(torch_cuda, oracle, cfg_idx, P, Q, H, weighted):
+    """Generators <= 256 wide, an even number of 256-particle blocks per sequence and more pairs of
+    blocks than CTA pairs: AUTO runs the two-slot kernel (two blocks of one sequence in flight per CTA
+    pair, one set of stateful epilogue warps each).  Ragged last block, zero weights, every output."""
+    import paper_2606_19729_b200 as vl
+    cfg = synth.CONFIGS[cfg_idx]
+    model = synth.make_model(cfg, prec=synth.PREC_BF16, action_cost=True)
+    inp = synth.make_inputs(cfg, P=P, Q=Q, H=H)
+    w = None
+    if weighted:
+        w = np.random.default_rng(3).uniform(0.0, 2.0, P).astype(np.float32)
+        w[::5] = 0.0
+    g = _run_gpu(torch_cuda, model, inp, synth.PREC_BF16, vl.KERNEL_AUTO, weights=w, seed=7)
+    assert "rollout_tc2d_kernel" in g["kernel"], g["kernel"]
+    o = _run_oracle(oracle, model, inp, weights=w, seed=7, bf16_inputs=True)
+    assert_close(g["final_states"], o["final_states"], TOL_BF16_STATE, "final states")
+    assert value_err(g["values"], o["values"]) <= TOL_BF16_VALUE
+    assert value_err(g["returns"], o["returns"]) <= TOL_BF16_STATE
+    assert_close(g["witness"], o["witness"], TOL_BF16_STATE, "witness")
+    # same inputs through the one-block kernel family: same arithmetic per row, so the per-trajectory
+    # returns agree to rounding order of the tensor-core accumulation (not bit-exact: block shapes differ)
+    h = _run_gpu(torch_cuda, model, inp, synth.PREC_BF16, vl.KERNEL_TCGEN05, weights=w, seed=7, want_final=False)
+    assert rel_l2(g["returns"], h["returns"]) <= 5e-3
+
+
 def test_rollout_bitwise_reproducible(torch_cuda):
     """No float atomics, fixed-order reductions: two calls give identical bits."""
     import paper_2606_19729_b200 as vl

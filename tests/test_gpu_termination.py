@@ -87,12 +87,14 @@ def test_termination_fp32_cfg1(torch_cuda, oracle):
     assert "ffma" in k
 
 
-@pytest.mark.parametrize("cfg_idx,P,Q,H", [(2, 1000, 12, 15), (3, 700, 6, 12)])
+@pytest.mark.parametrize("cfg_idx,P,Q,H", [(2, 1000, 12, 15), (3, 700, 6, 12), (2, 1000, 40, 10)])
 def test_termination_bf16_tensor_core(torch_cuda, oracle, cfg_idx, P, Q, H):
     import paper_2606_19729_b200 as vl
     k = _compare(torch_cuda, oracle, cfg_idx, synth.PREC_BF16, vl.KERNEL_AUTO, P=P, Q=Q, H=H,
                  tol=TOL_BF16_STATE, margin_min=3e-3, max_excluded=0.5)
     assert "rollout_tc2" in k
+    if Q == 40:  # four 256-particle blocks x 40 sequences: the two-slot kernel (alive flags per slot)
+        assert "rollout_tc2d" in k
 
 
 def test_termination_bf16_ffma(torch_cuda, oracle):
