@@ -125,7 +125,7 @@ __host__ __device__ inline Smem2 smem2_map(const T2Header &h) {
     Smem2 m;
     m.a = 0;
     m.ring = m.a + (uint32_t)h.a_chunks * kT2ChunkBytes;
-    m.layers = m.ring + (uint32_t)h.n_stages * kT2StageBytes;
+    m.layers = m.ring + (uint32_t)h.n_stages * (uint32_t)h.stage_rows * 128u;
     m.tiles = m.layers + kT2MaxLayers * (uint32_t)sizeof(T2Layer);
     m.bars = m.tiles + (((uint32_t)h.n_tiles * (uint32_t)sizeof(T2TileDev) + 15u) & ~15u);
     m.misc = m.bars + (8 + 8 + kT2EvtRing + kT2AccRing + kT2FreeRing) * 8;
@@ -417,6 +417,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         bool alive = true;  // the row's episode still runs (terminal regions, reading R25)
         const long long tr_start = clock64();
         EpiSync es;
+        es.tl_kind = my_slot > 0 ? 5u : 3u;
         es.evt_cl = evt_cl;
         es.layer_done = layer_done;
         es.cfree = layer_done + kT2AccRing;
@@ -552,7 +553,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
         for (int step = 0; step < total_steps; ++step) {
             const int a_t = clamp_action(__ldg(p.seqs + (size_t)q * p.H + t), p.A);
 #ifdef VOILA_T2_TRACE
-            es.tl_on = blockIdx.x == 0 && warp == 4 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
+            es.tl_on = blockIdx.x == 0 && ew == 0 && lane == 0 && step >= g_t2_tl_win[0] && step < g_t2_tl_win[1];
 #endif
             for (int li = 0; li < n_layers; ++li) {
                 const T2Layer l = L[li];
@@ -573,7 +574,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     else epi_hidden_layer(es, l, boff, ecs);
                 } else if (l.epi == T2_EPI_REWARD) {
                     wait_layer();
-                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 0) {
                         float r = 0.0f;
 #pragma unroll
@@ -596,7 +597,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     }
                     tc_fence_before();
                     arrive_event();
-                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
                 } else if (l.epi == T2_EPI_STATE) {
                     // w_Z(t) is independent of the state: draw it while the output layer's MMAs run
                     if (half == 1) gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)t, kStreamRolloutZ, Nz);
@@ -604,7 +605,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     else if (unit_i + 1 < n_my_units)
                         refresh_issue((cluster_id + (unit_i + 1) * n_clusters) / p.blocks_per_q, 0);
                     wait_layer();
-                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 0) {
 #pragma unroll
                         for (int g = 0; g < 4; ++g) {
@@ -632,13 +633,13 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
-                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
                 } else {  // T2_EPI_OBS: last layer of the step
                     const bool last_step = (t == p.H - 1);
                     if (half == 0 && !last_step)
                         gen_noise_call(nz, p.seed, (uint32_t)p_idx, (uint32_t)q, (uint32_t)(t + 1), kStreamRolloutT, Nz);
                     wait_layer();
-                    T2_TL(es.tl_on, (3u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | 0xffu);
                     if (half == 1) {
                         // no observation for a row whose episode ended at or before step t
                         const float disc_w = (MODE == 0 || alive_s[(t & 1) * kT2Rows + row] != 0) ? disc : 0.0f;
@@ -724,7 +725,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                     fence_proxy_async_smem();
                     tc_fence_before();
                     arrive_event();
-                    T2_TL(es.tl_on, (4u << 24) | (es.tl_layer << 8) | 0xffu);
+                    T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | 0xffu);
                 }
             }
         }
@@ -1265,6 +1266,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
         // ===== producer: this CTA's half of every weight tile, in issue order, once per step =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
+            const uint32_t stage_bytes = (uint32_t)p.hdr.stage_rows * 128u;
             long long tr_empty = 0;
             const long long tr_start = clock64();
             for (int step = 0; step < total_steps; ++step) {
@@ -1276,8 +1278,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                         mbar_wait(&empty[stage], phase ^ 1u);
                         T2_TRACE_ADD(tr_empty);
                     }
-                    if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2u * kT2StageBytes);
-                    tma_load_2d_2cta(smem + map.ring + stage * kT2StageBytes, &wmap, &full[stage], 0,
+                    if (rank == 0) mbar_arrive_expect_tx(&full[stage], 2u * stage_bytes);
+                    tma_load_2d_2cta(smem + map.ring + stage * stage_bytes, &wmap, &full[stage], 0,
                                      (int32_t)src_row + (int32_t)rank * rows);
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
@@ -1306,6 +1308,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             int waited0 = -1, waited1 = -1;  // latest event waited for, per publishing set (T2Tile::need2)
             const uint32_t a_desc_lo = (uint32_t)umma_desc_sw128(a_u32), ring_desc_lo = (uint32_t)umma_desc_sw128(ring_u32);
             const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0u) >> 32);
+            const uint32_t stage_b16 = (uint32_t)p.hdr.stage_rows * 8u;  // stage bytes / 16 (descriptor units)
             int base = p.hdr.init_events, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
@@ -1361,7 +1364,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                     // offsets to the low word instead of rebuilding them (the rebuilt form was ~100
                     // uniform-datapath instructions per tile)
                     uint32_t a_lo = a_desc_lo + r0.z;
-                    uint32_t b_lo = ring_desc_lo + stage * (kT2StageBytes >> 4);
+                    uint32_t b_lo = ring_desc_lo + stage * stage_b16;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {  // a stage holds up to 4 K chunks
                         if (c >= (int)nk) break;
@@ -1538,10 +1541,12 @@ struct Builder2 {
     int slot = 0, chunk_off = 0, col_off = 0, slot_chunks = 8;
     int n_blocks = 0;  // accumulator blocks of the step so far (each is handed to the epilogues on its own)
     int policy = 0;
+    int stage_rows = 128;  // weight rows per CTA per ring stage (T2Header::stage_rows)
 
     Builder2() {
         for (int &c : col_free) c = -1;
         for (int &a : a_ready) a = -1;
+        if (const char *e = getenv("VOILA_T2_STAGE_ROWS")) stage_rows = atoi(e) == 256 ? 256 : 128;  // tuning knob
     }
 
     // Two-slot mode: every layer is added once per slot (slot 1 shares slot 0's biases and weight
@@ -1614,7 +1619,7 @@ struct Builder2 {
         int n_start = 0;
         for (size_t bi = 0; bi < blocks.size(); ++bi) {
             const int bn = blocks[bi], half = bn / 2;
-            const int nk_max = std::max(1, std::min(4, 128 / half));
+            const int nk_max = std::max(1, std::min(4, stage_rows / half));
             int blk_need = -1000;
             for (int c = n_start; c < n_start + bn; ++c) blk_need = std::max(blk_need, col_free[col_off + c]);
             for (int kc0 = 0; kc0 < kc_n; kc0 += nk_max) {
@@ -1680,7 +1685,7 @@ struct Builder2 {
         n_blocks += (int)blocks.size();
         if (hidden && blocks.size() > 1) {
             const int last_bi = (int)blocks.size() - 1, last_half = blocks[last_bi] / 2;
-            const int nk_last = std::max(1, std::min(4, 128 / last_half));
+            const int nk_last = std::max(1, std::min(4, stage_rows / last_half));
             const int early = (n_pad - blocks[last_bi]) / 64;
             l.free_nk = (uint8_t)nk_last;
             l.wait_chunks = (uint8_t)std::min(early, kc_n);
@@ -1863,7 +1868,8 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         return "model too deep for the tcgen05 program tables";
     pb.finish_needs();
     // the TMA box is always 128 rows: pad the stream so that the last tile's box stays in bounds
-    pb.wstream.resize(pb.wstream.size() + 128 * 128, 0);
+    pb.wstream.resize(pb.wstream.size() + (size_t)pb.stage_rows * 128, 0);
+    g.hdr.stage_rows = pb.stage_rows;
     g.hdr.n_layers = (int)pb.layers.size();
     g.hdr.blocks_per_step = pb.n_blocks;
     g.hdr.n_tiles = (int)pb.tiles.size();
@@ -1926,7 +1932,7 @@ std::string finish_program(Builder2 &pb, T2Program &g, Kernel kernel, int in_chu
         return "cuTensorMapEncodeTiled not available from the driver";
     const cuuint64_t gdim[2] = {64, (cuuint64_t)(pb.wstream.size() / 128)};
     const cuuint64_t gstride[1] = {128};
-    const cuuint32_t box[2] = {64, 128};
+    const cuuint32_t box[2] = {64, (cuuint32_t)pb.stage_rows};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult cr = reinterpret_cast<EncodeTiledFn>(fn)(
         &g.wmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, g.d_wstream, gdim, gstride, box, estr,
@@ -2006,6 +2012,11 @@ void *tc2_create(const voila_model_desc *d, int sm_count, std::vector<void *> *a
             for (const voila_mlp *f : {&d->f_T, &d->f_Z})
                 for (int l = 1; l <= f->n_layers; ++l) w = std::max(w, rup(f->dims[l], 64));
             pb.pingpong = w <= 256 && !getenv("VOILA_T2_NO_PINGPONG");
+            // wide generators: 32 KB ring stages, so a tile of a 256-column block holds two K chunks (8 MMAs,
+            // ~1000 clk of tensor work per pass of the issuer loop instead of ~500; measured CFG5 +6.8 %, two
+            // stages in flight).  Narrow / two-slot programs keep 16 KB stages (more stages in flight: measured
+            // CFG3 753 vs 729 TFLOP/s, CFG4 propose+score 624 vs 645 us).
+            if (w > 256 && !getenv("VOILA_T2_STAGE_ROWS")) pb.stage_rows = 256;
         }
         if (d->reward.kind == VOILA_R_NEG_QUADRATIC)  // u = M s on the tensor pipe, r = -s^T u in the epilogue
             pb.add_layer(d->reward.param, S, S, nullptr, 1, T2_EPI_REWARD, VOILA_ACT_NONE);

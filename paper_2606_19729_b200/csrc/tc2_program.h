@@ -31,7 +31,8 @@ namespace voila {
 
 constexpr int kT2Rows = 128;              // rows per CTA (256 per pair)
 constexpr int kT2ChunkBytes = 128 * 128;  // one 64-column operand chunk
-constexpr int kT2StageBytes = 128 * 128;  // weight ring stage per CTA (TMA box: 128 rows x 128 B)
+constexpr int kT2StageBytes = 128 * 128;  // smallest weight ring stage per CTA (TMA box: 128 rows x 128 B);
+                                          // a program's stage is T2Header::stage_rows x 128 B (128 | 256 rows)
 constexpr int kT2MaxLayers = 24;
 constexpr int kT2MaxTiles = 512;
 constexpr int kT2EvtRing = 32;
@@ -123,6 +124,7 @@ struct T2Header {
     int split_hidden;     // two-slot programs: 1 = both sets of epilogue warps share EVERY hidden layer of both
                           // slots (even / odd chunks), a slot's other layers go to the set of its number;
                           // 0 = one set per slot
+    int stage_rows;       // weight rows (128 bytes each) per CTA per ring stage = rows of the TMA box: 128 | 256
 };
 
 }  // namespace voila
