@@ -1309,6 +1309,8 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
             const uint32_t a_desc_lo = (uint32_t)umma_desc_sw128(a_u32), ring_desc_lo = (uint32_t)umma_desc_sw128(ring_u32);
             const uint32_t desc_hi = (uint32_t)(umma_desc_sw128(0u) >> 32);
             const uint32_t stage_b16 = (uint32_t)p.hdr.stage_rows * 8u;  // stage bytes / 16 (descriptor units)
+            uint32_t b_stage = ring_desc_lo;  // descriptor low word of the current ring stage (kept running: a
+                                              // multiply here sat between the weight wait and the first MMA)
             int base = p.hdr.init_events, blk_base = 0;
             uint32_t free_seq = 0;
             uint64_t *cfree = layer_done + kT2AccRing;
@@ -1364,7 +1366,7 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                     // offsets to the low word instead of rebuilding them (the rebuilt form was ~100
                     // uniform-datapath instructions per tile)
                     uint32_t a_lo = a_desc_lo + r0.z;
-                    uint32_t b_lo = ring_desc_lo + stage * stage_b16;
+                    uint32_t b_lo = b_stage;
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {  // a stage holds up to 4 K chunks
                         if (c >= (int)nk) break;
@@ -1392,9 +1394,11 @@ __device__ __forceinline__ void tc2_body(const T2Params &p, const CUtensorMap &w
                     __syncwarp();
                     T2_TL_ISSUER(tl_on, (2u << 24) | (uint32_t)i);
                     free_seq += (misc >> 6) & 1u;
+                    b_stage += stage_b16;
                     if (++stage == (uint32_t)n_stages) {
                         stage = 0;
                         phase ^= 1u;
+                        b_stage = ring_desc_lo;
                     }
                 }
                 base += p.hdr.evt_per_step;
