@@ -23,21 +23,24 @@ constexpr int kWarps = kThreads / 32;
 // y[j][r] = act(sum_k Wt[k][j] x[k][r] + b[j]) for the tile's R rows.
 // Rows k in [skip_lo, skip_hi) of the input are skipped (the one-hot block) and row a_row of Wt is
 // added in their place (a_row < 0: nothing added).
-template <bool EMU>
-__device__ __forceinline__ void mlp_layer(const float *__restrict__ Wt, const float *__restrict__ bias,
-                                          int K, int N, int act, bool last, const float *xin,
-                                          float *xout, int skip_lo, int skip_hi, int a_row) {
-    for (int item = threadIdx.x; item < 2 * N; item += kThreads) {
-        const int half = item / N, j = item - half * N;
-        float acc[16];
+// RPT rows per thread: 16 (two threads per neuron) for wide layers; 8 (four threads per neuron) when a
+// layer has fewer than kThreads / 2 neurons (config 1's 64-wide layers left half the CTA idle).
+template <bool EMU, int RPT>
+__device__ __forceinline__ void mlp_layer_rpt(const float *__restrict__ Wt, const float *__restrict__ bias,
+                                              int K, int N, int act, bool last, const float *xin,
+                                              float *xout, int skip_lo, int skip_hi, int a_row) {
+    constexpr int kParts = R / RPT;
+    for (int item = threadIdx.x; item < kParts * N; item += kThreads) {
+        const int part = item / N, j = item - part * N;
+        float acc[RPT];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) acc[i] = 0.0f;
-        const float *xp = xin + 16 * half;
+        for (int i = 0; i < RPT; ++i) acc[i] = 0.0f;
+        const float *xp = xin + RPT * part;
         auto fma_row = [&](int k) {
             const float w = __ldg(Wt + (size_t)k * N + j);
             const float4 *x4 = reinterpret_cast<const float4 *>(xp + k * R);
 #pragma unroll
-            for (int v = 0; v < 4; ++v) {
+            for (int v = 0; v < RPT / 4; ++v) {
                 const float4 x = x4[v];
                 acc[4 * v + 0] = fmaf(w, x.x, acc[4 * v + 0]);
                 acc[4 * v + 1] = fmaf(w, x.y, acc[4 * v + 1]);
@@ -51,14 +54,14 @@ __device__ __forceinline__ void mlp_layer(const float *__restrict__ Wt, const fl
         if (a_row >= 0) {
             const float w = __ldg(Wt + (size_t)a_row * N + j);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) acc[i] += w;
+            for (int i = 0; i < RPT; ++i) acc[i] += w;
         }
 #pragma unroll 4
         for (int k = skip_hi; k < K; ++k) fma_row(k);
         const float bj = __ldg(bias + j);
-        float4 *o4 = reinterpret_cast<float4 *>(xout + j * R + 16 * half);
+        float4 *o4 = reinterpret_cast<float4 *>(xout + j * R + RPT * part);
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
+        for (int v = 0; v < RPT / 4; ++v) {
             float y[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
@@ -72,6 +75,14 @@ __device__ __forceinline__ void mlp_layer(const float *__restrict__ Wt, const fl
             o4[v] = make_float4(y[0], y[1], y[2], y[3]);
         }
     }
+}
+template <bool EMU>
+__device__ __forceinline__ void mlp_layer(const float *__restrict__ Wt, const float *__restrict__ bias,
+                                          int K, int N, int act, bool last, const float *xin,
+                                          float *xout, int skip_lo, int skip_hi, int a_row) {
+    // (same sums in the same order either way: a row's accumulation never crosses threads)
+    if (2 * N < kThreads) mlp_layer_rpt<EMU, 8>(Wt, bias, K, N, act, last, xin, xout, skip_lo, skip_hi, a_row);
+    else mlp_layer_rpt<EMU, 16>(Wt, bias, K, N, act, last, xin, xout, skip_lo, skip_hi, a_row);
 }
 
 // Input in bufA ([dims[0]][R]); hidden activations ping-pong bufB/bufA; the last layer writes out.
