@@ -40,7 +40,9 @@
  *   - Tuning knobs read once by voila_create from the environment (A/B measurements only; the defaults are
  *     what the tests and bench.py run): VOILA_T2_BLOCK_POLICY (0..4: accumulator block shapes of the
  *     tcgen05 pair kernels), VOILA_T2_ROLLOUT_WARPS (8 | 16 epilogue warps of the rollout kernel),
- *     VOILA_T2_STAGES (2..8 weight-ring stages), VOILA_T2_BELIEF_1SLOT (disable the two-slot programs),
+ *     VOILA_T2_STAGES (2..8 weight-ring stages), VOILA_T2_STAGE_ROWS (128 | 256: 16 KB | 32 KB ring stages
+ *     for every program), VOILA_T2_BELIEF_1SLOT / VOILA_T2_ROLLOUT_1SLOT (disable the two-slot belief /
+ *     rollout programs), VOILA_T2_NO_PINGPONG (narrow one-slot rollouts: one TMEM accumulator region),
  *     VOILA_T2_DUAL_SPLIT (both epilogue sets share every hidden layer of a two-slot program).
  */
 #ifndef VOILA_H_
