@@ -18,17 +18,19 @@ def _cfg(S, O, A, Nz, hidden, tower_hidden, tower_d):
                                tower_hidden=tower_hidden, tower_d=tower_d)
 
 
-@pytest.mark.parametrize("S,O,A,Nz,hidden,reward", [
-    (39, 36, 6, 12, [200, 200, 200], synth.R_NEG_QUADRATIC),   # LeggedNavigation-sized state, lidar-sized observation
-    (45, 36, 6, 5, [200, 136], synth.R_NEG_L2_GOAL),           # TargetFinding-sized state, odd noise width
+@pytest.mark.parametrize("S,O,A,Nz,hidden,reward,P,Q", [
+    (39, 36, 6, 12, [200, 200, 200], synth.R_NEG_QUADRATIC, 700, 10),   # LeggedNavigation-sized state, lidar-sized observation
+    (45, 36, 6, 5, [200, 136], synth.R_NEG_L2_GOAL, 700, 10),           # TargetFinding-sized state, odd noise width
+    (39, 36, 6, 12, [200, 200, 200], synth.R_NEG_QUADRATIC, 1000, 40),  # four blocks x 40 sequences: the two-slot rollout
+    (45, 36, 6, 5, [200, 136], synth.R_NEG_L2_GOAL, 400, 80),           # two blocks (the second ragged) x 80 sequences
 ])
-def test_paper_shaped_rollout_and_belief_update(oracle, S, O, A, Nz, hidden, reward):
+def test_paper_shaped_rollout_and_belief_update(oracle, S, O, A, Nz, hidden, reward, P, Q):
     import torch
     import paper_2606_19729_b200 as vl
     assert torch.cuda.is_available()
     cfg = dataclasses.replace(_cfg(S, O, A, Nz, hidden, [200], 100), reward_kind=reward)
     model = synth.make_model(cfg, action_cost=True)
-    P, Q, H, N = 700, 10, 7, 1500
+    H, N = 7, 1500
     inp = synth.make_inputs(cfg, P=P, Q=Q, H=H, N=N)
     ctx = vl.Voila(model, device=0)
     out = ctx.voila_rollout_values(ctx.to_particles(inp.particles), torch.from_numpy(inp.action_seqs).cuda(), None, 77,
@@ -38,6 +40,8 @@ def test_paper_shaped_rollout_and_belief_update(oracle, S, O, A, Nz, hidden, rew
                                  torch.from_numpy(w).cuda(), 78)
     torch.cuda.synchronize()
     assert "rollout_tc2" in ctx.voila_last_rollout_kernel(), ctx.voila_last_rollout_kernel()
+    if Q >= 40:
+        assert "rollout_tc2d" in ctx.voila_last_rollout_kernel(), ctx.voila_last_rollout_kernel()
     assert "belief_tc2" in ctx.voila_last_belief_kernel(), ctx.voila_last_belief_kernel()
     om = oracle.OracleModel(model)
     parts = synth.bf16_round_np(inp.particles)

@@ -156,7 +156,7 @@ def test_bf16_mode_within_north_star(torch_cuda, oracle, kernel_name, cfg_idx, P
 
 
 @pytest.mark.parametrize("cfg_idx,P,Q,H,weighted", [(2, 300, 80, 6, False), (3, 1000, 40, 4, True),
-                                                    (3, 512, 75, 3, False)])
+                                                    (3, 512, 75, 3, False), (2, 512, 150, 1, True)])
 def test_bf16_two_slot_rollout(torch_cuda, oracle, cfg_idx, P, Q, H, weighted):
     """Generators <= 256 wide, an even number of 256-particle blocks per sequence and more pairs of
     blocks than CTA pairs: AUTO runs the two-slot kernel (two blocks of one sequence in flight per CTA
