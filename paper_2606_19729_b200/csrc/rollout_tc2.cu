@@ -239,6 +239,7 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
     const int chunks = l.n_pad >> 6;
     const int wait_chunks = l.wait_chunks, free_nk = l.free_nk;
     const uint32_t blk_mask = l.blk_mask;
+    const bool one_event = l.one_event != 0;  // one event for the whole layer (T2Layer::one_event)
     int free_have = 0;
     // accumulator blocks are handed over one by one: a chunk may be loaded once the block it
     // belongs to has been committed (blk_mask: chunks that start a block)
@@ -265,9 +266,11 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
         const bool next_blk = (j + 1 < chunks) && ((blk_mask >> (j + 1)) & 1u);
         if (j + 1 < chunks && !next_blk) tmem_ld16(ec.taddr0 + (uint32_t)(64 * (j + 1)), va);
         hidden_store16<ACT>(vb, bj + 64u, row_addr, ec.sw[2], ec.sw[3]);
-        fence_proxy_async_smem();
-        tc_fence_before();
-        es.arrive_event();
+        if (!one_event || j + 1 == chunks) {
+            fence_proxy_async_smem();
+            tc_fence_before();
+            es.arrive_event();
+        }
         T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | (uint32_t)j);
         if (next_blk) {
             es.wait_layer();
@@ -560,7 +563,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params &p, const T2Layer *L,
                 es.tl_layer = (uint32_t)li;
                 if (my_slot >= 0 && (int)l.slot != my_slot) {  // the other set's record: sequence numbers only
                     const bool hid = l.epi == T2_EPI_HIDDEN;
-                    es.ev += hid ? (int)(l.n_pad >> 6) : 1;
+                    es.ev += (hid && !l.one_event) ? (int)(l.n_pad >> 6) : 1;
                     es.ld_seq += hid ? (uint32_t)__popc((unsigned)l.blk_mask) : 1u;
                     if (hid && l.wait_chunks > 0) es.free_seq += ((uint32_t)l.wait_chunks + l.free_nk - 1u) / l.free_nk;
                     continue;
@@ -929,7 +932,7 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
             }
             if (my_slot >= 0 && slot != my_slot) {  // the other set's record: sequence numbers only
                 const bool hid = l.epi == T2_EPI_HIDDEN;
-                es.ev += hid ? (int)(l.n_pad >> 6) : 1;
+                es.ev += (hid && !l.one_event) ? (int)(l.n_pad >> 6) : 1;
                 es.ld_seq += hid ? (uint32_t)__popc((unsigned)l.blk_mask) : 1u;
                 if (hid && l.wait_chunks > 0) es.free_seq += ((uint32_t)l.wait_chunks + l.free_nk - 1u) / l.free_nk;
                 continue;
@@ -1564,6 +1567,10 @@ struct Builder2 {
         dual = true;
         slot_chunks = chunks_per_slot;
         dual_cols = cols_per_slot;
+        // two-slot programs: one 256-column accumulator block per layer (one hand-off, no in-place
+        // chunk-free waits; the OTHER slot's MMAs overlap this slot's epilogue): measured CFG3 750 -> 759
+        // TFLOP/s, CFG4 propose+score 630 -> 616 us against two 128-column blocks
+        if (policy == 0) policy = 3;
         // slot 0's input / accumulator were last touched by the event BEFORE the previous step's last
         for (int j = 0; j < chunks_per_slot; ++j) a_ready[j] = -2;
         for (int c = 0; c < cols_per_slot; ++c) col_free[c] = -2;
@@ -1706,8 +1713,14 @@ struct Builder2 {
             if (n_sig > kT2FreeRing) bad_order = true;
         }
         tiles.insert(tiles.end(), lt.begin(), lt.end());
+        l.one_event = (hidden && dual && !par_split && blocks.size() == 1) ? 1 : 0;
         layers.push_back(l);
-        if (hidden) {
+        if (hidden && l.one_event) {
+            for (int c = 0; c < n_pad; ++c) col_free[col_off + c] = evt;
+            for (int j = 0; j < n_pad / 64; ++j) a_ready[chunk_off + j] = evt;
+            evt_set.push_back(0);
+            ++evt;
+        } else if (hidden) {
             for (int j = 0; j < n_pad / 64; ++j) {
                 for (int c = 64 * j; c < 64 * j + 64; ++c) col_free[col_off + c] = evt;
                 a_ready[chunk_off + j] = evt;

@@ -71,8 +71,13 @@ struct T2Layer {  // what the epilogue needs to know about a layer
     uint8_t slot;        // 0 | 1
     uint8_t chunk_off;   // first operand chunk of the slot
     uint16_t col_off;    // first TMEM column of the slot
+    // Hidden layer of a two-slot program with ONE accumulator block: every tile of the next layer waits for
+    // the layer's last chunk anyway (the block must be drained), so the epilogue publishes one event for
+    // the whole layer instead of one per 64-column chunk (a proxy fence + a cluster arrive each).
+    uint8_t one_event;
+    uint8_t pad[3];
 };
-static_assert(sizeof(T2Layer) == 20, "T2Layer is copied to shared memory as 32-bit words");
+static_assert(sizeof(T2Layer) == 24, "T2Layer is copied to shared memory as 32-bit words");
 
 struct T2Tile {  // one weight-ring stage: nk K-chunks of one accumulator block (20 bytes)
     uint32_t src_row;  // first 128-byte row of the tile in the weight stream (CTA r: + r * rows)
