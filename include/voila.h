@@ -65,7 +65,7 @@ typedef enum {
     VOILA_ERR_INVALID_ARG = 1, /* NULL / non-positive size / action out of range / misaligned pointer */
     VOILA_ERR_UNSUPPORTED = 2, /* no sm_100 device, or model dims over the kernels' limits */
     VOILA_ERR_CUDA = 3,        /* a CUDA runtime call failed; see voila_last_cuda_error */
-    VOILA_ERR_WORKSPACE = 4    /* sizes exceed what voila_reserve was given */
+    VOILA_ERR_WORKSPACE = 4    /* sizes exceed what voila_reserve was given (or VOILA_STATIC_MAX_N) */
 } voila_status;
 
 typedef enum { VOILA_ACT_NONE = 0, VOILA_ACT_RELU = 1, VOILA_ACT_SILU = 2 } voila_act;
@@ -214,6 +214,24 @@ voila_status voila_belief_update(voila_ctx *ctx, const void *particles, int N, i
 voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, uint64_t seed,
                                        int32_t *ancestors_out, int32_t *dev_status_out,
                                        void *cuda_stream);
+
+/* The same resampler for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no ctx, no workspace, NO cudaMalloc / cudaFree or allocating
+ * library call inside; three kernel launches on `cuda_stream` of the CURRENT device.  Its scratch (the
+ * uint64 CDF, the look-back tile records, the scan bookkeeping) is one static device array of
+ * 8 MiB + 16 KiB that every GPU loading libvoila holds until exit, hence the limit
+ * N <= VOILA_STATIC_MAX_N (2^20).  Arguments and results exactly as voila_resample_systematic
+ * (v, ancestors_out, dev_status_out are device pointers, 16-byte aligned; dev_status_out may be NULL).
+ * All calls share that one array: calls that may overlap on the GPU (different streams, different host
+ * threads) race on it -- issue them on one stream, or order them with events.  The array keeps the last
+ * call's contents; every call clears what must start at zero itself.
+ * Errors: VOILA_ERR_INVALID_ARG for NULL / N < 1 / misaligned pointers; VOILA_ERR_WORKSPACE for
+ * N > VOILA_STATIC_MAX_N (nothing is launched); VOILA_ERR_CUDA when a runtime call fails.
+ * voila_static_last_error() returns the calling thread's last message of this entry point ("" if none). */
+#define VOILA_STATIC_MAX_N (1 << 20)
+voila_status voila_resample_systematic_static(const float *v, int N, uint64_t seed, int32_t *ancestors_out,
+                                              int32_t *dev_status_out, void *cuda_stream);
+const char *voila_static_last_error(void);
 
 /* y = MLP_which(x): which = 0 f_T, 1 f_Z, 2 f (obs tower), 3 g (state tower).
  * x dev [rows][dims[0]] fp32 (the full input, one-hot block included), y dev [rows][dims[L]] fp32.

@@ -13,6 +13,8 @@
 //                  then coalesced vectorised row gathers.
 // HBM-bound; no tensor-core work here.
 #include "voila_device.cuh"
+#include <atomic>
+
 #include "voila_kernels.h"
 
 namespace voila {
@@ -572,6 +574,90 @@ cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *pro
     else
         resample_gather_kernel<2><<<grid, 256, 0, st>>>(sb, N, src, row_bytes, dst, weights_out, ancestors_out, w_in, from_logits ? 1 : 0);
     return cudaGetLastError();
+}
+
+// =====================================================================================
+// voila_resample_systematic_static: the stage-level resampler for callers that may not allocate
+// (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Same three kernels as
+// voila_resample_systematic; the scratch they need (the uint64 CDF, the look-back tile records, the
+// scan bookkeeping) lives in ONE file-scope device array of a fixed size instead of the ctx
+// workspace: 8 MiB + 16 KiB that every GPU loading the library holds until exit, good for
+// N <= kStaticMaxN = 2^20 particles (VOILA_STATIC_MAX_N in voila.h).
+// In host code `g_static_scratch` is a host-side stand-in for the symbol, not a device address:
+// the address the kernels get comes from cudaGetSymbolAddress, once per device, with that device
+// current.  Every call shares the array: calls that overlap on the GPU (two streams, two host
+// threads) race on it; bu_init_kernel clears what has to start at zero (tile flags, ScanState,
+// the running maximum) at the head of every call, the rest is overwritten before it is read.
+// =====================================================================================
+namespace {
+
+constexpr int kStaticMaxN = 1 << 20;
+constexpr int kStaticTiles = kStaticMaxN / kScanTile;
+static_assert(kStaticMaxN % kScanTile == 0, "whole tiles");
+// layout in 8-byte words, every part 256-byte aligned
+constexpr size_t kStOffCdf = 0;                                      // [kStaticMaxN] uint64
+constexpr size_t kStOffAgg = kStOffCdf + (size_t)kStaticMaxN;        // [tiles] uint64
+constexpr size_t kStOffIncl = kStOffAgg + kStaticTiles;              // [tiles] uint64
+constexpr size_t kStOffSumv = kStOffIncl + kStaticTiles;             // [2 * tiles] double
+constexpr size_t kStOffFlag = kStOffSumv + 2 * kStaticTiles;         // [tiles] uint32
+constexpr size_t kStOffState = kStOffFlag + kStaticTiles / 2;        // ScanState (<= 32 words)
+constexpr size_t kStOffMax = kStOffState + 32;                       // [1] int   (32 words)
+constexpr size_t kStOffWsum = kStOffMax + 32;                        // [1] double (32 words, unused by this path)
+constexpr size_t kStaticWords = kStOffWsum + 32;
+static_assert(sizeof(ScanState) <= 32 * 8, "ScanState fits its slot");
+static_assert(kStaticTiles % 64 == 0 && (kStOffAgg % 32) == 0 && (kStOffState % 32) == 0, "256-byte aligned parts");
+
+static __device__ __align__(256) unsigned long long g_static_scratch[kStaticWords];
+
+constexpr int kStaticMaxDevices = 64;
+std::atomic<unsigned long long *> g_static_addr[kStaticMaxDevices];  // device address of the array, per device
+
+}  // namespace
+
+int static_resample_max_n() { return kStaticMaxN; }
+size_t static_scratch_bytes() { return kStaticWords * sizeof(unsigned long long); }
+
+// Runs on the CURRENT device.  No cudaMalloc / cudaFree, no allocating library call; three launches.
+cudaError_t launch_resample_systematic_static(const float *v, int N, uint64_t seed, int32_t *ancestors_out,
+                                              int32_t *dev_status_out, cudaStream_t st, const char **why) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) {
+        if (why) *why = "device ordinal beyond the static scratch table (64 devices)";
+        return cudaErrorInvalidDevice;
+    }
+    unsigned long long *base = g_static_addr[dev].load(std::memory_order_acquire);
+    if (!base) {
+        // set-up, once per device, with that device current (two threads racing here store the same value)
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess) {
+            if (why) *why = "cudaGetSymbolAddress(g_static_scratch) failed";
+            return e;
+        }
+        base = reinterpret_cast<unsigned long long *>(ptr);
+        g_static_addr[dev].store(base, std::memory_order_release);
+    }
+    ScanBuffers sb;
+    sb.cdf = base + kStOffCdf;
+    sb.tile_agg = base + kStOffAgg;
+    sb.tile_incl = base + kStOffIncl;
+    sb.tile_sumv = reinterpret_cast<double *>(base + kStOffSumv);
+    sb.tile_flag = reinterpret_cast<unsigned int *>(base + kStOffFlag);
+    sb.state = reinterpret_cast<ScanState *>(base + kStOffState);
+    sb.max_ordered = reinterpret_cast<int *>(base + kStOffMax);
+    sb.part_wsum = reinterpret_cast<double *>(base + kStOffWsum);
+    e = launch_bu_init(sb, N, st);  // clears the tile flags, ScanState and the running maximum of the last call
+    if (e != cudaSuccess) return e;
+    FinalizeArgs fin{};
+    fin.enabled = 1;
+    fin.seed = seed;
+    fin.ess_threshold = INFINITY;
+    fin.dev_status_out = dev_status_out;
+    e = launch_weight_scan(sb, v, N, false, nullptr, st, &fin);
+    if (e != cudaSuccess) return e;
+    return launch_resample_gather(sb, N, nullptr, 16, nullptr, nullptr, ancestors_out, st, v, false);
 }
 
 }  // namespace voila

@@ -606,6 +606,43 @@ voila_status voila_resample_systematic(voila_ctx *ctx, const float *v, int N, ui
     return run_resample(ctx, sb, N, nullptr, nullptr, nullptr, ancestors_out, st, v, false);
 }
 
+// ---- the no-allocation resampler (scratch: a static device array in belief.cu) ----
+namespace {
+thread_local char g_static_err[160] = "";
+void static_err(const char *fmt, long a = 0, long b = 0) { snprintf(g_static_err, sizeof(g_static_err), fmt, a, b); }
+}  // namespace
+
+const char *voila_static_last_error(void) { return g_static_err; }
+
+voila_status voila_resample_systematic_static(const float *v, int N, uint64_t seed, int32_t *ancestors_out,
+                                              int32_t *dev_status_out, void *cuda_stream) {
+    g_static_err[0] = 0;
+    if (!v || !ancestors_out || N < 1) {
+        static_err("voila_resample_systematic_static: NULL pointer or N < 1 (N = %ld)", (long)N);
+        return VOILA_ERR_INVALID_ARG;
+    }
+    if (misaligned(v) || misaligned(ancestors_out)) {
+        static_err("voila_resample_systematic_static: v and ancestors_out must be 16-byte aligned");
+        return VOILA_ERR_INVALID_ARG;
+    }
+    if (N > static_resample_max_n()) {
+        static_err("voila_resample_systematic_static: N = %ld exceeds VOILA_STATIC_MAX_N = %ld (the static scratch "
+                   "array); use voila_resample_systematic with a reserved workspace", (long)N,
+                   (long)static_resample_max_n());
+        return VOILA_ERR_WORKSPACE;
+    }
+    const char *why = nullptr;
+    const cudaError_t e = launch_resample_systematic_static(v, N, seed, ancestors_out, dev_status_out,
+                                                            reinterpret_cast<cudaStream_t>(cuda_stream), &why);
+    if (e != cudaSuccess) {
+        snprintf(g_static_err, sizeof(g_static_err), "voila_resample_systematic_static: %s%s%s",
+                 why ? why : "", why ? ": " : "", cudaGetErrorString(e));
+        cudaGetLastError();
+        return VOILA_ERR_CUDA;
+    }
+    return VOILA_OK;
+}
+
 // ---- progressive widening ----
 namespace {
 struct PwLayout {

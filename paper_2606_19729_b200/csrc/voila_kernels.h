@@ -57,6 +57,12 @@ cudaError_t launch_resample_gather(const ScanBuffers &sb, int N, const void *pro
                                    int32_t *ancestors_out, cudaStream_t st, const float *w_in,
                                    bool from_logits);
 
+// voila_resample_systematic_static: scratch in a file-scope device array of belief.cu (no allocation)
+int static_resample_max_n();
+size_t static_scratch_bytes();
+cudaError_t launch_resample_systematic_static(const float *v, int N, uint64_t seed, int32_t *ancestors_out,
+                                              int32_t *dev_status_out, cudaStream_t st, const char **why);
+
 // ---- pw.cu / mlp_ffma.cu : vectorised progressive widening with batched likelihood (voila_pw_update) ----
 cudaError_t launch_pw_widen(const PwArgs &a, cudaStream_t st);          // widen + child offsets + sorted order (3 launches)
 cudaError_t launch_pw_propose_ffma(const ModelDev &m, const PwArgs &a, bool bf16, cudaStream_t st);

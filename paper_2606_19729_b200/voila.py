@@ -28,11 +28,36 @@ EXPORTS = [
     "voila_status_string", "voila_last_cuda_error", "voila_version", "voila_set_profiling",
     "voila_profile_read", "voila_pw_workspace_bytes", "voila_pw_reserve", "voila_pw_update",
     "voila_porpp_backup", "voila_diffusion_sample", "voila_plan_host",
+    "voila_resample_systematic_static", "voila_static_last_error",
 ]
 
 
 class VoilaError(RuntimeError):
     pass
+
+
+STATIC_MAX_N = 1 << 20  # VOILA_STATIC_MAX_N
+
+
+def voila_resample_systematic_static(v, seed, ancestors_out, status_out=None, stream=None):
+    """voila_resample_systematic_static (include/voila.h): the resampler that allocates nothing.  The
+    caller passes the outputs too (ancestors_out [N] int32, status_out [1] int32 or None); scratch is
+    the library's static device array, shared by every call: do not overlap calls on the GPU."""
+    import torch
+    lib = load_library()
+    N = v.numel()
+    assert v.dtype == torch.float32 and v.is_contiguous() and v.is_cuda
+    assert ancestors_out.dtype == torch.int32 and ancestors_out.is_contiguous() and ancestors_out.numel() >= N
+    assert status_out is None or (status_out.dtype == torch.int32 and status_out.numel() >= 1)
+    st = torch.cuda.current_stream(v.device).cuda_stream if stream is None else stream
+    with torch.cuda.device(v.device):
+        rc = lib.voila_resample_systematic_static(_dptr(v), N, C.c_uint64(int(seed)), _dptr(ancestors_out),
+                                                  _dptr(status_out) if status_out is not None else None,
+                                                  C.c_void_p(st))
+    if rc != 0:
+        raise VoilaError(f"voila_resample_systematic_static: status {rc}: "
+                         f"{lib.voila_static_last_error().decode()}")
+    return ancestors_out
 
 
 class _Mlp(C.Structure):
@@ -100,6 +125,10 @@ def load_library():
     lib.voila_belief_update_ess.restype = i32
     lib.voila_resample_systematic.argtypes = [vp, vp, i32, u64, vp, vp, vp]
     lib.voila_resample_systematic.restype = i32
+    lib.voila_resample_systematic_static.argtypes = [vp, i32, u64, vp, vp, vp]
+    lib.voila_resample_systematic_static.restype = i32
+    lib.voila_static_last_error.argtypes = []
+    lib.voila_static_last_error.restype = C.c_char_p
     lib.voila_mlp_forward.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.voila_mlp_forward.restype = i32
     lib.voila_best_action.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
