@@ -278,8 +278,45 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
         }
     }
 }
+// The same for a layer that is ONE accumulator block (every hidden layer of a two-slot program, narrow
+// layers elsewhere): no block hand-offs inside the layer and no in-place chunk-free waits, so the chunk
+// loop carries no bookkeeping at all (the general loop spends more instructions on control than on math).
+template <int ACT>
+__device__ __forceinline__ void epi_hidden_loop_1blk(EpiSync &es, const T2Layer &l, uint32_t bias_u32, const EpiConst &ec) {
+    uint32_t va[16], vb[16];
+    const int chunks = l.n_pad >> 6;
+    const bool one_event = l.one_event != 0;
+    es.wait_layer();
+    tmem_ld16(ec.taddr0, va);
+    uint32_t row_addr = ec.st_base, bj = bias_u32, ta = ec.taddr0;
+#pragma unroll 1
+    for (int j = chunks; j > 0; --j) {
+        tmem_ld_wait();
+        tmem_ld16(ta + 16u, vb);
+        T2_TL(es.tl_on, (es.tl_kind << 24) | (es.tl_layer << 8) | (uint32_t)(chunks - j));
+        hidden_store16<ACT>(va, bj, row_addr, ec.sw[0], ec.sw[1]);
+        tmem_ld_wait();
+        ta += 64u;
+        if (j > 1) tmem_ld16(ta, va);
+        hidden_store16<ACT>(vb, bj + 64u, row_addr, ec.sw[2], ec.sw[3]);
+        if (!one_event || j == 1) {
+            fence_proxy_async_smem();
+            tc_fence_before();
+            es.arrive_event();
+        }
+        T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | (uint32_t)(chunks - j));
+        row_addr += kT2ChunkBytes;
+        bj += 256u;
+    }
+}
 __device__ __forceinline__ void epi_hidden_layer(EpiSync &es, const T2Layer &l, int bias_float_off, const EpiConst &ec) {
     const uint32_t bias_u32 = ec.sbias_u32 + 4u * (uint32_t)bias_float_off;
+    if (l.blk_mask == 1u && l.wait_chunks == 0) {
+        if (l.act == VOILA_ACT_SILU) epi_hidden_loop_1blk<VOILA_ACT_SILU>(es, l, bias_u32, ec);
+        else if (l.act == VOILA_ACT_RELU) epi_hidden_loop_1blk<VOILA_ACT_RELU>(es, l, bias_u32, ec);
+        else epi_hidden_loop_1blk<VOILA_ACT_NONE>(es, l, bias_u32, ec);
+        return;
+    }
     if (l.act == VOILA_ACT_SILU) epi_hidden_loop<VOILA_ACT_SILU>(es, l, bias_u32, ec);
     else if (l.act == VOILA_ACT_RELU) epi_hidden_loop<VOILA_ACT_RELU>(es, l, bias_u32, ec);
     else epi_hidden_loop<VOILA_ACT_NONE>(es, l, bias_u32, ec);

@@ -52,3 +52,42 @@ def test_tensor_core_and_cuda_core_kernels_agree(cfg_idx):
         assert _rel_l2(res["tc"][1]["proposals"].float(), res["ffma"][1]["proposals"].float()) <= 5e-3, what
         assert float((res["tc"][1]["post_weights"] - res["ffma"][1]["post_weights"]).abs().max()) <= 2e-2, what
     ctx.close()
+
+
+@pytest.mark.parametrize("cfg_idx", [2, 3, 4])
+def test_two_slot_rollout_and_cuda_core_kernels_agree(cfg_idx):
+    """The two-slot rollout kernel (rollout_tc2d_kernel: two 256-particle blocks of a sequence in flight
+    per CTA pair) against the CUDA-core bf16 kernel on random shapes that select it: an even number of
+    256-particle blocks (the last one ragged), more pairs of blocks than CTA pairs, several units per
+    CTA pair, with and without prior weights."""
+    import torch
+    import paper_2606_19729_b200 as vl
+    assert torch.cuda.is_available()
+    rng = np.random.default_rng(2000 + cfg_idx)
+    cfg = synth.CONFIGS[cfg_idx]
+    model = synth.make_model(cfg, prec=synth.PREC_BF16)
+    ctx = vl.Voila(model, device=0, prec=synth.PREC_BF16)
+    for trial in range(8):
+        pairs = int(rng.integers(1, 5))                                # pairs of 256-particle blocks per sequence
+        P = 512 * pairs - int(rng.integers(0, 256))                    # ragged last block, block count stays even
+        Q = int(rng.integers(75 // pairs + 1, 75 // pairs + 60))       # pairs * Q > 74 CTA pairs
+        H = int(rng.integers(1, 7))
+        inp = synth.make_inputs(cfg, P=P, Q=Q, H=H, N=8, seed=int(rng.integers(1 << 30)))
+        parts = ctx.to_particles(inp.particles)
+        seqs = torch.from_numpy(inp.action_seqs).cuda()
+        w = torch.from_numpy(np.exp(rng.standard_normal(P)).astype(np.float32)).cuda() if trial % 2 else None
+        seed = int(rng.integers(1 << 40))
+        res = {}
+        for name, kernel in (("tc", vl.KERNEL_AUTO), ("ffma", vl.KERNEL_FFMA)):
+            ctx.voila_set_kernel(kernel)
+            res[name] = ctx.voila_rollout_values(parts, seqs, w, seed, want_witness=True, want_returns=True,
+                                                 want_final_states=True)
+            torch.cuda.synchronize()
+            if name == "tc":
+                assert "rollout_tc2d_kernel" in ctx.voila_last_rollout_kernel(), ctx.voila_last_rollout_kernel()
+        what = f"cfg{cfg_idx} P={P} Q={Q} H={H}"
+        assert _rel_l2(res["tc"]["returns"], res["ffma"]["returns"]) <= 5e-3, what
+        assert _rel_l2(res["tc"]["witness"], res["ffma"]["witness"]) <= 5e-3, what
+        assert _rel_l2(res["tc"]["final_states"].float(), res["ffma"]["final_states"].float()) <= 5e-3, what
+        assert _rel_l2(res["tc"]["values"], res["ffma"]["values"]) <= 5e-3, what
+    ctx.close()
