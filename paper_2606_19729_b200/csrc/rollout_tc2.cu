@@ -237,7 +237,8 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
     // through bias / activation / pack / store (32 live accumulator registers instead of 64)
     uint32_t va[16], vb[16];
     const int chunks = l.n_pad >> 6;
-    const int wait_chunks = l.wait_chunks, free_nk = l.free_nk;
+    const int wait_chunks = l.wait_chunks;
+    const int free_sh = 31 - __clz((int)l.free_nk);  // free_nk is 1, 2 or 4: a shift, not a division, per chunk
     const uint32_t blk_mask = l.blk_mask;
     const bool one_event = l.one_event != 0;  // one event for the whole layer (T2Layer::one_event)
     int free_have = 0;
@@ -251,7 +252,7 @@ __device__ __forceinline__ void epi_hidden_loop(EpiSync &es, const T2Layer &l, u
         tmem_ld_wait();
         tmem_ld16(ec.taddr0 + (uint32_t)(64 * j + 16), vb);
         if (j < wait_chunks) {  // in-place store: the last block must have read chunk j
-            const int need_free = j / free_nk + 1;
+            const int need_free = (j >> free_sh) + 1;
             while (free_have < need_free) {
                 es.wait_chunk_free();
                 ++free_have;
@@ -331,16 +332,16 @@ __device__ __forceinline__ void epi_hidden_loop_par(EpiSync &es, const T2Layer &
                                                     int parity) {
     uint32_t va[16], vb[16];
     const int chunks = l.n_pad >> 6;
-    const int wait_chunks = l.wait_chunks, free_nk = l.free_nk;
+    const int wait_chunks = l.wait_chunks;
+    const int free_sh = 31 - __clz((int)l.free_nk);  // free_nk is 1, 2 or 4 (K chunks per ring stage)
     const uint32_t blk_mask = l.blk_mask;
     const int n_blocks = __popc(blk_mask);
-    const int n_sig = wait_chunks > 0 ? (wait_chunks + free_nk - 1) / free_nk : 0;
+    const int n_sig = wait_chunks > 0 ? ((wait_chunks - 1) >> free_sh) + 1 : 0;
     int free_have = 0, blocks_waited = 0;
-    for (int j = 0; j < chunks; ++j) {
-        if ((j & 1) != parity) {
-            ++es.ev;
-            continue;
-        }
+    // this set's chunks: parity, parity + 2, ... (prefetching the next chunk's first columns across the
+    // event was tried: spills in the 56-register helper warps)
+    es.ev += parity;
+    for (int j = parity; j < chunks; j += 2) {
         // blocks that start at a chunk <= j must have been handed over
         const int need_blocks = __popc(blk_mask & ((2u << j) - 1u));
         while (blocks_waited < need_blocks) {
@@ -353,7 +354,7 @@ __device__ __forceinline__ void epi_hidden_loop_par(EpiSync &es, const T2Layer &
         tmem_ld_wait();
         tmem_ld16(ec.taddr0 + (uint32_t)(64 * j + 16), vb);
         if (j < wait_chunks) {  // in-place store: the last block must have read chunk j
-            const int need_free = j / free_nk + 1;
+            const int need_free = (j >> free_sh) + 1;
             while (free_have < need_free) {
                 es.wait_chunk_free();
                 ++free_have;
@@ -368,7 +369,10 @@ __device__ __forceinline__ void epi_hidden_loop_par(EpiSync &es, const T2Layer &
         tc_fence_before();
         es.arrive_event();
         T2_TL(es.tl_on, ((es.tl_kind + 1u) << 24) | (es.tl_layer << 8) | (uint32_t)j);
+        ++es.ev;  // the other set's chunk j + 1 (or j - 1: the count per layer is what matters)
     }
+    // (an odd number of chunks: the set without the last chunk has counted one event too many / too few)
+    es.ev += chunks - ((chunks - parity + 1) >> 1) * 2 - parity;
     es.ld_seq += (uint32_t)(n_blocks - blocks_waited);
     es.free_seq += (uint32_t)(n_sig - free_have);
 }
