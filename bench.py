@@ -666,8 +666,8 @@ def run_voila(args):
     # committed `ncu --set full` capture of this kernel at THIS size (full-size CFG5); null for any other
     # size or kernel (inputs are read once, per-(q, tile) partial sums written; the horizon loop never touches HBM)
     if cfg.index == 5 and not reduced and "rollout_tc2x" in ctx.voila_last_rollout_kernel():
-        roof["traffic"] = 5574656 + 28827648
-        roof["traffic_from"] = "profiles/r02h_rollout_tc2x_cfg5_fullsize.md (ncu --set full, the full-size launch)"
+        roof["traffic"] = 5590784 + 26686208
+        roof["traffic_from"] = "profiles/r02j_rollout_tc2x_cfg5_fullsize.md (ncu --set full, the full-size launch)"
     roof.update({"kernel": ctx.voila_last_rollout_kernel(), "kernel_ms": k_ms,
                  "flop_per_unit": flop_step, "units_per_launch": P * Q * H,
                  "share_of_step": k_ms / ms_per_step})
