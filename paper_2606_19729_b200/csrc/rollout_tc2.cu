@@ -2273,9 +2273,12 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
                                std::string *kernel_name, int *n_launches) {
     const T2Handle *h = reinterpret_cast<const T2Handle *>(tc);
     // two blocks in flight per CTA pair: when a sequence has an even number of 256-particle blocks (no
-    // idle slot) and every CTA pair gets more than one pair of blocks
+    // idle slot) or at least five, and every CTA pair gets more than one pair of blocks
     const int blocks = (a.P + 2 * kT2Rows - 1) / (2 * kT2Rows);
-    const bool dual = h->has_roll_dual && blocks % 2 == 0 && (blocks / 2) * a.Q > h->roll_dual.max_clusters;
+    // (an odd block count leaves the second slot of a sequence's last pair empty -- its rows are invalid --:
+    //  worth it from five blocks on, 1.27 x 5 / 6 against the one-block kernel)
+    const int pairs = (blocks + 1) / 2;
+    const bool dual = h->has_roll_dual && (blocks % 2 == 0 || blocks >= 5) && pairs * a.Q > h->roll_dual.max_clusters;
     const T2Program &g = dual ? h->roll_dual : h->roll;
     T2Params p = base_params(g, m);
     p.particles = reinterpret_cast<const uint16_t *>(a.particles);
@@ -2287,7 +2290,7 @@ cudaError_t launch_rollout_tc2(void *tc, const ModelDev &m, const RolloutArgs &a
     p.part_witness = a.part_witness;
     p.returns_out = a.returns_out;
     p.final_states_out = a.final_states_out;
-    p.blocks_per_q = dual ? blocks / 2 : blocks;  // work units of a CTA pair per sequence
+    p.blocks_per_q = dual ? pairs : blocks;  // work units of a CTA pair per sequence
     p.tiles_per_q = a.tiles;  // = 2 * blocks (see rollout_tile_count)
     p.n_units = p.blocks_per_q * a.Q;
     const int clusters = std::min(g.max_clusters, p.n_units);

@@ -156,10 +156,11 @@ def test_bf16_mode_within_north_star(torch_cuda, oracle, kernel_name, cfg_idx, P
 
 
 @pytest.mark.parametrize("cfg_idx,P,Q,H,weighted", [(2, 300, 80, 6, False), (3, 1000, 40, 4, True),
-                                                    (3, 512, 75, 3, False), (2, 512, 150, 1, True)])
+                                                    (3, 512, 75, 3, False), (2, 512, 150, 1, True),
+                                                    (2, 1200, 30, 3, True)])
 def test_bf16_two_slot_rollout(torch_cuda, oracle, cfg_idx, P, Q, H, weighted):
-    """Generators <= 256 wide, an even number of 256-particle blocks per sequence and more pairs of
-    blocks than CTA pairs: AUTO runs the two-slot kernel (two blocks of one sequence in flight per CTA
+    """Generators <= 256 wide, an even number of 256-particle blocks per sequence (or >= 5: P = 1200 is five
+    blocks, the last pair's second slot stays empty) and more pairs of blocks than CTA pairs: AUTO runs the two-slot kernel (two blocks of one sequence in flight per CTA
     pair, one set of stateful epilogue warps each).  Ragged last block, zero weights, every output."""
     import paper_2606_19729_b200 as vl
     cfg = synth.CONFIGS[cfg_idx]
