@@ -844,8 +844,9 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
         return ((unit * n_slots + slot) * 2 + (int)rank) * kT2Rows + row;
     };
     // f_T input [s_i ; w_i ; 0] of a row straight into the slot's operand chunks (half 0 warps)
-    auto load_input = [&](int unit_local, int slot, uint32_t a_slot) {
-        if (half != 0) return;
+    // (worker: the half of the warps that does it -- a row belongs to one thread of each half)
+    auto load_input = [&](int unit_local, int slot, uint32_t a_slot, int worker = 0) {
+        if (half != worker) return;
         const int i_idx = row_index(unit_local, slot);
         if (MODE == 4) {  // [bf16(obs)] of a stored branch
             const bool ok = i_idx < p.P && (i_idx % p.slot_M) < __ldg(p.slot_count + i_idx / p.slot_M);
@@ -1225,8 +1226,9 @@ __device__ __forceinline__ void t2_bu_epilogue(const T2Params &p, const T2Layer 
                         p.bu_part_wsum[i0 >> 5] = ws;
                     }
                 }
-                // this slot's next unit: its input goes into the slot's operand chunks with this event
-                if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot);
+                // this slot's next unit: its input goes into the slot's operand chunks with this event; the
+                // warps that had no part in the score fetch the rows and draw the noise meanwhile
+                if (step + 1 < n_my_units) load_input(step + 1, slot, a_slot, 1);
                 named_bar_sync(bar_id, 256);
                 fence_proxy_async_smem();
                 tc_fence_before();
