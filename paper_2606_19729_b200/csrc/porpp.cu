@@ -40,6 +40,8 @@ __global__ void __launch_bounds__(256, 8) porpp_backup_level_kernel(const float 
     auto preference = [&](int a) {
         const int j = b * A + a;
         const int c0 = __ldg(child_off + j), c1 = __ldg(child_off + j + 1);
+        // issued with the row offsets, not after the CSR walk: one round trip to HBM less per action node
+        const float lp = __ldg(logpi0 + j), r_j = __ldg(R + j);
         float fut = 0.0f;
         for (int c = c0; c < c1; c += 4) {
             int idx[4];
@@ -57,7 +59,7 @@ __global__ void __launch_bounds__(256, 8) porpp_backup_level_kernel(const float 
             for (int u = 0; u < 4; ++u)
                 if (c + u < c1) fut = fmaf(w[u], v[u], fut);
         }
-        const float psi = fmaf(__ldg(logpi0 + j), inv_eta, __ldg(R + j)) + gamma * fut;
+        const float psi = fmaf(lp, inv_eta, r_j) + gamma * fut;
         __stcs(psi_out + j, psi);
         if (psi == psi && (am == 0x7fffffff || psi > m)) {  // first maximum (a ascends); a NaN never wins
             m = psi;
