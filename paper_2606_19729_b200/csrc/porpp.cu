@@ -17,9 +17,10 @@ namespace {
 
 constexpr int kPsiRegs = 4;  // preferences kept in registers per lane (A <= 4 G); beyond that re-read
 
-// G = lanes per belief node: the power of two >= A (capped at 32; A > 32 strides over the lanes),
-// so a warp serves 32 / G belief nodes and narrow action sets (|A| = 4 ... 16) keep every lane busy.
-__global__ void __launch_bounds__(256, 8) porpp_backup_level_kernel(const float *__restrict__ R,
+// G = lanes per belief node: the power of two >= A / 2 (capped at 32; larger A strides over the lanes): a
+// lane takes two action nodes at a time, a warp serves 32 / G belief nodes, narrow action sets
+// (|A| = 4 ... 16) keep every lane busy.
+__global__ void __launch_bounds__(256, 6) porpp_backup_level_kernel(const float *__restrict__ R,
                                                                  const float *__restrict__ logpi0,
                                                                  const int32_t *__restrict__ child_off,
                                                                  const int32_t *__restrict__ child_idx,
@@ -67,12 +68,82 @@ __global__ void __launch_bounds__(256, 8) porpp_backup_level_kernel(const float 
         }
         return psi;
     };
-    if (live) {
+    // The same for TWO action nodes of this lane at once (a and a + G): the loads of a phase (offsets + R +
+    // log pi0; indices + weights of the first four branches; V of the children) are issued for both before
+    // anything is consumed: twice the bytes in flight per thread (the kernel is latency-bound: three
+    // dependent round trips to HBM per action node).  Same arithmetic in the same order as preference().
+    auto preference2 = [&](int a, bool has1, float &psi0_out, float &psi1_out) {
+        int j[2], c0[2], c1[2];
+        float lp[2], r_j[2];
 #pragma unroll
-        for (int slot = 0; slot < kPsiRegs; ++slot) {  // compile-time slots: the array stays in registers
-            const int a = a0 + slot * G;
-            psi_reg[slot] = a < A ? preference(a) : 0.0f;
+        for (int s = 0; s < 2; ++s) {
+            j[s] = b * A + a + s * G;
+            if (s == 0 || has1) {
+                c0[s] = __ldg(child_off + j[s]);
+                c1[s] = __ldg(child_off + j[s] + 1);
+                lp[s] = __ldg(logpi0 + j[s]);
+                r_j[s] = __ldg(R + j[s]);
+            } else {
+                c0[s] = c1[s] = 0;
+                lp[s] = r_j[s] = 0.0f;
+            }
         }
+        int idx[2][4];
+        float w[2][4], v[2][4];
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (c0[s] + u < c1[s]) {
+                    idx[s][u] = __ldg(child_idx + c0[s] + u);
+                    w[s][u] = __ldg(child_w + c0[s] + u);
+                }
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (c0[s] + u < c1[s]) v[s][u] = __ldg(v_next + idx[s][u]);
+        float psi[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            float fut = 0.0f;
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (c0[s] + u < c1[s]) fut = fmaf(w[s][u], v[s][u], fut);
+            for (int c = c0[s] + 4; c < c1[s]; c += 4) {  // rows longer than four branches
+                int idx2[4];
+                float w2[4], v2[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (c + u < c1[s]) {
+                        idx2[u] = __ldg(child_idx + c + u);
+                        w2[u] = __ldg(child_w + c + u);
+                    }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (c + u < c1[s]) v2[u] = __ldg(v_next + idx2[u]);
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (c + u < c1[s]) fut = fmaf(w2[u], v2[u], fut);
+            }
+            psi[s] = fmaf(lp[s], inv_eta, r_j[s]) + gamma * fut;
+            if (s == 0 || has1) {
+                __stcs(psi_out + j[s], psi[s]);
+                if (psi[s] == psi[s] && (am == 0x7fffffff || psi[s] > m)) {  // first maximum (a ascends); a NaN never wins
+                    m = psi[s];
+                    am = a + s * G;
+                }
+            }
+        }
+        psi0_out = psi[0];
+        psi1_out = has1 ? psi[1] : 0.0f;
+    };
+    if (live) {
+        // slots 0 and 1 together, then 2 and 3 (compile-time slots: the array stays in registers)
+        if (a0 < A) preference2(a0, a0 + G < A, psi_reg[0], psi_reg[1]);
+        else psi_reg[0] = psi_reg[1] = 0.0f;
+        if (a0 + 2 * G < A) preference2(a0 + 2 * G, a0 + 3 * G < A, psi_reg[2], psi_reg[3]);
+        else psi_reg[2] = psi_reg[3] = 0.0f;
         for (int a = a0 + kPsiRegs * G; a < A; a += G) preference(a);
     }
     for (int o = G >> 1; o > 0; o >>= 1) {
@@ -107,7 +178,7 @@ cudaError_t launch_porpp_backup_level(const float *R, const float *logpi0, const
                                       int32_t *argmax_out) {
     const int warps_per_cta = 8;
     int G = 1;
-    while (G < A && G < 32) G *= 2;
+    while (2 * G < A && G < 32) G *= 2;  // two action nodes per lane (preference2)
     const int per_cta = warps_per_cta * (32 / G);
     const int grid = (n_belief + per_cta - 1) / per_cta;
     porpp_backup_level_kernel<<<grid, 32 * warps_per_cta, 0, st>>>(R, logpi0, child_off, child_idx, child_w, v_next,
