@@ -32,20 +32,21 @@ __device__ __forceinline__ void mlp_layer_rpt(const float *__restrict__ Wt, cons
     constexpr int kParts = R / RPT;
     for (int item = threadIdx.x; item < kParts * N; item += kThreads) {
         const int part = item / N, j = item - part * N;
-        float acc[RPT];
+        // accumulators as fp32 PAIRS: sm_100's packed FFMA2 (fma.rn.f32x2) does two rows per instruction,
+        // each component an ordinary IEEE fma (the same bits as two fmaf)
+        float2 acc2[RPT / 2];
 #pragma unroll
-        for (int i = 0; i < RPT; ++i) acc[i] = 0.0f;
+        for (int i = 0; i < RPT / 2; ++i) acc2[i] = make_float2(0.0f, 0.0f);
         const float *xp = xin + RPT * part;
         auto fma_row = [&](int k) {
             const float w = __ldg(Wt + (size_t)k * N + j);
+            const float2 w2 = make_float2(w, w);
             const float4 *x4 = reinterpret_cast<const float4 *>(xp + k * R);
 #pragma unroll
             for (int v = 0; v < RPT / 4; ++v) {
                 const float4 x = x4[v];
-                acc[4 * v + 0] = fmaf(w, x.x, acc[4 * v + 0]);
-                acc[4 * v + 1] = fmaf(w, x.y, acc[4 * v + 1]);
-                acc[4 * v + 2] = fmaf(w, x.z, acc[4 * v + 2]);
-                acc[4 * v + 3] = fmaf(w, x.w, acc[4 * v + 3]);
+                acc2[2 * v] = __ffma2_rn(w2, make_float2(x.x, x.y), acc2[2 * v]);
+                acc2[2 * v + 1] = __ffma2_rn(w2, make_float2(x.z, x.w), acc2[2 * v + 1]);
             }
         };
         const int k_end0 = skip_lo < K ? skip_lo : K;
@@ -54,7 +55,10 @@ __device__ __forceinline__ void mlp_layer_rpt(const float *__restrict__ Wt, cons
         if (a_row >= 0) {
             const float w = __ldg(Wt + (size_t)a_row * N + j);
 #pragma unroll
-            for (int i = 0; i < RPT; ++i) acc[i] += w;
+            for (int i = 0; i < RPT / 2; ++i) {
+                acc2[i].x += w;
+                acc2[i].y += w;
+            }
         }
 #pragma unroll 4
         for (int k = skip_hi; k < K; ++k) fma_row(k);
@@ -65,7 +69,8 @@ __device__ __forceinline__ void mlp_layer_rpt(const float *__restrict__ Wt, cons
             float y[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                float t = acc[4 * v + i] + bj;
+                const float2 a2 = acc2[2 * v + (i >> 1)];
+                float t = ((i & 1) ? a2.y : a2.x) + bj;
                 if (!last) {
                     t = act_apply(t, act);
                     if (EMU) t = bf16_round(t);  // the next layer's operand is bf16
