@@ -106,33 +106,46 @@ __global__ void __launch_bounds__(kWidenWarps * 32) pw_widen_kernel(PwArgs a) {
     }
 }
 
-// Exclusive scan of the child sizes (n = G * M_max entries), one CTA.
+// Exclusive scan of the child sizes (n = G * M_max entries), one CTA: every WARP scans a contiguous
+// run of the array 32 entries at a time (coalesced, shuffles only, the running prefix in a register),
+// one block scan of the 32 run totals, then the run offsets are added in a second coalesced sweep.
+// (The first version scanned 1024 entries per round with three block barriers each: 36 us for 2^15
+// entries.  Integer sums, so the grouping does not change a bit.)
 __global__ void __launch_bounds__(1024) pw_seg_scan_kernel(const int32_t *__restrict__ cnt, int n, int32_t *off) {
     __shared__ int warp_tot[32];
-    __shared__ int carry_s;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < n; base += 1024) {
-        const int idx = base + tid;
-        const int v = idx < n ? cnt[idx] : 0;
+    const int per = ((n + 1023) / 1024) * 32;  // entries per warp, a multiple of 32
+    const int lo = min(n, warp * per), hi = min(n, lo + per);
+    int carry = 0;
+    for (int base = lo; base < hi; base += 32) {
+        const int idx = base + lane;
+        const int v = idx < hi ? __ldg(cnt + idx) : 0;
         int incl = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int t = __shfl_up_sync(0xffffffffu, incl, o);
             if (lane >= o) incl += t;
         }
-        if (lane == 31) warp_tot[warp] = incl;
-        __syncthreads();
-        int wp = 0;
-        for (int w = 0; w < warp; ++w) wp += warp_tot[w];
-        const int carry = carry_s;
-        if (idx < n) off[idx] = carry + wp + incl - v;
-        __syncthreads();
-        if (tid == 1023) carry_s = carry + wp + incl;
-        __syncthreads();
+        if (idx < hi) off[idx] = carry + incl - v;
+        carry += __shfl_sync(0xffffffffu, incl, 31);
     }
-    if (tid == 0) off[n] = carry_s;
+    if (lane == 0) warp_tot[warp] = carry;
+    __syncthreads();
+    if (warp == 0) {
+        const int t = warp_tot[lane];
+        int w_incl = t;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, w_incl, o);
+            if (lane >= o) w_incl += u;
+        }
+        warp_tot[lane] = w_incl - t;  // exclusive prefix of the run totals
+        if (lane == 31) off[n] = w_incl;
+    }
+    __syncthreads();
+    const int add = warp_tot[warp];
+    if (add != 0)
+        for (int idx = lo + lane; idx < hi; idx += 32) off[idx] += add;
 }
 
 __global__ void pw_perm_kernel(PwArgs a) {
