@@ -56,6 +56,9 @@ def test_rollout_full_size_sampled(torch_cuda, oracle, cfg_idx, n_pairs):
     kernel = ctx.voila_last_rollout_kernel()
     if bf16:
         assert "rollout_tc2" in kernel, kernel  # what bench.py times
+        # ... in the launch configuration it times: the two-slot kernel for the <= 256-wide generators
+        # (configs 2, 3), the 16-epilogue-warp one-block kernel for config 5
+        assert ("rollout_tc2d_kernel" if cfg_idx in (2, 3) else "rollout_tc2x_kernel") in kernel, kernel
     values, returns, witness = t2n(out["values"]), t2n(out["returns"]), t2n(out["witness"])
     ctx.close()
     assert returns.shape == (Q, P) and np.all(np.isfinite(returns)) and np.all(np.isfinite(witness))
